@@ -1,0 +1,291 @@
+#!/usr/bin/env python
+"""bench.py -- GAME hot path on B200: chromosome x pattern fitness evaluations / second.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
+
+A *step* is one generation of the whole hot path (fused fitness of every chromosome
+on every pattern, rank, stop test, elitism, selection, crossover, mutation) on the config's synthetic
+workload.  `game_evolve(K)` runs K such steps plus the final re-evaluation of the returned population
+(DESIGN G18); the timed region is exactly that call, so `value` counts (K+1)*N*P evaluations and
+`ms_per_step` = time / K (the final evaluation is charged to the steps).  Prints ONE JSON line.
+
+--impl reference times the fp64 CPU oracle (oracle/, as it stands) on the box's host cores on a bounded
+sample of the same workload -- a deliberately slow baseline, not a target.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "chromosome x pattern fitness evaluations per second"
+UNIT = "evals/s"
+
+
+def read_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=d["hbm_gbs"], bf16_tflops=d["bf16_tflops"],
+                    bf16_tflops_sustained=d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                    sm_max_mhz=d.get("sm_max_mhz", 1965.0), source="measured")
+    # fallback stated in B200_PROFILING.md
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks + throttle reasons DURING the timed region (profiling recipe's clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        super().__init__(daemon=True)
+        self.index = index
+        self.samples = []
+        self.stop_flag = False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                f = [x.strip() for x in out.strip().split(",")]
+                if len(f) >= 7:
+                    self.samples.append(f)
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = sorted(float(s[0]) for s in self.samples)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(s[3 + i].lower().startswith("active") for s in self.samples)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.samples[0][1]), "reasons": reasons,
+                "power_w_max": max(float(s[2]) for s in self.samples), "samples": len(self.samples)}
+
+
+def workload_dict(w, path_name):
+    return {"workload": "%s: N=%d F=%d %s d=%d K=%d P=%d" % (w.name, w.N, w.F, "trig" if w.family == 0 else "cheb",
+                                                              w.degree, w.K, w.P),
+            "N": w.N, "F": w.F, "K": w.K, "P": w.P, "error": ["mse", "tmse", "rmse"][w.err], "activation": "sigmoid",
+            "ga": "tournament %d, crossover %.2f, mutation %.2f, elitism %d, init normal" % (
+                w.tournament_size, w.p_crossover, w.p_mutation, w.elitism),
+            "fitness_path": path_name,
+            "l2": "inputs larger than L2 (expansion matrix re-read every step)" if w.N * w.K * 2 > 126e6
+                  else "L2 flushed between timed repeats is not needed: one timed region of K back-to-back steps; working set noted",
+            "parallelism": "single GPU (replicas at N>1)"}
+
+
+def cpu_sample(w, oracle, X, t, seconds_target=15.0):
+    """Time the oracle as it stands on a bounded sample: all N patterns x a few chromosomes."""
+    from paper_1304_0597_b200 import workloads as wl
+    cores = oracle.set_threads(0)
+    pop = wl.uniform_population(max(2 * cores, 4), w.K, w.seed)
+    t0 = time.perf_counter()
+    oracle.fitness(w.family, w.degree, X, t, pop[:cores], act=w.act, err=w.err, R=w.R)
+    probe = time.perf_counter() - t0
+    ps = int(min(pop.shape[0] * 64, max(cores, cores * round(seconds_target / max(probe, 1e-3)))))
+    pop = wl.uniform_population(ps, w.K, w.seed)
+    t0 = time.perf_counter()
+    oracle.fitness(w.family, w.degree, X, t, pop, act=w.act, err=w.err, R=w.R)
+    dt = time.perf_counter() - t0
+    return {"value": w.N * ps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "fp64 oracle fitness (expansion + contraction + error) of %d chromosomes on all N=%d patterns, %.1f s"
+                      % (ps, w.N, dt)}, ps, dt
+
+
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    from paper_1304_0597_b200 import workloads as wl
+    X, t, _ = wl.make(w, lambda X, c: oracle.forward(w.family, w.degree, X, c))
+    cores = oracle.set_threads(0)
+    ps = max(cores, 8)
+    pop = wl.uniform_population(ps, w.K, w.seed)
+
+    def step():
+        oracle.fitness(w.family, w.degree, X, t, pop, act=w.act, err=w.err, R=w.R)
+    for _ in range(args.warmup if args.warmup < 2 else 1):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    val = w.N * ps * args.steps / dt
+    sample = "each step = fp64 oracle fitness of %d chromosomes on all N=%d patterns (bounded sample of the P=%d population)" % (
+        ps, w.N, w.P)
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                      "config": workload_dict(w, "cpu-oracle"),
+                      "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+                      "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                      "gpu_launches": 0}))
+
+
+def run_ours(args, w):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1304_0597_b200 as g
+    from paper_1304_0597_b200 import workloads as wl
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks = read_peaks()
+
+    # replicas: every rank runs the same-shaped problem with its own seed (weak scaling, no data-path collective)
+    from dataclasses import replace
+    wr = replace(w, seed=w.seed + 1000 * rank)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        # planted targets need a forward pass of the planted chromosome: the library's own game_predict
+        holder = {}
+
+        def fwd(X, c0):
+            ctx0 = g.Game(wr.family, wr.degree, wr.F, stream=stream)
+            ctx0.load(torch.from_numpy(X).cuda(), torch.zeros(X.shape[0], device="cuda"))
+            z, y = ctx0.predict(torch.from_numpy(c0).cuda())
+            stream.synchronize()
+            out = (z.cpu().numpy(), y.cpu().numpy())
+            ctx0.destroy()
+            return out
+        X, t, _ = wl.make(wr, fwd)
+        ctx = g.Game(wr.family, wr.degree, wr.F, stream=stream)
+        ctx.set_error(wr.err, wr.R)
+        if args.path != "auto":
+            ctx.set_path({"fp32": g.GAME_PATH_FP32, "tensor": g.GAME_PATH_TENSOR}[args.path])
+        Xp, tp = torch.from_numpy(X).pin_memory(), torch.from_numpy(t).pin_memory()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        ctx.load_host(Xp.numpy(), tp.numpy())
+        e1.record(stream)
+        stream.synchronize()
+        load_ms = e0.elapsed_time(e1)
+        path = ctx.resolved_path(wr.P)
+        path_name = {g.GAME_PATH_FP32: "fp32-ffma", g.GAME_PATH_TENSOR: "tensor-tcgen05-f16"}[path]
+        gp = g.ga_params(P=wr.P, tournament_size=wr.tournament_size, elitism=wr.elitism, init_mode=wr.init_mode,
+                         p_crossover=wr.p_crossover, p_mutation=wr.p_mutation, stop_error=-1.0)
+
+        def barrier():
+            if world > 1:
+                dist.barrier()
+            torch.cuda.synchronize()
+
+        ctx.evolve(max(args.warmup, 3), wr.seed, gp)            # W untimed warm-up steps (also creates the population)
+        ctx.set_kernel_timing(True)
+        ctx.get_kernel_timing()
+        sampler = ClockSampler(local)
+        sampler.start()
+        barrier()
+        launches0 = ctx.launch_count()
+        e0.record(stream)
+        res = ctx.evolve(args.steps, wr.seed, gp)               # exactly K steps (+ the final re-evaluation)
+        e1.record(stream)
+        barrier()
+        sampler.stop_flag = True
+        ms = e0.elapsed_time(e1)
+        launches = ctx.launch_count() - launches0
+        kern_ms, kern_n = ctx.get_kernel_timing()
+        ctx.set_kernel_timing(False)
+        sampler.join()
+        assert res.generations_run == args.steps
+
+        tms = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+        ms_max = float(tms.item())
+        evals = float(w.N) * w.P * (args.steps + 1) * world
+        value = evals / (ms_max * 1e-3)
+
+        # e2e: the same metric through the C ABI with HOST buffers: population in, fitness out, every step
+        pop_host, _, _ = ctx.get_population_host()
+        pop_pin = torch.from_numpy(pop_host).pin_memory()
+        fit_pin = torch.empty(wr.P, dtype=torch.float32).pin_memory()
+        for _ in range(2):
+            ctx.fitness_host(pop_pin.numpy(), fit_pin.numpy())
+        e2e_steps = max(3, min(args.steps, 10))
+        barrier()
+        e0.record(stream)
+        for _ in range(e2e_steps):
+            ctx.fitness_host(pop_pin.numpy(), fit_pin.numpy())
+        e1.record(stream)
+        barrier()
+        e2e_ms = torch.tensor([e0.elapsed_time(e1)], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(e2e_ms, op=dist.ReduceOp.MAX)
+        e2e = {"value": float(w.N) * w.P * e2e_steps * world / (float(e2e_ms.item()) * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": int(wr.P * wr.K * 4), "d2h_bytes_per_step": int(wr.P * 4),
+               "what": "game_fitness_host: population from pinned host memory in, fitness back out, per step; "
+                       "dataset resident (game_load_host took %.1f ms once, incl. H2D of X and the expansion)" % load_ms}
+
+    if rank != 0:
+        return
+    # roofline of the dominant kernel (fused contraction + epilogue)
+    flops = 2.0 * w.N * w.K * w.P
+    avg_s = kern_ms * 1e-3 / max(kern_n, 1)
+    if path == g.GAME_PATH_TENSOR:
+        peak = peaks["bf16_tflops_sustained"]      # fp16 in / fp32 accumulate: same rate as bf16; timed inside a long step
+        roof = {"bound": "tensor", "achieved": flops / avg_s / 1e12, "peak": peak, "unit": "TFLOP/s",
+                "peak_source": "MEASURED_PEAKS.json bf16_tflops_sustained (%s), fp16 = bf16 rate" % peaks["source"]}
+    else:
+        peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+        roof = {"bound": "alu", "achieved": flops / avg_s / 1e12, "peak": peak, "unit": "TFLOP/s",
+                "peak_source": "148 SM x 128 FFMA lanes x 2 flop x sm_max_mhz (derived, DESIGN.md section 7)"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"] = None
+    roof["kernel_ms_avg"] = avg_s * 1e3
+    roof["kernel_launches_timed"] = kern_n
+    roof["kernel_share_of_step"] = kern_ms / ms
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+        Xo, to, _ = wl.make(w, lambda X, c: oracle.forward(w.family, w.degree, X, c))
+        cpu, _, _ = cpu_sample(w, oracle, Xo, to)
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+           "ms_per_step": ms_max / args.steps, "generations_per_sec": args.steps / (ms_max * 1e-3),
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f16 operands, f32 accumulate" if path == g.GAME_PATH_TENSOR else "f32",
+           "data": "synthetic", "config": workload_dict(w, path_name), "clocks": sampler.summary(), "e2e": e2e,
+           "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
+           "best_error": float(res.best_error), "load_ms": load_ms}
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number (1-5); 5 = the largest, the one the north star's target is quoted on")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--path", default="auto", choices=["auto", "fp32", "tensor"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    from paper_1304_0597_b200 import workloads as wl
+    w = wl.config(args.config)
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_ours(args, w)
+
+
+if __name__ == "__main__":
+    main()

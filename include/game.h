@@ -1,0 +1,156 @@
+/*
+ * game.h -- C ABI of libgame_b200: the GAME (Genetic Algorithm Model Experiment) fitness / GA
+ * hot path of Cavuoti et al., arXiv:1304.0597, as hand-written sm_100a CUDA kernels.
+ *
+ * Citations "L<n>" are line numbers of the paper text; "DESIGN Gx/Rx" are the
+ * readings listed in DESIGN.md section 3 for what the paper leaves open.
+ *
+ * Notation (BASELINE.json's): N patterns, F features, d degree, K terms = genes per chromosome,
+ * P chromosomes, G generations.  K = F*(2d+1) for GAME_TRIG, F*(d+1) for GAME_CHEB.
+ *
+ * Conventions
+ *  - Every function returns 0 (GAME_OK) or a positive error code; game_last_error() gives the text.
+ *    No exceptions, no exit(), no global state, no CPU fallback: without a CUDA device every
+ *    compute call fails with GAME_ERR_CUDA.
+ *  - Pointer arguments are marked DEV (CUDA device memory, caller-owned, must stay valid until the
+ *    context's stream has consumed them) or HOST (ordinary or pinned host memory).  The library
+ *    never frees or keeps caller memory; game_load* copies / re-lays what it needs.
+ *  - Calls enqueue work on the context's stream and return without waiting, except where noted.
+ *  - A context is not thread-safe; use one per thread.
+ *  - Fitness values are ERRORS: lower is better (the paper says "maximum fitness", L131, while
+ *    minimising eq. 3-5; DESIGN G12).
+ */
+#ifndef GAME_B200_H
+#define GAME_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct game_ctx game_ctx; /* opaque */
+
+enum { GAME_OK = 0, GAME_ERR_INVALID_ARG = 1, GAME_ERR_NOT_LOADED = 2, GAME_ERR_ALLOC = 3,
+       GAME_ERR_CUDA = 4, GAME_ERR_UNSUPPORTED = 5, GAME_ERR_NONFINITE_INPUT = 6 };
+
+enum { GAME_TRIG = 0, GAME_CHEB = 1 };                 /* expansion family: eq. 8-9 (L95-L103) / eq. 1 with g^j = T_j */
+enum { GAME_ACT_SIGMOID = 0, GAME_ACT_IDENTITY = 1 };  /* DESIGN G4; identity is the paper-literal eq. 2 */
+enum { GAME_ERR_MSE = 0, GAME_ERR_TMSE = 1, GAME_ERR_RMSE = 2 };   /* eq. 4, eq. 10, eq. 5 (L71-L75, L113) */
+enum { GAME_SEL_TOURNAMENT = 0, GAME_SEL_ROULETTE = 1 };           /* L147, L290; DESIGN G14 */
+enum { GAME_INIT_UNIFORM_PM1 = 0, GAME_INIT_NORMAL_PM1 = 1, GAME_INIT_UNIFORM_01 = 2 }; /* L133-L142; DESIGN G13 */
+enum { GAME_ELITE_COPIES_OF_BEST = 0, GAME_ELITE_TOP_E = 1 };      /* L148; DESIGN G17 */
+/* Fitness kernel choice.  FP32: FFMA contraction, |rel err| <= 1e-5 class.  TENSOR: tcgen05 fp16-input /
+ * fp32-accumulate MMA (same 11-bit significand as TF32), 1e-3 class.  AUTO picks by problem shape. */
+enum { GAME_PATH_AUTO = 0, GAME_PATH_FP32 = 1, GAME_PATH_TENSOR = 2 };
+
+/* GA parameters (L275-L291).  Probabilities are per parent pair (crossover, DESIGN G15) and per gene
+ * (mutation, DESIGN G16).  stop_error < 0 disables the error-threshold stop (L219, L287). */
+typedef struct {
+    int   P;                /* population size, >= 2 */
+    int   tournament_size;  /* >= 1 (L290) */
+    int   elitism;          /* 0 <= elitism < P (L291) */
+    int   elite_mode;       /* GAME_ELITE_* */
+    int   selection;        /* GAME_SEL_* */
+    int   init_mode;        /* GAME_INIT_* */
+    float p_crossover;      /* [0,1] (L288) */
+    float p_mutation;       /* [0,1] (L289) */
+    float stop_error;       /* stop when best error <= stop_error; < 0: never */
+} game_ga_params;
+
+typedef struct {
+    int   generations_run;   /* evolution steps performed by this call */
+    int   stopped_on_error;  /* 1 if the last evaluation met stop_error */
+    float best_error;        /* error of the best chromosome of the returned population */
+    int   best_index;        /* its row in the population */
+} game_result;
+
+/* Create a context for one problem shape.  1 <= degree <= 32, F >= 1.  HOST out pointer.
+ * The model: Out(pat) = sum_i G(f_i), G a degree-d expansion of feature f_i (eq. 1-2). */
+int game_create(int family, int degree, int F, game_ctx **out);
+void game_destroy(game_ctx *ctx);   /* synchronises the stream, frees all device memory */
+
+/* K, the number of terms / genes per chromosome (eq. 7 generalised per feature, DESIGN G1). */
+int game_num_terms(const game_ctx *ctx);
+/* Absolute generation counter: number of evolution steps applied to the current population. */
+long long game_generation(const game_ctx *ctx);
+const char *game_last_error(const game_ctx *ctx);   /* HOST string owned by the context */
+
+/* cuda_stream is a cudaStream_t (0 = legacy default stream).  Takes effect for later calls. */
+int game_set_stream(game_ctx *ctx, void *cuda_stream);
+int game_set_activation(game_ctx *ctx, int act);                 /* default GAME_ACT_SIGMOID */
+int game_set_error(game_ctx *ctx, int err_type, float tmse_R);   /* default MSE; R in (0,1) for TMSE (L116) */
+int game_set_path(game_ctx *ctx, int path);                      /* default GAME_PATH_AUTO */
+/* Which path the next fitness call will take for population size P: GAME_PATH_FP32 or GAME_PATH_TENSOR. */
+int game_resolved_path(const game_ctx *ctx, int P);
+
+/* a0 + a1: load the dataset and expand it (L254: "calculate the time consuming trigonometric functions
+ * only once").  X is N x F row-major fp32, targets N fp32.  Builds the device-resident expansion
+ * matrix E (fp32 K x N for the FP32 path, fp16 N x K for the TENSOR path) and rejects NaN/Inf inputs
+ * with GAME_ERR_NONFINITE_INPUT (this check synchronises the stream).  X and targets may be freed once
+ * the stream has passed this call.  game_load: DEV pointers.  game_load_host: HOST pointers, copied with
+ * cudaMemcpyAsync on the context's stream. */
+int game_load(game_ctx *ctx, const float *X, const float *targets, long long N);
+int game_load_host(game_ctx *ctx, const float *X, const float *targets, long long N);
+
+/* a1-a5: out[p] = error of chromosome p over all N patterns (eq. 2-5, eq. 9-10):
+ *   z = sum_k E[n][k] pop[p][k];  y = act(z);  r = t_n - y;  e = r^2 (TMSE: 0 if |r| <= R);
+ *   out[p] = mean_n e  (RMSE: sqrt).
+ * pop is P x K row-major fp32, out is P fp32.  Asynchronous.  The N x P matrix z never reaches HBM.
+ * game_fitness: DEV pointers.  game_fitness_host: HOST pointers; copies pop in, runs, copies out back
+ * and synchronises the stream before returning. */
+int game_fitness(game_ctx *ctx, const float *pop, int P, float *out);
+int game_fitness_host(game_ctx *ctx, const float *pop, int P, float *out);
+
+/* Forward pass of ONE chromosome (the paper's test / run use cases, L127-L129): z_out[n] = Out(pat_n),
+ * y_out[n] = act(z).  genes: K fp32, z_out / y_out: N fp32, either may be NULL.  DEV pointers. fp32. */
+int game_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out);
+
+/* Install a population (P x K fp32, DEV) instead of the random initial one; resets nothing else. */
+int game_set_population(game_ctx *ctx, const float *pop, int P);
+/* Set the absolute generation counter (checkpoint resume; Philox draws are keyed on it). */
+int game_set_generation(game_ctx *ctx, long long generation);
+
+/* The training loop (L217-L220):  [random initial population if none is set, a12]  then up to
+ * `generations` x ( fitness a1-a5, rank a6, stop test a7, elitism a8, selection a9, crossover a10,
+ * mutation a11 ), then one more fitness + rank so the returned fitness belongs to the returned
+ * population (DESIGN G18).  All random decisions come from Philox4x32-10 keyed on
+ * (seed; index, index, absolute generation, purpose) -- DESIGN R0-R6 -- so stepping one generation at
+ * a time equals one long call, and a CPU implementation of the same rules draws identical numbers.
+ * Runs entirely on the device; synchronises the stream before filling *res (HOST, may be NULL).
+ * params is a HOST pointer.  params->P must match an installed population, if any. */
+int game_evolve(game_ctx *ctx, int generations, unsigned long long seed, const game_ga_params *params,
+                game_result *res);
+
+/* Copy out the current population (P x K), its fitness (P) and rank order (P int32, order[0] = best).
+ * Any pointer may be NULL.  fit / order are valid after game_evolve.  DEV pointers; asynchronous. */
+int game_get_population(game_ctx *ctx, float *pop, float *fit, int *order);
+/* HOST pointers; synchronises. */
+int game_get_population_host(game_ctx *ctx, float *pop, float *fit, int *order);
+
+/* Individual operators, exposed so each can be checked bit for bit (all DEV pointers, asynchronous):
+ * game_rank: order = argsort of (fit, index) ascending, NaN last (a6, DESIGN G20).
+ * game_ga_step: next (P x K) from pop (P x K), order and fit for absolute generation `generation`
+ *   (a8-a11; fit is read only by roulette selection).
+ * game_init_population: a12. */
+int game_rank(game_ctx *ctx, const float *fit, int P, int *order);
+int game_ga_step(game_ctx *ctx, const game_ga_params *params, unsigned long long seed, long long generation,
+                 const int *order, const float *fit, const float *pop, float *next);
+int game_init_population(game_ctx *ctx, int init_mode, unsigned long long seed, int P, float *pop);
+
+/* Raw Philox4x32-10 words for n counters (ctr: n x 4 uint32, out: n x 4 uint32, DEV): lets a test
+ * compare the device generator with an independent implementation word for word. */
+int game_philox(game_ctx *ctx, unsigned long long seed, const unsigned int *ctr, int n, unsigned int *out);
+
+/* Number of kernels this context has launched since creation (bench.py reports it). */
+long long game_launch_count(const game_ctx *ctx);
+
+/* Measurement aid: while enabled, every launch of the dominant kernel (the fused contraction +
+ * epilogue of game_fitness / game_evolve) is bracketed by CUDA events on the context's stream.
+ * game_get_kernel_timing synchronises the stream, returns the summed duration in milliseconds and the
+ * number of launches since the last call, and resets both.  HOST out pointers. */
+int game_set_kernel_timing(game_ctx *ctx, int enabled);
+int game_get_kernel_timing(game_ctx *ctx, double *total_ms, long long *launches);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

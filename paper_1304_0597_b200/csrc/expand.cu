@@ -1,0 +1,118 @@
+// a0/a1: dataset checks and feature expansion (eq. 8-9; Chebyshev per DESIGN G7),
+// computed ONCE per game_load as the paper does (L254).  Terms are evaluated in fp64 on the device and
+// rounded once to the storage type, so E is the correctly rounded expansion to within an ulp.
+#include "game_internal.cuh"
+
+namespace game {
+
+__global__ void check_finite_kernel(const float *__restrict__ a, long long na, const float *__restrict__ b,
+                                    long long nb, int *flag)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    long long stride = (long long)gridDim.x * blockDim.x;
+    bool bad = false;
+    for (long long j = i; j < na; j += stride) bad |= !isfinite(a[j]);
+    for (long long j = i; j < nb; j += stride) bad |= !isfinite(b[j]);
+    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(flag, 1);
+}
+
+int launch_check_finite(game_ctx *ctx, const float *X, long long nX, const float *t, long long nT, int *flag_dev)
+{
+    long long n = nX > nT ? nX : nT;
+    int blocks = (int)((n + 255) / 256);
+    if (blocks > ctx->sm_count * 8) blocks = ctx->sm_count * 8;
+    if (blocks < 1) blocks = 1;
+    check_finite_kernel<<<blocks, 256, 0, ctx->stream>>>(X, nX, t, nT, flag_dev);
+    GAME_LAUNCHED(ctx);
+    return GAME_OK;
+}
+
+// One thread per (feature i, pattern n); n is the fastest thread index so the term-major stores
+// ET[k][n] are coalesced.  Term index k = i*B + m, block order [1, cos 1..d, sin 1..d] / [T_0..T_d].
+template <typename OutT, bool PATTERN_MAJOR>
+__global__ void expand_kernel(const float *__restrict__ X, long long N, int F, int family, int d,
+                              OutT *__restrict__ E, long long ld, float *maxabs)
+{
+    long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    int i = blockIdx.y;
+    float local_max = 0.f;
+    if (n < N) {
+        double x = (double)X[n * F + i];
+        int B = family == GAME_TRIG ? 2 * d + 1 : d + 1;
+        int k0 = i * B;
+        auto put = [&](int k, double v) {
+            float f = (float)v;
+            local_max = fmaxf(local_max, fabsf(f));
+            if (PATTERN_MAJOR) E[n * ld + k] = (OutT)f;
+            else E[(long long)k * ld + n] = (OutT)f;
+        };
+        put(k0, 1.0);
+        if (family == GAME_TRIG) {
+            for (int m = 1; m <= d; ++m) {
+                double s, c;
+                sincos((double)m * x, &s, &c);
+                put(k0 + m, c);
+                put(k0 + d + m, s);
+            }
+        } else {
+            double tm1 = 1.0, t0 = x;
+            if (d >= 1) put(k0 + 1, x);
+            for (int m = 2; m <= d; ++m) {
+                double t1 = 2.0 * x * t0 - tm1;
+                put(k0 + m, t1);
+                tm1 = t0;
+                t0 = t1;
+            }
+        }
+    }
+    if (maxabs) {
+        for (int o = 16; o; o >>= 1) local_max = fmaxf(local_max, __shfl_xor_sync(0xffffffffu, local_max, o));
+        if ((threadIdx.x & 31) == 0 && local_max > 0.f)
+            atomicMax((int *)maxabs, __float_as_int(local_max));   // non-negative floats order as ints
+    }
+}
+
+int launch_expand_fp32(game_ctx *ctx)
+{
+    dim3 grid((unsigned)((ctx->N + 255) / 256), (unsigned)ctx->F);
+    expand_kernel<float, false><<<grid, 256, 0, ctx->stream>>>(ctx->X, ctx->N, ctx->F, ctx->family, ctx->degree,
+                                                                ctx->ET, ctx->Npad, nullptr);
+    GAME_LAUNCHED(ctx);
+    return GAME_OK;
+}
+
+int launch_expand_fp16(game_ctx *ctx, float *maxabs_dev)
+{
+    dim3 grid((unsigned)((ctx->N + 255) / 256), (unsigned)ctx->F);
+    expand_kernel<__half, true><<<grid, 256, 0, ctx->stream>>>(ctx->X, ctx->N, ctx->F, ctx->family, ctx->degree,
+                                                                ctx->E16, ctx->Kpad, maxabs_dev);
+    GAME_LAUNCHED(ctx);
+    return GAME_OK;
+}
+
+// Forward pass of one chromosome (the paper's test / run use cases, L127-L129): thread per pattern,
+// coalesced reads of the term-major expansion, fp32 accumulate in ascending k.
+__global__ void predict_kernel(const float *__restrict__ ET, long long Npad, long long N, int K,
+                               const float *__restrict__ genes, int act, float *z_out, float *y_out)
+{
+    extern __shared__ float g[];
+    for (int k = threadIdx.x; k < K; k += blockDim.x) g[k] = genes[k];
+    __syncthreads();
+    long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n >= N) return;
+    float z = 0.f;
+    for (int k = 0; k < K; ++k) z = fmaf(ET[(long long)k * Npad + n], g[k], z);
+    if (z_out) z_out[n] = z;
+    if (y_out) y_out[n] = act == GAME_ACT_SIGMOID ? 1.0f / (1.0f + expf(-z)) : z;
+}
+
+int launch_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out)
+{
+    int blocks = (int)((ctx->N + 255) / 256);
+    predict_kernel<<<blocks, 256, ctx->K * sizeof(float), ctx->stream>>>(ctx->ET, ctx->Npad, ctx->N, ctx->K, genes,
+                                                                        ctx->act, z_out, y_out);
+    GAME_LAUNCHED(ctx);
+    return GAME_OK;
+}
+
+}  // namespace game

@@ -1,0 +1,438 @@
+// The C ABI of libgame_b200 (include/game.h): context management, argument validation and the
+// host-side sequencing of the kernels.  No arithmetic of the method happens on the host.
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "game_internal.cuh"
+
+namespace game {
+
+int fail(game_ctx *ctx, int code, const char *what)
+{
+    if (ctx) ctx->msg = what;
+    return code;
+}
+
+int cuda_fail(game_ctx *ctx, cudaError_t e, const char *where)
+{
+    if (ctx) {
+        ctx->msg = std::string("CUDA error: ") + cudaGetErrorString(e) + " at " + where;
+    }
+    return e == cudaErrorMemoryAllocation ? GAME_ERR_ALLOC : GAME_ERR_CUDA;
+}
+
+template <typename T>
+static void dfree(T *&p)
+{
+    if (p) cudaFree(p);
+    p = nullptr;
+}
+
+static void free_dataset(game_ctx *c)
+{
+    dfree(c->X); dfree(c->t); dfree(c->ET); dfree(c->E16);
+    c->N = 0; c->tensor_ok = false;
+}
+
+static void free_population(game_ctx *c)
+{
+    dfree(c->pop); dfree(c->pop_next); dfree(c->fit); dfree(c->order); dfree(c->rank);
+    dfree(c->rw); dfree(c->rprefix);
+    c->pop_cap = 0; c->have_pop = false; c->have_fit = false; c->P = 0;
+}
+
+static int ensure_population(game_ctx *c, int P)
+{
+    if ((size_t)P <= c->pop_cap) return GAME_OK;
+    free_population(c);
+    size_t n = (size_t)P * c->K;
+    GAME_CUDA(c, cudaMalloc(&c->pop, n * sizeof(float)));
+    GAME_CUDA(c, cudaMalloc(&c->pop_next, n * sizeof(float)));
+    GAME_CUDA(c, cudaMalloc(&c->fit, (size_t)P * sizeof(float)));
+    GAME_CUDA(c, cudaMalloc(&c->order, (size_t)P * sizeof(int)));
+    GAME_CUDA(c, cudaMalloc(&c->rank, (size_t)P * sizeof(int)));
+    GAME_CUDA(c, cudaMalloc(&c->rw, (size_t)P * sizeof(unsigned int)));
+    GAME_CUDA(c, cudaMalloc(&c->rprefix, (size_t)P * sizeof(unsigned long long)));
+    c->pop_cap = P;
+    return GAME_OK;
+}
+
+static int ensure_scratch(game_ctx *c, int P)
+{
+    size_t need = fitness_partial_floats(c, P);
+    if (need > c->partial_cap) {
+        dfree(c->partial);
+        GAME_CUDA(c, cudaMalloc(&c->partial, need * sizeof(float)));
+        c->partial_cap = need;
+    }
+    size_t need16 = (size_t)((P + 255) / 256) * 256 * (size_t)c->Kpad;
+    if (c->tensor_ok && need16 > c->c16_cap) {
+        dfree(c->C16);
+        GAME_CUDA(c, cudaMalloc(&c->C16, need16 * sizeof(__half)));
+        GAME_CUDA(c, cudaMemsetAsync(c->C16, 0, need16 * sizeof(__half), c->stream));
+        c->c16_cap = need16;
+    }
+    return GAME_OK;
+}
+
+static int resolve_path(const game_ctx *c, int P)
+{
+    bool can_tensor = tensor_path_built() && c->tensor_ok;
+    if (c->path == GAME_PATH_FP32) return GAME_PATH_FP32;
+    if (c->path == GAME_PATH_TENSOR) return can_tensor ? GAME_PATH_TENSOR : -1;
+    return (can_tensor && P >= 256 && c->N >= 16384) ? GAME_PATH_TENSOR : GAME_PATH_FP32;
+}
+
+static int run_fitness(game_ctx *c, const float *pop, int P, float *out, const DevState *state)
+{
+    int rc = ensure_scratch(c, P);
+    if (rc) return rc;
+    int path = resolve_path(c, P);
+    if (path < 0) return fail(c, GAME_ERR_UNSUPPORTED, "tensor path unavailable for this dataset (not built, or |E| exceeds fp16 range)");
+    return path == GAME_PATH_TENSOR ? launch_fitness_tensor(c, pop, P, out, state)
+                                    : launch_fitness_fp32(c, pop, P, out, state);
+}
+
+static int validate_params(game_ctx *c, const game_ga_params *g)
+{
+    if (!g) return fail(c, GAME_ERR_INVALID_ARG, "params is NULL");
+    if (g->P < 2) return fail(c, GAME_ERR_INVALID_ARG, "P must be >= 2");
+    if (g->tournament_size < 1) return fail(c, GAME_ERR_INVALID_ARG, "tournament_size must be >= 1");
+    if (g->elitism < 0 || g->elitism >= g->P) return fail(c, GAME_ERR_INVALID_ARG, "need 0 <= elitism < P");
+    if (g->elite_mode != GAME_ELITE_COPIES_OF_BEST && g->elite_mode != GAME_ELITE_TOP_E)
+        return fail(c, GAME_ERR_INVALID_ARG, "bad elite_mode");
+    if (g->selection != GAME_SEL_TOURNAMENT && g->selection != GAME_SEL_ROULETTE)
+        return fail(c, GAME_ERR_INVALID_ARG, "bad selection");
+    if (g->init_mode < 0 || g->init_mode > 2) return fail(c, GAME_ERR_INVALID_ARG, "bad init_mode");
+    if (!(g->p_crossover >= 0.f && g->p_crossover <= 1.f) || !(g->p_mutation >= 0.f && g->p_mutation <= 1.f))
+        return fail(c, GAME_ERR_INVALID_ARG, "probabilities must be in [0,1]");
+    return GAME_OK;
+}
+
+static int load_common(game_ctx *c, const float *X, const float *targets, long long N)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!X || !targets || N < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_load: X, targets must be non-NULL and N >= 1");
+    free_dataset(c);
+    dfree(c->partial); c->partial_cap = 0;
+    const int K = c->K;
+    c->N = N;
+    c->n_slabs = (int)((N + SLAB - 1) / SLAB);
+    c->Npad = (long long)c->n_slabs * SLAB;
+    c->Npad256 = ((N + 255) / 256) * 256;
+    int *flag = nullptr;
+    GAME_CUDA(c, cudaMalloc(&c->X, (size_t)N * c->F * sizeof(float)));
+    GAME_CUDA(c, cudaMalloc(&c->t, (size_t)c->Npad256 * sizeof(float)));
+    GAME_CUDA(c, cudaMalloc(&c->ET, (size_t)K * c->Npad * sizeof(float)));
+    GAME_CUDA(c, cudaMalloc(&flag, 2 * sizeof(int)));
+    GAME_CUDA(c, cudaMemsetAsync(flag, 0, 2 * sizeof(int), c->stream));
+    GAME_CUDA(c, cudaMemsetAsync(c->t, 0, (size_t)c->Npad256 * sizeof(float), c->stream));
+    GAME_CUDA(c, cudaMemsetAsync(c->ET, 0, (size_t)K * c->Npad * sizeof(float), c->stream));
+    GAME_CUDA(c, cudaMemcpyAsync(c->X, X, (size_t)N * c->F * sizeof(float), cudaMemcpyDefault, c->stream));
+    GAME_CUDA(c, cudaMemcpyAsync(c->t, targets, (size_t)N * sizeof(float), cudaMemcpyDefault, c->stream));
+    int rc = launch_check_finite(c, c->X, N * c->F, c->t, N, flag);
+    if (rc) { cudaFree(flag); return rc; }
+    rc = launch_expand_fp32(c);
+    if (rc) { cudaFree(flag); return rc; }
+    if (tensor_path_built()) {
+        size_t n16 = (size_t)c->Npad256 * c->Kpad;
+        GAME_CUDA(c, cudaMalloc(&c->E16, n16 * sizeof(__half)));
+        GAME_CUDA(c, cudaMemsetAsync(c->E16, 0, n16 * sizeof(__half), c->stream));
+        rc = launch_expand_fp16(c, reinterpret_cast<float *>(flag + 1));
+        if (rc) { cudaFree(flag); return rc; }
+    }
+    int h[2] = {0, 0};
+    GAME_CUDA(c, cudaMemcpyAsync(h, flag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+    cudaFree(flag);
+    if (h[0]) {
+        free_dataset(c);
+        return fail(c, GAME_ERR_NONFINITE_INPUT, "game_load: X or targets contain NaN/Inf");
+    }
+    if (tensor_path_built()) {
+        float mx;
+        memcpy(&mx, &h[1], sizeof(float));
+        c->tensor_ok = mx <= 60000.0f;
+        if (c->tensor_ok) {
+            rc = tensor_prepare(c);
+            if (rc) return rc;
+        } else {
+            dfree(c->E16);
+        }
+    }
+    return GAME_OK;
+}
+
+}  // namespace game
+
+using namespace game;
+
+extern "C" {
+
+int game_create(int family, int degree, int F, game_ctx **out)
+{
+    if (!out) return GAME_ERR_INVALID_ARG;
+    *out = nullptr;
+    if ((family != GAME_TRIG && family != GAME_CHEB) || degree < 1 || degree > 32 || F < 1) return GAME_ERR_INVALID_ARG;
+    game_ctx *c = new (std::nothrow) game_ctx();
+    if (!c) return GAME_ERR_ALLOC;
+    c->family = family; c->degree = degree; c->F = F;
+    c->K = F * (family == GAME_TRIG ? 2 * degree + 1 : degree + 1);
+    c->Kpad = ((c->K + TC_KBLK - 1) / TC_KBLK) * TC_KBLK;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaMalloc(&c->state, sizeof(DevState));
+    if (e == cudaSuccess) e = cudaMemset(c->state, 0, sizeof(DevState));
+    if (e != cudaSuccess) {       // no CPU fallback: without a device there is no context
+        cudaGetLastError();
+        delete c;
+        return GAME_ERR_CUDA;
+    }
+    *out = c;
+    return GAME_OK;
+}
+
+void game_destroy(game_ctx *c)
+{
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    free_dataset(c);
+    free_population(c);
+    dfree(c->partial); dfree(c->C16); dfree(c->stage_pop); dfree(c->stage_fit); dfree(c->state);
+    free(c->tmap_E); free(c->tmap_C);
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    delete c;
+}
+
+int game_num_terms(const game_ctx *c) { return c ? c->K : -1; }
+long long game_generation(const game_ctx *c) { return c ? c->generation : -1; }
+const char *game_last_error(const game_ctx *c) { return c ? c->msg.c_str() : "null context"; }
+long long game_launch_count(const game_ctx *c) { return c ? c->launches : -1; }
+
+int game_set_stream(game_ctx *c, void *s)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    c->stream = (cudaStream_t)s;
+    return GAME_OK;
+}
+
+int game_set_activation(game_ctx *c, int act)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (act != GAME_ACT_SIGMOID && act != GAME_ACT_IDENTITY) return fail(c, GAME_ERR_INVALID_ARG, "bad activation");
+    c->act = act;
+    c->have_fit = false;
+    return GAME_OK;
+}
+
+int game_set_error(game_ctx *c, int err, float R)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (err != GAME_ERR_MSE && err != GAME_ERR_TMSE && err != GAME_ERR_RMSE) return fail(c, GAME_ERR_INVALID_ARG, "bad error type");
+    if (err == GAME_ERR_TMSE && !(R > 0.f && R < 1.f)) return fail(c, GAME_ERR_INVALID_ARG, "TMSE threshold R must be in (0,1)");
+    c->err = err; c->R = R;
+    c->have_fit = false;
+    return GAME_OK;
+}
+
+int game_set_path(game_ctx *c, int path)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (path < GAME_PATH_AUTO || path > GAME_PATH_TENSOR) return fail(c, GAME_ERR_INVALID_ARG, "bad path");
+    c->path = path;
+    return GAME_OK;
+}
+
+int game_resolved_path(const game_ctx *c, int P) { return c ? resolve_path(c, P) : -1; }
+
+int game_load(game_ctx *c, const float *X, const float *t, long long N) { return load_common(c, X, t, N); }
+int game_load_host(game_ctx *c, const float *X, const float *t, long long N) { return load_common(c, X, t, N); }
+
+int game_fitness(game_ctx *c, const float *pop, int P, float *out)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!c->N) return fail(c, GAME_ERR_NOT_LOADED, "game_fitness before game_load");
+    if (!pop || !out || P < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_fitness: pop/out NULL or P < 1");
+    return run_fitness(c, pop, P, out, nullptr);
+}
+
+int game_fitness_host(game_ctx *c, const float *pop, int P, float *out)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!c->N) return fail(c, GAME_ERR_NOT_LOADED, "game_fitness_host before game_load");
+    if (!pop || !out || P < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_fitness_host: pop/out NULL or P < 1");
+    if ((size_t)P > c->stage_cap) {
+        dfree(c->stage_pop); dfree(c->stage_fit);
+        GAME_CUDA(c, cudaMalloc(&c->stage_pop, (size_t)P * c->K * sizeof(float)));
+        GAME_CUDA(c, cudaMalloc(&c->stage_fit, (size_t)P * sizeof(float)));
+        c->stage_cap = P;
+    }
+    GAME_CUDA(c, cudaMemcpyAsync(c->stage_pop, pop, (size_t)P * c->K * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    int rc = run_fitness(c, c->stage_pop, P, c->stage_fit, nullptr);
+    if (rc) return rc;
+    GAME_CUDA(c, cudaMemcpyAsync(out, c->stage_fit, (size_t)P * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+    return GAME_OK;
+}
+
+int game_predict(game_ctx *c, const float *genes, float *z_out, float *y_out)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!c->N) return fail(c, GAME_ERR_NOT_LOADED, "game_predict before game_load");
+    if (!genes) return fail(c, GAME_ERR_INVALID_ARG, "game_predict: genes is NULL");
+    return launch_predict(c, genes, z_out, y_out);
+}
+
+int game_set_population(game_ctx *c, const float *pop, int P)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!pop || P < 2) return fail(c, GAME_ERR_INVALID_ARG, "game_set_population: pop NULL or P < 2");
+    int rc = ensure_population(c, P);
+    if (rc) return rc;
+    GAME_CUDA(c, cudaMemcpyAsync(c->pop, pop, (size_t)P * c->K * sizeof(float), cudaMemcpyDefault, c->stream));
+    c->P = P; c->have_pop = true; c->have_fit = false;
+    return GAME_OK;
+}
+
+int game_set_generation(game_ctx *c, long long g)
+{
+    if (!c || g < 0) return GAME_ERR_INVALID_ARG;
+    c->generation = g;
+    return GAME_OK;
+}
+
+int game_evolve(game_ctx *c, int generations, unsigned long long seed, const game_ga_params *gp, game_result *res)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!c->N) return fail(c, GAME_ERR_NOT_LOADED, "game_evolve before game_load");
+    int rc = validate_params(c, gp);
+    if (rc) return rc;
+    if (generations < 0) return fail(c, GAME_ERR_INVALID_ARG, "generations < 0");
+    if (c->have_pop && c->P != gp->P) return fail(c, GAME_ERR_INVALID_ARG, "params->P differs from the installed population");
+    const int P = gp->P;
+    if (!c->have_pop) {
+        rc = ensure_population(c, P);
+        if (rc) return rc;
+        rc = launch_init_population(c, gp->init_mode, seed, P, c->pop);     // a12
+        if (rc) return rc;
+        c->P = P; c->have_pop = true;
+    }
+    GAME_CUDA(c, cudaMemsetAsync(c->state, 0, sizeof(DevState), c->stream));
+    DevState h{};
+    const bool can_stop = gp->stop_error >= 0.f;
+    for (int g = 0; g <= generations; ++g) {
+        rc = run_fitness(c, c->pop, P, c->fit, c->state);                                    // a1-a5
+        if (rc) return rc;
+        rc = launch_rank(c, c->fit, P, c->rank, c->order, c->state, gp->stop_error, true);    // a6, a7
+        if (rc) return rc;
+        if (g == generations) break;
+        if (can_stop && (g & 31) == 31) {        // poll the device-side stop flag now and then
+            GAME_CUDA(c, cudaMemcpyAsync(&h, c->state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+            GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+            if (h.stopped) break;
+        }
+        rc = launch_ga_step(c, gp, seed, (unsigned int)(c->generation + g), c->order, c->fit, c->pop, c->pop_next,
+                            c->state, c->rw, c->rprefix);                                     // a8-a11
+        if (rc) return rc;
+        float *tmp = c->pop; c->pop = c->pop_next; c->pop_next = tmp;
+    }
+    GAME_CUDA(c, cudaMemcpyAsync(&h, c->state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->generation += h.gens_run;
+    c->have_fit = true;
+    if (res) {
+        res->generations_run = h.gens_run;
+        res->stopped_on_error = h.stopped;
+        res->best_error = h.best_error;
+        res->best_index = h.best_index;
+    }
+    return GAME_OK;
+}
+
+static int get_population(game_ctx *c, float *pop, float *fit, int *order, bool sync)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!c->have_pop) return fail(c, GAME_ERR_NOT_LOADED, "no population yet");
+    if ((fit || order) && !c->have_fit) return fail(c, GAME_ERR_NOT_LOADED, "fitness / order are only valid after game_evolve");
+    if (pop) GAME_CUDA(c, cudaMemcpyAsync(pop, c->pop, (size_t)c->P * c->K * sizeof(float), cudaMemcpyDefault, c->stream));
+    if (fit) GAME_CUDA(c, cudaMemcpyAsync(fit, c->fit, (size_t)c->P * sizeof(float), cudaMemcpyDefault, c->stream));
+    if (order) GAME_CUDA(c, cudaMemcpyAsync(order, c->order, (size_t)c->P * sizeof(int), cudaMemcpyDefault, c->stream));
+    if (sync) GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+    return GAME_OK;
+}
+
+int game_get_population(game_ctx *c, float *pop, float *fit, int *order) { return get_population(c, pop, fit, order, false); }
+int game_get_population_host(game_ctx *c, float *pop, float *fit, int *order) { return get_population(c, pop, fit, order, true); }
+
+int game_rank(game_ctx *c, const float *fit, int P, int *order)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!fit || !order || P < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_rank: NULL pointer or P < 1");
+    int *scratch = nullptr;
+    GAME_CUDA(c, cudaMallocAsync(&scratch, (size_t)P * sizeof(int), c->stream));
+    int rc = launch_rank(c, fit, P, scratch, order, nullptr, -1.f, false);
+    cudaFreeAsync(scratch, c->stream);
+    return rc;
+}
+
+int game_ga_step(game_ctx *c, const game_ga_params *gp, unsigned long long seed, long long generation, const int *order,
+                 const float *fit, const float *pop, float *next)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    int rc = validate_params(c, gp);
+    if (rc) return rc;
+    if (!order || !pop || !next || generation < 0) return fail(c, GAME_ERR_INVALID_ARG, "game_ga_step: NULL pointer or generation < 0");
+    if (gp->selection == GAME_SEL_ROULETTE && !fit) return fail(c, GAME_ERR_INVALID_ARG, "roulette selection needs fit");
+    unsigned int *rw = nullptr;
+    unsigned long long *rp = nullptr;
+    if (gp->selection == GAME_SEL_ROULETTE) {
+        GAME_CUDA(c, cudaMallocAsync(&rw, (size_t)gp->P * sizeof(unsigned int), c->stream));
+        GAME_CUDA(c, cudaMallocAsync(&rp, (size_t)gp->P * sizeof(unsigned long long), c->stream));
+    }
+    rc = launch_ga_step(c, gp, seed, (unsigned int)generation, order, fit, pop, next, nullptr, rw, rp);
+    if (rw) cudaFreeAsync(rw, c->stream);
+    if (rp) cudaFreeAsync(rp, c->stream);
+    return rc;
+}
+
+int game_init_population(game_ctx *c, int mode, unsigned long long seed, int P, float *pop)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!pop || P < 1 || mode < 0 || mode > 2) return fail(c, GAME_ERR_INVALID_ARG, "game_init_population: bad argument");
+    return launch_init_population(c, mode, seed, P, pop);
+}
+
+int game_set_kernel_timing(game_ctx *c, int enabled)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    c->timing = enabled != 0;
+    return GAME_OK;
+}
+
+int game_get_kernel_timing(game_ctx *c, double *total_ms, long long *launches)
+{
+    if (!c || !total_ms || !launches) return GAME_ERR_INVALID_ARG;
+    GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+    double tot = 0.0;
+    for (size_t i = 0; i + 1 < c->ev.size(); i += 2) {
+        float ms = 0.f;
+        GAME_CUDA(c, cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]));
+        tot += ms;
+    }
+    *total_ms = tot;
+    *launches = (long long)(c->ev.size() / 2);
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    c->ev.clear();
+    return GAME_OK;
+}
+
+int game_philox(game_ctx *c, unsigned long long seed, const unsigned int *ctr, int n, unsigned int *out)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!ctr || !out || n < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_philox: bad argument");
+    return launch_philox(c, seed, ctr, n, out);
+}
+
+}  // extern "C"

@@ -1,0 +1,132 @@
+// Internal declarations shared by the translation units of libgame_b200 (not part of the ABI).
+#pragma once
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/game.h"
+
+namespace game {
+
+constexpr int SLAB = 128;        // patterns per n-slab: unit of the per-chromosome partial sums
+constexpr int TC_KBLK = 64;      // fp16 elements per 128-byte swizzled smem row (tensor path k-block)
+
+// Device-resident loop state, so a generation needs no host round trip.
+struct DevState {
+    int stopped;          // set by the stop test (a7); later kernels of the loop become no-ops
+    int gens_run;         // evolution steps actually applied
+    float best_error;
+    int best_index;
+};
+
+struct FitnessCfg {
+    int act, err;
+    float R;
+};
+
+}  // namespace game
+
+struct game_ctx {
+    int family = 0, degree = 0, F = 0, K = 0;
+    int act = GAME_ACT_SIGMOID, err = GAME_ERR_MSE, path = GAME_PATH_AUTO;
+    float R = 0.f;
+    cudaStream_t stream = 0;
+    int sm_count = 148;
+
+    // dataset (a0/a1)
+    long long N = 0, Npad = 0;
+    int n_slabs = 0;
+    float *X = nullptr;        // N x F copy (kept for game_predict-style regeneration)
+    float *t = nullptr;        // Npad, zero padded
+    float *ET = nullptr;       // K x Npad fp32, term-major (FP32 path), zero padded
+    __half *E16 = nullptr;     // Npad256 x Kpad fp16, pattern-major (TENSOR path), zero padded
+    long long Npad256 = 0;
+    int Kpad = 0;              // K rounded up to TC_KBLK
+    bool tensor_ok = false;    // E16 built and all |E| representable
+
+    // population / loop state
+    int P = 0;
+    bool have_pop = false, have_fit = false;
+    long long generation = 0;
+    float *pop = nullptr, *pop_next = nullptr, *fit = nullptr;
+    int *order = nullptr, *rank = nullptr;
+    unsigned int *rw = nullptr;              // roulette weights
+    unsigned long long *rprefix = nullptr;   // roulette inclusive prefix sums
+    size_t pop_cap = 0;                      // capacity in chromosomes of the buffers above
+    game::DevState *state = nullptr;
+
+    // scratch
+    float *partial = nullptr;  // n_chunks x Ppad per-chunk error sums
+    size_t partial_cap = 0;
+    __half *C16 = nullptr;     // Ppad128 x Kpad fp16 population copy (TENSOR path)
+    size_t c16_cap = 0;
+    float *stage_pop = nullptr, *stage_fit = nullptr;   // device staging for *_host calls
+    size_t stage_cap = 0;
+    void *tmap_E = nullptr, *tmap_C = nullptr;          // host copies of CUtensorMap (TENSOR path)
+
+    long long launches = 0;
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;     // start/stop pairs recorded around the dominant kernel
+    std::string msg;
+};
+
+namespace game {
+
+int fail(game_ctx *ctx, int code, const char *what);
+int cuda_fail(game_ctx *ctx, cudaError_t e, const char *where);
+
+#define GAME_CUDA(ctx, call)                                                   \
+    do {                                                                       \
+        cudaError_t e__ = (call);                                              \
+        if (e__ != cudaSuccess) return game::cuda_fail(ctx, e__, #call);       \
+    } while (0)
+#define GAME_LAUNCHED(ctx)                                                     \
+    do {                                                                       \
+        ++(ctx)->launches;                                                     \
+        cudaError_t e__ = cudaGetLastError();                                  \
+        if (e__ != cudaSuccess) return game::cuda_fail(ctx, e__, "kernel launch"); \
+    } while (0)
+
+// brackets the dominant kernel with events when ctx->timing is on
+struct KernelTimer {
+    game_ctx *c;
+    explicit KernelTimer(game_ctx *ctx) : c(ctx)
+    {
+        if (!c->timing) return;
+        cudaEvent_t a, b;
+        cudaEventCreate(&a); cudaEventCreate(&b);
+        c->ev.push_back(a); c->ev.push_back(b);
+        cudaEventRecord(a, c->stream);
+    }
+    ~KernelTimer() { if (c->timing) cudaEventRecord(c->ev.back(), c->stream); }
+};
+
+// expand.cu
+int launch_check_finite(game_ctx *ctx, const float *X, long long nX, const float *t, long long nT, int *flag_dev);
+int launch_expand_fp32(game_ctx *ctx);      // X -> ET
+int launch_expand_fp16(game_ctx *ctx, float *maxabs_dev);   // X -> E16
+int launch_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out);
+
+// fitness_fp32.cu
+size_t fitness_partial_floats(const game_ctx *ctx, int P);
+int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state);
+int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, const DevState *state);
+
+// fitness_tc.cu
+bool tensor_path_built();
+int tensor_prepare(game_ctx *ctx);                               // tensor maps etc. after load
+int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state);
+
+// ga.cu
+int launch_init_population(game_ctx *ctx, int mode, unsigned long long seed, int P, float *pop);
+int launch_rank(game_ctx *ctx, const float *fit, int P, int *rank_scratch, int *order, DevState *state,
+                float stop_error, bool update_state);
+int launch_ga_step(game_ctx *ctx, const game_ga_params *gp, unsigned long long seed, unsigned int gen,
+                   const int *order, const float *fit, const float *pop, float *next, DevState *state,
+                   unsigned int *rw, unsigned long long *rprefix);
+int launch_philox(game_ctx *ctx, unsigned long long seed, const unsigned int *ctr, int n, unsigned int *out);
+
+}  // namespace game

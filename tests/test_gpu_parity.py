@@ -1,0 +1,358 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element.
+
+Tolerances: fitness |gpu - ref| <= rtol*|ref| + atol with rtol=1e-5, atol=1e-7 on
+the FP32 path and rtol=1e-3, atol=1e-5 on the TENSOR path; TMSE is discontinuous at |r| = R, so its
+bound is widened by near_p*(R+delta)^2/N where near_p counts the patterns within delta of the tube
+(delta = 1e-5 / 5e-3).  GA decisions (rank, parents, cut points, mutation masks and values, initial
+genes, Philox words) are bit-exact.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+if not torch.cuda.is_available():
+    pytest.skip("no CUDA device", allow_module_level=True)
+
+import paper_1304_0597_b200 as g  # noqa: E402
+from paper_1304_0597_b200 import workloads as wl  # noqa: E402
+
+TRIG, CHEB = 0, 1
+SIGMOID, IDENTITY = 0, 1
+MSE, TMSE, RMSE = 0, 1, 2
+TOL = {g.GAME_PATH_FP32: (1e-5, 1e-7, 1e-5), g.GAME_PATH_TENSOR: (1e-3, 1e-5, 5e-3)}
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def check_fitness(orc, gpu_fit, fam, d, X, t, pop, act, err, R, path, what=""):
+    rtol, atol, delta = TOL[path]
+    if err == TMSE:
+        ref, near = orc.fitness(fam, d, X, t, pop, act=act, err=err, R=R, delta=delta)
+        slack = near * (R + delta) ** 2 / X.shape[0]
+    else:
+        ref = orc.fitness(fam, d, X, t, pop, act=act, err=err, R=R)
+        slack = 0.0
+    got = np.asarray(gpu_fit, dtype=np.float64)
+    bound = rtol * np.abs(ref) + atol + slack
+    bad = np.abs(got - ref) > bound
+    assert not bad.any(), "%s: %d/%d off; worst %g (bound %g) at p=%d" % (
+        what, bad.sum(), bad.size, np.abs(got - ref).max(), bound[np.abs(got - ref).argmax()],
+        int(np.abs(got - ref).argmax()))
+    return ref
+
+
+def make_ctx(fam, d, X, t, act=SIGMOID, err=MSE, R=0.0, path=g.GAME_PATH_AUTO):
+    ctx = g.Game(fam, d, X.shape[1])
+    ctx.set_activation(act)
+    ctx.set_error(err, R)
+    ctx.set_path(path)
+    ctx.load(dev(X), dev(t))
+    return ctx
+
+
+def paths_available(ctx, P):
+    out = [g.GAME_PATH_FP32]
+    ctx.set_path(g.GAME_PATH_TENSOR)
+    if ctx.resolved_path(P) == g.GAME_PATH_TENSOR:
+        out.append(g.GAME_PATH_TENSOR)
+    ctx.set_path(g.GAME_PATH_AUTO)
+    return out
+
+
+# ---- RNG and operators: bit-exact ----------------------------------------------------------------
+def test_philox_words(orc):
+    ctx = g.Game(TRIG, 1, 1)
+    rng = np.random.default_rng(20)
+    ctr = rng.integers(0, 2**32, (513, 4), dtype=np.uint64).astype(np.uint32)
+    ctr[0] = 0
+    ctr[1] = 0xFFFFFFFF
+    for seed in (0, 1, 0xDEADBEEFCAFEF00D, 2**64 - 1):
+        out = ctx.philox(seed, dev(ctr.view(np.int32))).cpu().numpy().view(np.uint32)
+        for i in range(0, 513, 7):
+            ref = orc.philox4x32_10([seed & 0xFFFFFFFF, seed >> 32], ctr[i])
+            assert np.array_equal(out[i], ref), (seed, i)
+
+
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_init_population_bit_exact(orc, mode):
+    ctx = g.Game(CHEB, 8, 11)          # K = 99
+    for seed, P in ((1, 20), (0xABCDEF0123456789, 333)):
+        got = ctx.init_population(mode, seed, P).cpu().numpy()
+        ref = orc.init_population(mode, seed, P, ctx.K)
+        assert np.array_equal(got.view(np.uint32), ref.view(np.uint32))
+
+
+def test_rank_bit_exact(orc):
+    ctx = g.Game(TRIG, 1, 1)
+    rng = np.random.default_rng(21)
+    for P in (1, 2, 20, 255, 256, 257, 2048, 2049, 5000, 8192):
+        fit = rng.random(P).astype(np.float32)
+        if P > 10:
+            fit[rng.integers(0, P, P // 10)] = fit[0]          # ties
+            fit[rng.integers(0, P, 3)] = np.nan
+            fit[rng.integers(0, P, 2)] = np.inf
+            fit[rng.integers(0, P, 2)] = -0.0
+            fit[rng.integers(0, P, 2)] = 0.0
+        got = ctx.rank(dev(fit)).cpu().numpy()
+        assert np.array_equal(got, orc.rank(fit)), P
+
+
+GA_CASES = [
+    dict(P=20, K_fd=(TRIG, 4, 11), tournament_size=3, elitism=2),
+    dict(P=21, K_fd=(CHEB, 8, 11), tournament_size=4, elitism=2, p_mutation=0.2),      # paper's parameters, odd children
+    dict(P=64, K_fd=(CHEB, 1, 1), tournament_size=1, elitism=0, p_crossover=1.0),       # K = 2: only cut = 1
+    dict(P=33, K_fd=(TRIG, 1, 1), tournament_size=9, elitism=5, elite_mode=1, p_crossover=0.5, p_mutation=1.0),
+    dict(P=1024, K_fd=(CHEB, 8, 11), tournament_size=3, elitism=2),
+    dict(P=50, K_fd=(TRIG, 8, 32), selection=1, elitism=1),                              # roulette, K = 544
+    dict(P=4096, K_fd=(CHEB, 6, 16), selection=1, elitism=2, p_mutation=0.0),
+    dict(P=300, K_fd=(CHEB, 12, 64), tournament_size=2, elitism=299),                    # almost all elites
+]
+
+
+@pytest.mark.parametrize("case", GA_CASES)
+def test_ga_step_bit_exact(orc, case):
+    case = dict(case)
+    fam, d, F = case.pop("K_fd")
+    ctx = g.Game(fam, d, F)
+    K, P = ctx.K, case["P"]
+    rng = np.random.default_rng(22)
+    pop = rng.uniform(-1, 1, (P, K)).astype(np.float32)
+    fit = rng.random(P).astype(np.float32)
+    fit[rng.integers(0, P, 2)] = np.nan
+    order = orc.rank(fit)
+    gp_g = g.ga_params(**case)
+    gp_o = orc.GaParams(P=P, tournament_size=gp_g.tournament_size, elitism=gp_g.elitism, elite_mode=gp_g.elite_mode,
+                        selection=gp_g.selection, init_mode=gp_g.init_mode, p_crossover=gp_g.p_crossover,
+                        p_mutation=gp_g.p_mutation, stop_error=-1.0)
+    for seed, gen in ((5, 0), (2**63 + 11, 7), (5, 4000000000)):
+        got = ctx.ga_step(gp_g, seed, gen, dev(order), dev(fit), dev(pop)).cpu().numpy()
+        ref = orc.ga_step(gp_o, seed, gen, order, fit, pop)
+        assert np.array_equal(got.view(np.uint32), ref.view(np.uint32)), (seed, gen)
+
+
+# ---- fitness parity at sizes spanning several tiles and ragged tails -------------------------------
+FIT_SHAPES = [
+    # fam, d, F, N, P
+    (TRIG, 4, 11, 2100, 20),       # config 1's shape
+    (CHEB, 8, 11, 2100, 300),      # config 2's shape, ragged P
+    (CHEB, 6, 16, 1000, 257),
+    (TRIG, 8, 32, 777, 130),       # K = 544
+    (CHEB, 12, 64, 515, 384),      # K = 832
+    (TRIG, 1, 1, 1, 2),            # degenerate: one pattern, K = 3
+    (CHEB, 1, 1, 129, 1),          # one chromosome
+]
+
+
+@pytest.mark.parametrize("shape", FIT_SHAPES)
+@pytest.mark.parametrize("act,err,R", [(SIGMOID, MSE, 0.0), (SIGMOID, TMSE, 0.49), (SIGMOID, RMSE, 0.0),
+                                       (IDENTITY, MSE, 0.0), (IDENTITY, TMSE, 0.3)])
+def test_fitness_parity_small(orc, shape, act, err, R):
+    fam, d, F, N, P = shape
+    rng = np.random.default_rng(23)
+    X = rng.uniform(-1, 1, (N, F)).astype(np.float32)
+    t = rng.integers(0, 2, N).astype(np.float32)
+    K = orc.num_terms(fam, d, F)
+    scale = 1.0 if act == SIGMOID else 1.0 / np.sqrt(K)
+    pop = (rng.uniform(-1, 1, (P, K)) * scale).astype(np.float32)
+    ctx = make_ctx(fam, d, X, t, act, err, R)
+    for path in paths_available(ctx, P):
+        ctx.set_path(path)
+        got = ctx.fitness(dev(pop)).cpu().numpy()
+        check_fitness(orc, got, fam, d, X, t, pop, act, err, R, path, "path %d" % path)
+        # P20: a chromosome's fitness does not depend on where it sits in the population
+        perm = rng.permutation(P)
+        got2 = ctx.fitness(dev(pop[perm])).cpu().numpy()
+        assert np.array_equal(got2.view(np.uint32), got[perm].view(np.uint32))
+
+
+def test_fitness_host_matches_device(orc):
+    fam, d, F, N, P = CHEB, 8, 11, 2100, 64
+    w = wl.config(2).scaled(P=P)
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    pop = wl.uniform_population(P, w.K, 2)
+    ctx = g.Game(fam, d, F)
+    ctx.set_error(TMSE, 0.49)
+    ctx.load_host(X, t)
+    a = ctx.fitness_host(pop)
+    b = ctx.fitness(dev(pop)).cpu().numpy()
+    assert np.array_equal(a.view(np.uint32), b.view(np.uint32))
+    check_fitness(orc, a, fam, d, X, t, pop, SIGMOID, TMSE, 0.49, ctx.resolved_path(P))
+
+
+def test_planted_and_replication(orc):
+    # P8 / P10 on the GPU: the planted chromosome scores ~0; replicated rows leave the error unchanged
+    fam, d, F, N = TRIG, 4, 11, 2100
+    rng = np.random.default_rng(24)
+    X = rng.uniform(-1, 1, (N, F)).astype(np.float32)
+    c0 = rng.standard_normal(orc.num_terms(fam, d, F)).astype(np.float32)
+    _, y = orc.forward(fam, d, X, c0)
+    t = y.astype(np.float32)
+    pop = np.stack([c0, -c0, c0 * 0.5]).astype(np.float32)
+    ctx = make_ctx(fam, d, X, t, SIGMOID, MSE, path=g.GAME_PATH_FP32)
+    f = ctx.fitness(dev(pop)).cpu().numpy()
+    assert 0.0 <= f[0] <= 1e-7 and f[1] > 1e-3 and f[2] > 1e-5
+    ctx4 = make_ctx(fam, d, np.tile(X, (4, 1)), np.tile(t, 4), SIGMOID, MSE, path=g.GAME_PATH_FP32)
+    f4 = ctx4.fitness(dev(pop)).cpu().numpy()
+    assert np.allclose(f4[1:], f[1:], rtol=2e-6)
+
+
+def test_predict_parity(orc):
+    fam, d, F, N = CHEB, 12, 64, 1000
+    rng = np.random.default_rng(25)
+    X = rng.uniform(-1, 1, (N, F)).astype(np.float32)
+    c = (rng.standard_normal(orc.num_terms(fam, d, F)) * 0.1).astype(np.float32)
+    ctx = make_ctx(fam, d, X, np.zeros(N, dtype=np.float32))
+    z, y = ctx.predict(dev(c))
+    zr, yr = orc.forward(fam, d, X, c)
+    assert np.allclose(z.cpu().numpy(), zr, rtol=1e-5, atol=1e-5)
+    assert np.allclose(y.cpu().numpy(), yr, rtol=1e-5, atol=1e-6)
+
+
+def test_error_paths():
+    ctx = g.Game(TRIG, 2, 3)
+    pop = torch.zeros((4, ctx.K), device="cuda")
+    with pytest.raises(g.GameError) as e:
+        ctx.fitness(pop)
+    assert e.value.code == 2                                   # NOT_LOADED
+    X = torch.zeros((10, 3), device="cuda")
+    X[3, 1] = float("nan")
+    with pytest.raises(g.GameError) as e:
+        ctx.load(X, torch.zeros(10, device="cuda"))
+    assert e.value.code == 6                                   # NONFINITE_INPUT
+    with pytest.raises(g.GameError) as e:
+        ctx.set_error(TMSE, 1.5)
+    assert e.value.code == 1
+    ctx.load(torch.zeros((10, 3), device="cuda"), torch.zeros(10, device="cuda"))
+    with pytest.raises(g.GameError) as e:
+        ctx.evolve(1, 1, g.ga_params(P=1))
+    assert e.value.code == 1
+
+
+# ---- whole GA runs, generation by generation, GPU population injected into the oracle (c.4) --------
+def trajectory(orc, w, generations, full_check_every=1, subset=None):
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    ctx = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    path = ctx.resolved_path(w.P)
+    gp_g = g.ga_params(P=w.P, tournament_size=w.tournament_size, elitism=w.elitism, init_mode=w.init_mode,
+                       p_crossover=w.p_crossover, p_mutation=w.p_mutation)
+    gp_o = orc.GaParams(P=w.P, tournament_size=w.tournament_size, elitism=w.elitism, elite_mode=0, selection=0,
+                        init_mode=w.init_mode, p_crossover=w.p_crossover, p_mutation=w.p_mutation, stop_error=-1.0)
+    res = ctx.evolve(0, w.seed, gp_g)                         # init + fitness + rank
+    pop, fit, order = ctx.get_population_host()
+    assert np.array_equal(pop.view(np.uint32), orc.init_population(w.init_mode, w.seed, w.P, w.K).view(np.uint32))
+    best_prev = None
+    rng = np.random.default_rng(99)
+    for gen in range(generations + 1):
+        # (ii) fitness of the GPU's population within tolerance
+        if gen % full_check_every == 0 or gen == generations:
+            rows = np.arange(w.P) if subset is None else np.sort(rng.choice(w.P, subset, replace=False))
+            check_fitness(orc, fit[rows], fam, d, X, t, pop[rows], w.act, w.err, w.R, path, "gen %d" % gen)
+        # (iii) the rank kernel sorted the GPU's own fitness bits exactly
+        assert np.array_equal(order, orc.rank(fit)), gen
+        assert res.best_index == order[0] and res.best_error == fit[order[0]]
+        # P20: elitism never lets the best error worsen, exactly
+        if best_prev is not None:
+            assert fit[order[0]] <= best_prev, gen
+        best_prev = fit[order[0]]
+        if gen == generations:
+            break
+        # (iv) the operators, from the GPU's order, reproduce the GPU's next population bit for bit
+        ref_next = orc.ga_step(gp_o, w.seed, gen, order, fit, pop)
+        res = ctx.evolve(1, w.seed, gp_g)
+        assert res.generations_run == 1 and ctx.generation() == gen + 1
+        pop, fit, order = ctx.get_population_host()
+        assert np.array_equal(pop.view(np.uint32), ref_next.view(np.uint32)), gen
+    return ctx, pop, fit, order
+
+
+def test_trajectory_config1_full(orc):
+    trajectory(orc, wl.config(1), 100)
+
+
+def test_trajectory_config2_scaled(orc):
+    # config 2's data and GA parameters, full P, fewer generations (the oracle needs ~0.2 s each)
+    trajectory(orc, wl.config(2), 24, full_check_every=4)
+
+
+def test_trajectory_paper_parameters(orc):
+    # the paper's own settings (L282-L291): tournament 4, mutation 0.2, P = 23 (eq. 6), TMSE 0.49
+    w = wl.config(1)
+    from dataclasses import replace
+    trajectory(orc, replace(w, P=23, tournament_size=4, p_mutation=0.2), 20)
+
+
+def test_resume_and_single_call_agree(orc):
+    # P22: evolve(a); evolve(b) == evolve(a+b), bit for bit; and == the step-by-step run
+    w = wl.config(1)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    gp = g.ga_params(P=w.P)
+    a = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    ra = a.evolve(30, w.seed, gp)
+    b = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    b.evolve(12, w.seed, gp)
+    rb = b.evolve(18, w.seed, gp)
+    pa, fa, oa = a.get_population_host()
+    pb, fb, ob = b.get_population_host()
+    assert a.generation() == b.generation() == 30 and ra.generations_run == 30 and rb.generations_run == 18
+    assert np.array_equal(pa.view(np.uint32), pb.view(np.uint32))
+    assert np.array_equal(fa.view(np.uint32), fb.view(np.uint32)) and np.array_equal(oa, ob)
+    assert ra.best_error == rb.best_error and ra.best_index == rb.best_index
+    # checkpoint: export, import into a fresh context, continue
+    c = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    p12 = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    p12.evolve(12, w.seed, gp)
+    pop12, _, _ = p12.get_population()
+    c.set_population(pop12)
+    c.set_generation(12)
+    c.evolve(18, w.seed, gp)
+    pc, fc, oc = c.get_population_host()
+    assert np.array_equal(pc.view(np.uint32), pa.view(np.uint32)) and np.array_equal(oc, oa)
+
+
+def test_stop_criterion(orc):
+    w = wl.config(1)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    gp = g.ga_params(P=w.P)
+    a = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    hist = [a.evolve(0, w.seed, gp).best_error]              # hist[i] = best error after i generations
+    for _ in range(80):
+        hist.append(a.evolve(1, w.seed, gp).best_error)
+    target = hist[40]
+    first = next(i for i, h in enumerate(hist) if h <= target)           # generations needed
+    b = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    gp_stop = g.ga_params(P=w.P, stop_error=float(target))
+    r = b.evolve(80, w.seed, gp_stop)
+    assert r.stopped_on_error == 1 and r.generations_run == first and b.generation() == first
+    assert r.best_error <= target
+    pop, fit, order = b.get_population_host()
+    assert fit[order[0]] == r.best_error
+
+
+# ---- BASELINE.json's full sizes, in the launch configuration bench.py times: sampled outputs ---------
+@pytest.mark.parametrize("cfg,nsample", [(3, 24), (4, 8), (5, 8)])
+def test_full_size_sampled(orc, cfg, nsample):
+    w = wl.config(cfg)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    ctx = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    path = ctx.resolved_path(w.P)
+    gp = g.ga_params(P=w.P)
+    ctx.evolve(2, w.seed, gp)                                 # init + two real generations at full size
+    pop, fit, order = ctx.get_population_host()
+    assert np.array_equal(order, orc.rank(fit))
+    rng = np.random.default_rng(cfg)
+    rows = np.unique(np.concatenate([[0, 1, order[0], order[-1], w.P - 1], rng.choice(w.P, nsample, replace=False)]))
+    check_fitness(orc, fit[rows], fam, d, X, t, pop[rows], w.act, w.err, w.R, path, "cfg %d" % cfg)
+    # stand-alone fitness call on the same population gives the same bits as the loop's
+    f2 = ctx.fitness(dev(pop)).cpu().numpy()
+    assert np.array_equal(f2.view(np.uint32), fit.view(np.uint32))
+    # properties that hold at any size: elites are copies of the previous winner -> rows 0,1 identical
+    assert np.array_equal(pop[0], pop[1]) and fit[0] == fit[1]
+    assert np.all(np.abs(pop) <= 1.0) and np.all(np.isfinite(fit)) and np.all(fit >= 0)
