@@ -168,7 +168,7 @@ static int pick_slabs_per_cta(const game_ctx *ctx, int P)
 size_t fitness_partial_floats(const game_ctx *ctx, int P)
 {
     size_t Ppad = (size_t)((P + 255) / 256) * 256;
-    return (size_t)ctx->n_slabs * Ppad;     // worst case: one row per slab
+    return (size_t)(ctx->n_slabs + 2) * Ppad;     // worst case: one row per slab (tensor path pads N to 256)
 }
 
 int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, const DevState *state)

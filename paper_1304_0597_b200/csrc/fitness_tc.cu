@@ -1,10 +1,447 @@
-// placeholder until the tcgen05 kernel lands: reports the tensor path as not built
+// a2-a5, TENSOR path: the N x K x P contraction on the 5th-generation tensor cores (tcgen05.mma,
+// kind::f16: fp16 operands -- the same 11-bit significand as TF32 at twice the rate and half the bytes --
+// fp32 accumulate in TMEM) with the activation, error and per-chromosome reduction fused in the epilogue
+// (eq. 2-5, eq. 9-10).  z never leaves the SM.
+//
+// Orientation: chromosomes sit on the MMA's M axis (TMEM lanes), patterns on its N axis (TMEM columns),
+// so an epilogue thread owns ONE chromosome, walks its row of the accumulator and sums the errors of the
+// tile's patterns in a register: no shuffles, targets are a shared-memory broadcast.
+//
+// Persistent, warp-specialised CTAs (one per SM, or one CTA pair per two SMs with cta_group::2):
+//   warp 0      TMA producer: 128B-swizzled [rows x 64] fp16 boxes of C (A operand) and E (B operand)
+//               into a ring of shared-memory stages, completion on mbarriers
+//   warp 1      TMEM allocator and the single-thread MMA issuer; tcgen05.commit frees stages and
+//               publishes finished accumulators
+//   warps 2-9   epilogue: tcgen05.ld the accumulator (two 128x256 fp32 buffers = all 512 TMEM columns, so
+//               the epilogue of tile i overlaps the MMAs of tile i+1), sigmoid, error, row sum, one
+//               coalesced store per warp into partial[slab][p]
+// Tiles are ordered chromosome-block fastest so CTAs running together share the same E tile out of L2.
+// finalize_kernel (fitness_fp32.cu) then adds the slabs in fixed order: no float atomics, bit-reproducible,
+// and a chromosome's result does not depend on its row (DESIGN P20).
+#include <cuda.h>
+
 #include "game_internal.cuh"
+
 namespace game {
-bool tensor_path_built() { return false; }
-int tensor_prepare(game_ctx *) { return GAME_OK; }
-int launch_fitness_tensor(game_ctx *ctx, const float *, int, float *, const DevState *)
+
+constexpr int BM = 128;            // chromosomes per CTA  = TMEM lanes
+constexpr int BN = 256;            // patterns per tile    = TMEM columns of one accumulator
+constexpr int BKB = TC_KBLK;       // 64 fp16 = one 128-byte swizzle row per k-block
+constexpr int UMMA_K = 16;
+constexpr int A_BYTES = BM * BKB * 2;
+constexpr int N_EPI_WARPS = 8;
+constexpr int TC_THREADS = 64 + 32 * N_EPI_WARPS;
+
+template <int CG> struct Cfg {
+    static constexpr int BNL = BN / CG;                 // pattern rows this CTA stages
+    static constexpr int B_BYTES = BNL * BKB * 2;
+    static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+    static constexpr int STAGES = CG == 1 ? 4 : 6;
+    static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/ + 2 * BN * 4 /*targets*/;
+};
+
+// ---- PTX wrappers ------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {
-    return fail(ctx, GAME_ERR_UNSUPPORTED, "tensor path not built");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// arrive on the barrier at the same offset in CTA `rank` of the cluster
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t rank)
+{
+    asm volatile("{\n\t.reg .b32 ra;\n\tmapa.shared::cluster.u32 ra, %0, %1;\n\t"
+                 "mbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n\t}" ::"r"(bar), "r"(rank) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok = 0;
+    for (uint32_t spin = 0; !ok; ++spin) {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (spin > (1u << 22)) __trap();      // a protocol bug must fail loudly, not hang the device
+    }
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+template <int CG>
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, int c0, int c1, uint32_t bar)
+{
+    if (CG == 1) {
+        asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                     ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
+    } else {    // both CTAs of the pair issue; the bytes are accounted on the LEADER's barrier (rank 0)
+        asm volatile("{\n\t.reg .b32 rb;\n\tmapa.shared::cluster.u32 rb, %4, 0;\n\t"
+                     "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [rb];\n\t}"
+                     ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
+    }
+}
+
+template <int CG> __device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t cols)
+{
+    if (CG == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    } else {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+}
+template <int CG> __device__ __forceinline__ void tmem_dealloc(uint32_t addr, uint32_t cols)
+{
+    if (CG == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
+    else asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
+}
+
+// D[tmem] (+)= A[smem] . B[smem]^T, both operands K-major
+template <int CG>
+__device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
+{
+    if (CG == 1) {
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                     "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+                     ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+    } else {
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                     "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+                     ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+    }
+}
+
+// arrive on `bar` (same offset in every CTA of the pair) once all MMAs issued so far have completed
+template <int CG> __device__ __forceinline__ void umma_commit(uint32_t bar)
+{
+    if (CG == 1) {
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+    } else {
+        asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                     ::"r"(bar), "h"((unsigned short)3) : "memory");
+    }
+}
+
+// shared-memory matrix descriptor: K-major tile of [rows x 64] fp16, 128-byte swizzle, 8-row groups 1024 B apart
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t addr)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((addr & 0x3FFFF) >> 4);          // start address, 16-byte units        bits [0,14)
+    d |= (uint64_t)1 << 16;                          // leading byte offset (unused here)   bits [16,30)
+    d |= (uint64_t)(1024 >> 4) << 32;                // stride byte offset: 8 rows x 128 B  bits [32,46)
+    d |= (uint64_t)1 << 46;                          // descriptor version (sm_100)         bits [46,48)
+    d |= (uint64_t)2 << 61;                          // layout: SWIZZLE_128B                bits [61,64)
+    return d;
+}
+
+// instruction descriptor, kind::f16: fp16 x fp16 -> fp32, both K-major, M x N tile
+__host__ __device__ constexpr uint32_t make_idesc(int M, int N)
+{
+    return (1u << 4)                 // D format: F32
+         | (0u << 7) | (0u << 10)    // A, B format: F16
+         | (0u << 15) | (0u << 16)   // A, B major: K
+         | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+template <int ACT, bool TMSE>
+__device__ __forceinline__ float err_of(float z, float t, float R)
+{
+    float y = ACT == GAME_ACT_SIGMOID ? rcp_approx(1.0f + ex2_approx(z * -1.4426950408889634f)) : z;
+    float r = t - y;
+    float e = r * r;
+    if (TMSE) e = fabsf(r) > R ? e : 0.f;
+    return e;
+}
+
+// ---- the kernel -----------------------------------------------------------------------------------------
+template <int CG, int ACT, bool TMSE>
+__global__ void __launch_bounds__(TC_THREADS, 1)
+fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmE,
+                  int n_tiles, int m_blocks, int k_blocks, long long N, const float *__restrict__ tgt, float R,
+                  float *__restrict__ partial, int Ppad, const DevState *state)
+{
+    using C = Cfg<CG>;
+    if (state && state->stopped) return;          // uniform across the grid: nobody has touched a barrier yet
+
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t *gbase = smem_raw + (base - smem_u32(smem_raw));
+    const uint32_t bar0 = base + C::STAGES * C::STAGE_BYTES;
+    auto full_bar = [&](int s) { return bar0 + 8u * s; };
+    auto empty_bar = [&](int s) { return bar0 + 8u * (C::STAGES + s); };
+    auto tfull_bar = [&](int a) { return bar0 + 8u * (2 * C::STAGES + a); };
+    auto tempty_bar = [&](int a) { return bar0 + 8u * (2 * C::STAGES + 2 + a); };
+    const uint32_t tmem_slot = bar0 + 8u * (2 * C::STAGES + 4);
+    volatile uint32_t *tmem_slot_g = reinterpret_cast<volatile uint32_t *>(gbase + C::STAGES * C::STAGE_BYTES + 8 * (2 * C::STAGES + 4));
+    float *tgt_s = reinterpret_cast<float *>(gbase + C::STAGES * C::STAGE_BYTES + 256);   // [2][BN]
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint32_t cta_rank = 0;
+    if (CG == 2) asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(cta_rank));
+    const int pair = blockIdx.x / CG, n_pairs = gridDim.x / CG;
+    const int total_tiles = n_tiles * m_blocks;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < C::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), CG * N_EPI_WARPS); }
+        fence_barrier_init();
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmC) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmE) : "memory");
+    }
+    if (warp == 1) tmem_alloc<CG>(tmem_slot, 512);
+    tc_fence_before();
+    if (CG == 2) { asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+    else __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_g;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            int s = 0; uint32_t ph = 0;
+            for (int tile = pair; tile < total_tiles; tile += n_pairs) {
+                const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
+                const int rowC = (m_blk * CG + (int)cta_rank) * BM;
+                const int rowE = n_tile * BN + (int)cta_rank * C::BNL;
+                for (int kb = 0; kb < k_blocks; ++kb) {
+                    mbar_wait(empty_bar(s), ph ^ 1);
+                    const uint32_t sa = base + s * C::STAGE_BYTES, sb = sa + A_BYTES;
+                    if (CG == 1 || cta_rank == 0) mbar_expect_tx(full_bar(s), CG * C::STAGE_BYTES);
+                    tma_load_2d<CG>(sa, &tmC, kb * BKB, rowC, full_bar(s));
+                    tma_load_2d<CG>(sb, &tmE, kb * BKB, rowE, full_bar(s));
+                    if (++s == C::STAGES) { s = 0; ph ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (one thread; leader CTA only when paired) =====
+        if (lane == 0 && cta_rank == 0) {
+            constexpr uint32_t idesc = make_idesc(BM * CG, BN);
+            int s = 0; uint32_t ph = 0;
+            int acc = 0; uint32_t aph = 0;
+            for (int tile = pair; tile < total_tiles; tile += n_pairs) {
+                mbar_wait(tempty_bar(acc), aph ^ 1);          // epilogue has drained this accumulator
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
+                for (int kb = 0; kb < k_blocks; ++kb) {
+                    mbar_wait(full_bar(s), ph);               // operands have landed
+                    tc_fence_after();
+                    const uint32_t sa = base + s * C::STAGE_BYTES, sb = sa + A_BYTES;
+                    const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sb);
+#pragma unroll
+                    for (int k = 0; k < BKB / UMMA_K; ++k) {
+                        // advance 16 fp16 = 32 bytes inside the swizzle row: +2 in 16-byte units
+                        umma_f16<CG>(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
+                    }
+                    umma_commit<CG>(empty_bar(s));            // stage reusable when these MMAs retire
+                    if (++s == C::STAGES) { s = 0; ph ^= 1; }
+                }
+                umma_commit<CG>(tfull_bar(acc));              // accumulator complete
+                if (++acc == 2) { acc = 0; aph ^= 1; }
+            }
+        }
+    } else {
+        // ===== epilogue warps =====
+        const int ew = warp - 2;
+        const int quarter = warp & 3;          // TMEM lane quarter this warp may touch
+        const int half = ew >> 2;              // which 128 columns of the 256-column tile
+        const int et = threadIdx.x - 64;
+        int acc = 0; uint32_t aph = 0;
+        for (int tile = pair; tile < total_tiles; tile += n_pairs) {
+            const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
+            const long long n0 = (long long)n_tile * BN;
+            tgt_s[acc * BN + et] = tgt[n0 + et];
+            asm volatile("bar.sync 1, %0;" ::"n"(32 * N_EPI_WARPS) : "memory");
+            long long rem = N - (n0 + half * 128);
+            const int valid = rem >= 128 ? 128 : (rem > 0 ? (int)rem : 0);
+            mbar_wait(tfull_bar(acc), aph);
+            tc_fence_after();
+            const uint32_t t0 = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(acc * BN + half * 128);
+            const float *ts = tgt_s + acc * BN + half * 128;
+            float sum = 0.f;
+#pragma unroll 1
+            for (int c = 0; c < 4; ++c) {
+                if (c * 32 >= valid) break;
+                uint32_t v[32];
+                tmem_ld32(t0 + c * 32, v);
+                tmem_ld_wait();
+                if (c * 32 + 32 <= valid) {
+#pragma unroll
+                    for (int j = 0; j < 32; j += 4) {
+                        float4 t4 = *reinterpret_cast<const float4 *>(ts + c * 32 + j);
+                        sum += err_of<ACT, TMSE>(__uint_as_float(v[j]), t4.x, R);
+                        sum += err_of<ACT, TMSE>(__uint_as_float(v[j + 1]), t4.y, R);
+                        sum += err_of<ACT, TMSE>(__uint_as_float(v[j + 2]), t4.z, R);
+                        sum += err_of<ACT, TMSE>(__uint_as_float(v[j + 3]), t4.w, R);
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        float e = err_of<ACT, TMSE>(__uint_as_float(v[j]), ts[c * 32 + j], R);
+                        sum += (c * 32 + j < valid) ? e : 0.f;
+                    }
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+                if (CG == 1) mbar_arrive(tempty_bar(acc));
+                else mbar_arrive_cluster(tempty_bar(acc), 0);
+            }
+            const int p = (m_blk * CG + (int)cta_rank) * BM + quarter * 32 + lane;
+            partial[(long long)(n_tile * 2 + half) * Ppad + p] = sum;
+            if (++acc == 2) { acc = 0; aph ^= 1; }
+        }
+    }
+
+    // teardown: everyone done with TMEM before it is released
+    tc_fence_before();
+    if (CG == 2) { asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+    else __syncthreads();
+    if (warp == 1) { __syncwarp(); tc_fence_after(); tmem_dealloc<CG>(tmem_base, 512); }
+}
+
+// pop fp32 [P][K] -> C16 fp16 [Ppad][Kpad] (round to nearest even, clamped to the finite fp16 range)
+__global__ void pop_to_f16_kernel(const float *__restrict__ pop, int P, int K, int Kpad, __half *__restrict__ C16,
+                                  const DevState *state)
+{
+    if (state && state->stopped) return;
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= (long long)P * K) return;
+    int p = (int)(i / K), k = (int)(i % K);
+    float v = fminf(fmaxf(pop[i], -65504.f), 65504.f);
+    C16[(long long)p * Kpad + k] = __float2half_rn(v);
+}
+
+// ---- host side ------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// [rows][Kpad] fp16 row-major, boxes of [box_rows][64], 128-byte swizzle
+static int encode_map(game_ctx *ctx, CUtensorMap *m, void *ptr, long long rows, int Kpad, int box_rows)
+{
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return fail(ctx, GAME_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+    cuuint64_t dims[2] = {(cuuint64_t)Kpad, (cuuint64_t)rows};
+    cuuint64_t strides[1] = {(cuuint64_t)Kpad * 2};
+    cuuint32_t box[2] = {(cuuint32_t)BKB, (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, ptr, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(ctx, GAME_ERR_CUDA, "cuTensorMapEncodeTiled failed");
+    return GAME_OK;
+}
+
+bool tensor_path_built() { return true; }
+
+static int cta_group(const game_ctx *) {
+    static int cg = 0;
+    if (!cg) {
+        const char *e = getenv("GAME_TC_CTA_GROUP");      // measurement knob; default chosen by measurement
+        cg = (e && e[0] == '2') ? 2 : 1;
+    }
+    return cg;
+}
+
+int tensor_prepare(game_ctx *ctx)
+{
+    if (!ctx->tmap_E) ctx->tmap_E = aligned_alloc(64, sizeof(CUtensorMap));
+    if (!ctx->tmap_C) ctx->tmap_C = aligned_alloc(64, sizeof(CUtensorMap));
+    if (!ctx->tmap_E || !ctx->tmap_C) return fail(ctx, GAME_ERR_ALLOC, "tensor map allocation failed");
+    const int cg = cta_group(ctx);
+    return encode_map(ctx, (CUtensorMap *)ctx->tmap_E, ctx->E16, ctx->Npad256, ctx->Kpad, BN / cg);
+}
+
+template <int CG, int ACT, bool TMSE>
+static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, const DevState *state)
+{
+    using C = Cfg<CG>;
+    auto kern = fitness_tc_kernel<CG, ACT, TMSE>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        GAME_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+        attr_set = true;
+    }
+    long long total = (long long)n_tiles * m_blocks;
+    int pairs = ctx->sm_count / CG;
+    if (pairs > total) pairs = (int)total;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)(pairs * CG));
+    cfg.blockDim = dim3(TC_THREADS);
+    cfg.dynamicSmemBytes = C::SMEM;
+    cfg.stream = ctx->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    KernelTimer timer(ctx);
+    GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, *(const CUtensorMap *)ctx->tmap_E, n_tiles,
+                                      m_blocks, ctx->Kpad / BKB, ctx->N, (const float *)ctx->t, ctx->R, ctx->partial, Ppad, state));
+    return GAME_OK;
+}
+
+int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state)
+{
+    const int cg = cta_group(ctx);
+    const int Ppad = ((P + 255) / 256) * 256;
+    const int n_tiles = (int)(ctx->Npad256 / BN);
+    const int m_blocks = Ppad / (BM * cg);
+    long long n = (long long)P * ctx->K;
+    pop_to_f16_kernel<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(pop, P, ctx->K, ctx->Kpad, ctx->C16, state);
+    GAME_LAUNCHED(ctx);
+    int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_C, ctx->C16, Ppad, ctx->Kpad, BM);
+    if (rc) return rc;
+    const bool tmse = ctx->err == GAME_ERR_TMSE;
+    const bool sig = ctx->act == GAME_ACT_SIGMOID;
+#define GAME_TC_DISPATCH(CGV)                                                                              \
+    rc = sig ? (tmse ? launch_variant<CGV, GAME_ACT_SIGMOID, true>(ctx, n_tiles, m_blocks, Ppad, state)       \
+                     : launch_variant<CGV, GAME_ACT_SIGMOID, false>(ctx, n_tiles, m_blocks, Ppad, state))     \
+             : (tmse ? launch_variant<CGV, GAME_ACT_IDENTITY, true>(ctx, n_tiles, m_blocks, Ppad, state)      \
+                     : launch_variant<CGV, GAME_ACT_IDENTITY, false>(ctx, n_tiles, m_blocks, Ppad, state))
+    if (cg == 2) { GAME_TC_DISPATCH(2); } else { GAME_TC_DISPATCH(1); }
+#undef GAME_TC_DISPATCH
+    if (rc) return rc;
+    ++ctx->launches;
+    return launch_finalize(ctx, (int)(ctx->Npad256 / SLAB), Ppad, P, out, state);
+}
+
 }  // namespace game
