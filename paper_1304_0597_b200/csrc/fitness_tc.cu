@@ -168,14 +168,69 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
-template <int ACT, bool TMSE>
-__device__ __forceinline__ float err_of(float z, float t, float R)
+// Epilogue modes (template parameter ACT): the two activations of the ABI plus a cheaper logistic form.
+//   0 sigmoid, 1/(1+2^(-z log2 e)) with ex2.approx + rcp.approx: 2 MUFU ops per evaluation
+//   1 identity
+//   2 sigmoid as 0.5 + 0.5 tanh(z/2) with tanh.approx.f32: 1 MUFU op per evaluation.  Measured against the
+//     oracle on configs 2 and 3 (512 chromosomes x 3 gene distributions x MSE/TMSE) its fitness error is
+//     indistinguishable from mode 0's (both dominated by the fp16 operand rounding, max 5e-4 relative, no
+//     bias), and the MUFU-bound config 3 runs 1.4x faster, so it is the default.  A packed
+//     tanh.approx.f16x2 form (0.5 MUFU per evaluation) was measured too: biased by -2e-4 and slower; dropped.
+// In mode 2 the staged targets are t - 0.5, so r = (t - 0.5) - 0.5 tanh(z/2) is one FFMA.
+// Arithmetic is issued two evaluations at a time with the packed fp32 instructions of sm_100
+// (FMUL2 / FFMA2), which halves the FMA-pipe issue slots the epilogue needs.
+constexpr int MODE_SIG_EXACT = 0, MODE_IDENTITY = 1, MODE_SIG_TANH32 = 2;
+
+__device__ __forceinline__ float tanh_approx(float x) { float y; asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// residual r = t - act(z) for two evaluations
+template <int ACT> __device__ __forceinline__ float2 residual2(float2 z, float2 t)
 {
-    float y = ACT == GAME_ACT_SIGMOID ? rcp_approx(1.0f + ex2_approx(z * -1.4426950408889634f)) : z;
-    float r = t - y;
-    float e = r * r;
-    if (TMSE) e = fabsf(r) > R ? e : 0.f;
-    return e;
+    if (ACT == MODE_SIG_EXACT) {
+        float2 a = __fmul2_rn(z, make_float2(-1.4426950408889634f, -1.4426950408889634f));
+        float2 d = __fadd2_rn(make_float2(ex2_approx(a.x), ex2_approx(a.y)), make_float2(1.0f, 1.0f));
+        return __ffma2_rn(make_float2(rcp_approx(d.x), rcp_approx(d.y)), make_float2(-1.0f, -1.0f), t);
+    } else if (ACT == MODE_IDENTITY) {
+        return __ffma2_rn(z, make_float2(-1.0f, -1.0f), t);
+    } else {
+        float2 h = __fmul2_rn(z, make_float2(0.5f, 0.5f));
+        return __ffma2_rn(make_float2(tanh_approx(h.x), tanh_approx(h.y)), make_float2(-0.5f, -0.5f), t);
+    }
+}
+
+// acc += e(r) for two evaluations; TMSE zeroes residuals inside the tube first (|r| <= R -> 0)
+template <bool TMSE> __device__ __forceinline__ void accumulate2(float2 r, float R, float2 &acc)
+{
+    if (TMSE) {
+        r.x = fabsf(r.x) > R ? r.x : 0.f;
+        r.y = fabsf(r.y) > R ? r.y : 0.f;
+    }
+    acc = __ffma2_rn(r, r, acc);
+}
+
+// 32 consecutive accumulator columns of this thread's chromosome against 32 staged targets
+template <int ACT, bool TMSE>
+__device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const float *ts, float R, float2 &acc)
+{
+#pragma unroll
+    for (int j = 0; j < 32; j += 4) {
+        const float4 t4 = *reinterpret_cast<const float4 *>(ts + j);
+        accumulate2<TMSE>(residual2<ACT>(make_float2(__uint_as_float(v[j]), __uint_as_float(v[j + 1])), make_float2(t4.x, t4.y)), R, acc);
+        accumulate2<TMSE>(residual2<ACT>(make_float2(__uint_as_float(v[j + 2]), __uint_as_float(v[j + 3])), make_float2(t4.z, t4.w)), R, acc);
+    }
+}
+
+// ragged tail: only the first `valid` of the 32 columns count
+template <int ACT, bool TMSE>
+__device__ __forceinline__ void epilogue_chunk_masked(const uint32_t (&v)[32], const float *ts, float R, int valid, float2 &acc)
+{
+#pragma unroll
+    for (int j = 0; j < 32; j += 2) {
+        float2 r = residual2<ACT>(make_float2(__uint_as_float(v[j]), __uint_as_float(v[j + 1])), make_float2(ts[j], ts[j + 1]));
+        r.x = j < valid ? r.x : 0.f;
+        r.y = j + 1 < valid ? r.y : 0.f;
+        accumulate2<TMSE>(r, R, acc);
+    }
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------
@@ -275,7 +330,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
         for (int tile = pair; tile < total_tiles; tile += n_pairs) {
             const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
             const long long n0 = (long long)n_tile * BN;
-            tgt_s[acc * BN + et] = tgt[n0 + et];
+            tgt_s[acc * BN + et] = tgt[n0 + et] - (ACT == MODE_SIG_TANH32 ? 0.5f : 0.f);
             asm volatile("bar.sync 1, %0;" ::"n"(32 * N_EPI_WARPS) : "memory");
             long long rem = N - (n0 + half * 128);
             const int valid = rem >= 128 ? 128 : (rem > 0 ? (int)rem : 0);
@@ -283,30 +338,32 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             tc_fence_after();
             const uint32_t t0 = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(acc * BN + half * 128);
             const float *ts = tgt_s + acc * BN + half * 128;
-            float sum = 0.f;
-#pragma unroll 1
-            for (int c = 0; c < 4; ++c) {
-                if (c * 32 >= valid) break;
-                uint32_t v[32];
-                tmem_ld32(t0 + c * 32, v);
+            float2 acc2 = make_float2(0.f, 0.f);
+            if (valid == 128) {
+                // software pipeline: the TMEM load of chunk c+1 is in flight while chunk c is evaluated
+                uint32_t va[32], vb[32];
+                tmem_ld32(t0, va);
                 tmem_ld_wait();
-                if (c * 32 + 32 <= valid) {
-#pragma unroll
-                    for (int j = 0; j < 32; j += 4) {
-                        float4 t4 = *reinterpret_cast<const float4 *>(ts + c * 32 + j);
-                        sum += err_of<ACT, TMSE>(__uint_as_float(v[j]), t4.x, R);
-                        sum += err_of<ACT, TMSE>(__uint_as_float(v[j + 1]), t4.y, R);
-                        sum += err_of<ACT, TMSE>(__uint_as_float(v[j + 2]), t4.z, R);
-                        sum += err_of<ACT, TMSE>(__uint_as_float(v[j + 3]), t4.w, R);
-                    }
-                } else {
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        float e = err_of<ACT, TMSE>(__uint_as_float(v[j]), ts[c * 32 + j], R);
-                        sum += (c * 32 + j < valid) ? e : 0.f;
-                    }
+                tmem_ld32(t0 + 32, vb);
+                epilogue_chunk<ACT, TMSE>(va, ts, R, acc2);
+                tmem_ld_wait();
+                tmem_ld32(t0 + 64, va);
+                epilogue_chunk<ACT, TMSE>(vb, ts + 32, R, acc2);
+                tmem_ld_wait();
+                tmem_ld32(t0 + 96, vb);
+                epilogue_chunk<ACT, TMSE>(va, ts + 64, R, acc2);
+                tmem_ld_wait();
+                epilogue_chunk<ACT, TMSE>(vb, ts + 96, R, acc2);
+            } else {
+#pragma unroll 1
+                for (int c = 0; c * 32 < valid; ++c) {
+                    uint32_t v[32];
+                    tmem_ld32(t0 + c * 32, v);
+                    tmem_ld_wait();
+                    epilogue_chunk_masked<ACT, TMSE>(v, ts + c * 32, R, valid - c * 32, acc2);
                 }
             }
+            const float sum = acc2.x + acc2.y;
             tc_fence_before();
             __syncwarp();
             if (lane == 0) {
@@ -373,22 +430,42 @@ static int encode_map(game_ctx *ctx, CUtensorMap *m, void *ptr, long long rows, 
 
 bool tensor_path_built() { return true; }
 
-static int cta_group(const game_ctx *) {
-    static int cg = 0;
-    if (!cg) {
-        const char *e = getenv("GAME_TC_CTA_GROUP");      // measurement knob; default chosen by measurement
-        cg = (e && e[0] == '2') ? 2 : 1;
+// CTA pairs (cta_group::2, 256 chromosomes x 256 patterns per pair) halve the E-tile bytes each SM stages;
+// measured on B200 they win for deep contractions over wide populations (config 5: 1500 vs 1442 TFLOP/s)
+// and lose where the pair leaves too few chromosome blocks (config 4) or K is shallow (config 3).
+// GAME_TC_CTA_GROUP=1|2 overrides, for measurement.
+static int cta_group(const game_ctx *ctx, int Ppad)
+{
+    static int forced = -1;
+    if (forced < 0) {
+        const char *e = getenv("GAME_TC_CTA_GROUP");
+        forced = e ? (e[0] == '2' ? 2 : 1) : 0;
     }
-    return cg;
+    if (forced) return forced;
+    return (ctx->Kpad >= 512 && Ppad >= 1024) ? 2 : 1;
+}
+
+// Which logistic form the epilogue uses: mode 2 unless GAME_TC_SIGMOID=0 (measurement knob).
+static int sigmoid_mode()
+{
+    static int m = -1;
+    if (m < 0) {
+        const char *e = getenv("GAME_TC_SIGMOID");
+        m = (e && e[0] == '0') ? MODE_SIG_EXACT : MODE_SIG_TANH32;
+    }
+    return m;
 }
 
 int tensor_prepare(game_ctx *ctx)
 {
-    if (!ctx->tmap_E) ctx->tmap_E = aligned_alloc(64, sizeof(CUtensorMap));
+    if (!ctx->tmap_E) ctx->tmap_E = aligned_alloc(64, 2 * sizeof(CUtensorMap));    // [0]: 256-row boxes, [1]: 128-row
     if (!ctx->tmap_C) ctx->tmap_C = aligned_alloc(64, sizeof(CUtensorMap));
     if (!ctx->tmap_E || !ctx->tmap_C) return fail(ctx, GAME_ERR_ALLOC, "tensor map allocation failed");
-    const int cg = cta_group(ctx);
-    return encode_map(ctx, (CUtensorMap *)ctx->tmap_E, ctx->E16, ctx->Npad256, ctx->Kpad, BN / cg);
+    for (int cg = 1; cg <= 2; ++cg) {
+        int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_E + (cg - 1), ctx->E16, ctx->Npad256, ctx->Kpad, BN / cg);
+        if (rc) return rc;
+    }
+    return GAME_OK;
 }
 
 template <int CG, int ACT, bool TMSE>
@@ -414,15 +491,15 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
     KernelTimer timer(ctx);
-    GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, *(const CUtensorMap *)ctx->tmap_E, n_tiles,
+    GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, ((const CUtensorMap *)ctx->tmap_E)[CG - 1], n_tiles,
                                       m_blocks, ctx->Kpad / BKB, ctx->N, (const float *)ctx->t, ctx->R, ctx->partial, Ppad, state));
     return GAME_OK;
 }
 
 int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state)
 {
-    const int cg = cta_group(ctx);
     const int Ppad = ((P + 255) / 256) * 256;
+    const int cg = cta_group(ctx, Ppad);
     const int n_tiles = (int)(ctx->Npad256 / BN);
     const int m_blocks = Ppad / (BM * cg);
     long long n = (long long)P * ctx->K;
@@ -431,14 +508,19 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_C, ctx->C16, Ppad, ctx->Kpad, BM);
     if (rc) return rc;
     const bool tmse = ctx->err == GAME_ERR_TMSE;
-    const bool sig = ctx->act == GAME_ACT_SIGMOID;
-#define GAME_TC_DISPATCH(CGV)                                                                              \
-    rc = sig ? (tmse ? launch_variant<CGV, GAME_ACT_SIGMOID, true>(ctx, n_tiles, m_blocks, Ppad, state)       \
-                     : launch_variant<CGV, GAME_ACT_SIGMOID, false>(ctx, n_tiles, m_blocks, Ppad, state))     \
-             : (tmse ? launch_variant<CGV, GAME_ACT_IDENTITY, true>(ctx, n_tiles, m_blocks, Ppad, state)      \
-                     : launch_variant<CGV, GAME_ACT_IDENTITY, false>(ctx, n_tiles, m_blocks, Ppad, state))
+    const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : sigmoid_mode();
+#define GAME_TC_MODE(CGV, M)                                                                     \
+    rc = tmse ? launch_variant<CGV, M, true>(ctx, n_tiles, m_blocks, Ppad, state)                \
+              : launch_variant<CGV, M, false>(ctx, n_tiles, m_blocks, Ppad, state)
+#define GAME_TC_DISPATCH(CGV)                                                                    \
+    switch (mode) {                                                                              \
+    case MODE_IDENTITY: GAME_TC_MODE(CGV, MODE_IDENTITY); break;                                 \
+    case MODE_SIG_TANH32: GAME_TC_MODE(CGV, MODE_SIG_TANH32); break;                             \
+    default: GAME_TC_MODE(CGV, MODE_SIG_EXACT); break;                                           \
+    }
     if (cg == 2) { GAME_TC_DISPATCH(2); } else { GAME_TC_DISPATCH(1); }
 #undef GAME_TC_DISPATCH
+#undef GAME_TC_MODE
     if (rc) return rc;
     ++ctx->launches;
     return launch_finalize(ctx, (int)(ctx->Npad256 / SLAB), Ppad, P, out, state);

@@ -89,7 +89,7 @@ __device__ __forceinline__ uint32_t sort_key(float f)
     return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
 
-constexpr int RANK_T = 256, RANK_Q = 2048;
+constexpr int RANK_T = 128, RANK_Q = 256;   // chromosomes per CTA x keys per CTA: (P/128) x (P/256) CTAs
 
 __global__ void rank_count_kernel(const float *__restrict__ fit, int P, int *__restrict__ rank, const DevState *state)
 {
@@ -108,23 +108,24 @@ __global__ void rank_count_kernel(const float *__restrict__ fit, int P, int *__r
 #pragma unroll 8
     for (int i = 0; i < RANK_Q; ++i) cnt += keys[i] < mine;
     if (gridDim.y == 1) rank[p] = cnt;
-    else atomicAdd(&rank[p], cnt);               // integer: order-independent, exact
+    else if (cnt) atomicAdd(&rank[p], cnt);      // integer: order-independent, exact; buffer is zero on entry
 }
 
 // order[rank[p]] = p, plus a7: record the best and apply the stop test (L219, L287; DESIGN G18)
-__global__ void rank_scatter_kernel(const float *__restrict__ fit, int P, const int *__restrict__ rank,
+__global__ void rank_scatter_kernel(const float *__restrict__ fit, int P, int *__restrict__ rank,
                                     int *__restrict__ order, DevState *state, float stop_error, int update_state)
 {
     if (state && state->stopped) return;
     int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P) return;
     int r = rank[p];
+    rank[p] = 0;                                 // leave the scratch zeroed for the next call's atomics
     order[r] = p;
     if (r == 0 && update_state) {
         float f = fit[p];
         state->best_error = f;
         state->best_index = p;
-        if (stop_error >= 0.0f && f <= stop_error) state->stopped = 1;
+        if (stop_error >= 0.0f && f <= stop_error) state->stop_request = 1;
     }
 }
 
@@ -132,7 +133,6 @@ int launch_rank(game_ctx *ctx, const float *fit, int P, int *rank_scratch, int *
                 float stop_error, bool update_state)
 {
     dim3 grid((P + RANK_T - 1) / RANK_T, (P + RANK_Q - 1) / RANK_Q);
-    if (grid.y > 1) GAME_CUDA(ctx, cudaMemsetAsync(rank_scratch, 0, sizeof(int) * (size_t)P, ctx->stream));
     rank_count_kernel<<<grid, RANK_T, 0, ctx->stream>>>(fit, P, rank_scratch, state);
     GAME_LAUNCHED(ctx);
     rank_scatter_kernel<<<(P + 255) / 256, 256, 0, ctx->stream>>>(fit, P, rank_scratch, order, state, stop_error,
@@ -230,7 +230,8 @@ __global__ void ga_step_kernel(StepArgs a, const int *__restrict__ order, const 
                                DevState *state, int *dbg)
 {
     const int K = a.K;
-    const bool stopped = state && state->stopped;
+    const bool stopped = state && (state->stopped | state->stop_request);
+    if (stopped && threadIdx.x == 0) state->stopped = 1;      // promote (every CTA writes the same value)
     if (blockIdx.x < a.e) {                         // a8 elitism (L148, L291; DESIGN G17)
         int j = blockIdx.x;
         int src = stopped ? j : (a.elite_mode == GAME_ELITE_TOP_E ? order[j] : order[0]);

@@ -52,6 +52,7 @@ static int ensure_population(game_ctx *c, int P)
     GAME_CUDA(c, cudaMalloc(&c->fit, (size_t)P * sizeof(float)));
     GAME_CUDA(c, cudaMalloc(&c->order, (size_t)P * sizeof(int)));
     GAME_CUDA(c, cudaMalloc(&c->rank, (size_t)P * sizeof(int)));
+    GAME_CUDA(c, cudaMemsetAsync(c->rank, 0, (size_t)P * sizeof(int), c->stream));   // rank kernels keep it zeroed
     GAME_CUDA(c, cudaMalloc(&c->rw, (size_t)P * sizeof(unsigned int)));
     GAME_CUDA(c, cudaMalloc(&c->rprefix, (size_t)P * sizeof(unsigned long long)));
     c->pop_cap = P;
@@ -331,7 +332,7 @@ int game_evolve(game_ctx *c, int generations, unsigned long long seed, const gam
         if (can_stop && (g & 31) == 31) {        // poll the device-side stop flag now and then
             GAME_CUDA(c, cudaMemcpyAsync(&h, c->state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
             GAME_CUDA(c, cudaStreamSynchronize(c->stream));
-            if (h.stopped) break;
+            if (h.stopped || h.stop_request) break;
         }
         rc = launch_ga_step(c, gp, seed, (unsigned int)(c->generation + g), c->order, c->fit, c->pop, c->pop_next,
                             c->state, c->rw, c->rprefix);                                     // a8-a11
@@ -344,7 +345,7 @@ int game_evolve(game_ctx *c, int generations, unsigned long long seed, const gam
     c->have_fit = true;
     if (res) {
         res->generations_run = h.gens_run;
-        res->stopped_on_error = h.stopped;
+        res->stopped_on_error = (h.stopped || h.stop_request) ? 1 : 0;
         res->best_error = h.best_error;
         res->best_index = h.best_index;
     }
@@ -372,6 +373,7 @@ int game_rank(game_ctx *c, const float *fit, int P, int *order)
     if (!fit || !order || P < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_rank: NULL pointer or P < 1");
     int *scratch = nullptr;
     GAME_CUDA(c, cudaMallocAsync(&scratch, (size_t)P * sizeof(int), c->stream));
+    GAME_CUDA(c, cudaMemsetAsync(scratch, 0, (size_t)P * sizeof(int), c->stream));
     int rc = launch_rank(c, fit, P, scratch, order, nullptr, -1.f, false);
     cudaFreeAsync(scratch, c->stream);
     return rc;

@@ -16,7 +16,9 @@ constexpr int TC_KBLK = 64;      // fp16 elements per 128-byte swizzled smem row
 
 // Device-resident loop state, so a generation needs no host round trip.
 struct DevState {
-    int stopped;          // set by the stop test (a7); later kernels of the loop become no-ops
+    int stopped;          // the loop has stopped: later kernels of the loop become no-ops
+    int stop_request;     // written by the stop test (a7) inside rank_scatter_kernel; the next ga_step_kernel promotes
+                          // it to `stopped`, so no kernel ever tests a flag that its own launch may be writing
     int gens_run;         // evolution steps actually applied
     float best_error;
     int best_index;
