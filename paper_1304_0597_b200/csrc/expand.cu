@@ -43,7 +43,8 @@ __global__ void expand_kernel(const float *__restrict__ X, long long N, int F, i
         auto put = [&](int k, double v) {
             float f = (float)v;
             local_max = fmaxf(local_max, fabsf(f));
-            if (PATTERN_MAJOR) E[n * ld + k] = (OutT)f;
+            // TENSOR path: tile-blocked [n/256][k/64][256][64] so that every TMA box is one contiguous 32 KB run
+            if (PATTERN_MAJOR) E[(((n >> 8) * (ld >> 6) + (k >> 6)) << 14) + ((n & 255) << 6) + (k & 63)] = (OutT)f;
             else E[(long long)k * ld + n] = (OutT)f;
         };
         put(k0, 1.0);

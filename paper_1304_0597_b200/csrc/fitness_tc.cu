@@ -282,13 +282,13 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             for (int tile = pair; tile < total_tiles; tile += n_pairs) {
                 const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
                 const int rowC = (m_blk * CG + (int)cta_rank) * BM;
-                const int rowE = n_tile * BN + (int)cta_rank * C::BNL;
+                const int rowE = n_tile * k_blocks * BN + (int)cta_rank * C::BNL;     // E16 is tile-blocked: [n_tile][kb][256][64]
                 for (int kb = 0; kb < k_blocks; ++kb) {
                     mbar_wait(empty_bar(s), ph ^ 1);
                     const uint32_t sa = base + s * C::STAGE_BYTES, sb = sa + A_BYTES;
                     if (CG == 1 || cta_rank == 0) mbar_expect_tx(full_bar(s), CG * C::STAGE_BYTES);
                     tma_load_2d<CG>(sa, &tmC, kb * BKB, rowC, full_bar(s));
-                    tma_load_2d<CG>(sb, &tmE, kb * BKB, rowE, full_bar(s));
+                    tma_load_2d<CG>(sb, &tmE, 0, rowE + kb * BN, full_bar(s));
                     if (++s == C::STAGES) { s = 0; ph ^= 1; }
                 }
             }
@@ -413,7 +413,7 @@ static EncodeTiledFn get_encode()
     return fn;
 }
 
-// [rows][Kpad] fp16 row-major, boxes of [box_rows][64], 128-byte swizzle
+// [rows][row_elems] fp16 row-major, boxes of [box_rows][64], 128-byte swizzle
 static int encode_map(game_ctx *ctx, CUtensorMap *m, void *ptr, long long rows, int Kpad, int box_rows)
 {
     EncodeTiledFn enc = get_encode();
@@ -462,7 +462,8 @@ int tensor_prepare(game_ctx *ctx)
     if (!ctx->tmap_C) ctx->tmap_C = aligned_alloc(64, sizeof(CUtensorMap));
     if (!ctx->tmap_E || !ctx->tmap_C) return fail(ctx, GAME_ERR_ALLOC, "tensor map allocation failed");
     for (int cg = 1; cg <= 2; ++cg) {
-        int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_E + (cg - 1), ctx->E16, ctx->Npad256, ctx->Kpad, BN / cg);
+        // E16 viewed as [(Npad256/256) * (Kpad/64) * 256][64]: one 128-byte row per (pattern, k-block)
+        int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_E + (cg - 1), ctx->E16, ctx->Npad256 * (ctx->Kpad / BKB), BKB, BN / cg);
         if (rc) return rc;
     }
     return GAME_OK;
