@@ -219,7 +219,11 @@ def run_ours(args, w):
             torch.cuda.synchronize()
 
         ctx.evolve(max(args.warmup, 3), wr.seed, gp)            # W untimed warm-up steps (also creates the population)
-        ctx.set_kernel_timing(True)
+        # The dominant kernel is bracketed by CUDA events inside the timed region -- except on the launch-latency
+        # bound configs (1-2), where per-launch events would perturb the captured-graph loop being timed: there
+        # the kernel is timed in a second, identical pass right after.
+        separate_pass = float(w.N) * w.P * w.K < 2e10
+        ctx.set_kernel_timing(not separate_pass)
         ctx.get_kernel_timing()
         sampler = ClockSampler(local)
         sampler.start()
@@ -233,6 +237,15 @@ def run_ours(args, w):
         ms = e0.elapsed_time(e1)
         launches = ctx.launch_count() - launches0
         kern_ms, kern_n = ctx.get_kernel_timing()
+        kern_pass_ms = ms
+        if separate_pass:
+            ctx.set_kernel_timing(True)
+            e0.record(stream)
+            ctx.evolve(min(args.steps, 200), wr.seed, gp)
+            e1.record(stream)
+            stream.synchronize()
+            kern_pass_ms = e0.elapsed_time(e1)
+            kern_ms, kern_n = ctx.get_kernel_timing()
         ctx.set_kernel_timing(False)
         sampler.join()
         assert res.generations_run == args.steps
@@ -275,7 +288,8 @@ def run_ours(args, w):
     roof["traffic"] = ncu_traffic(w, path_name)
     roof["kernel_ms_avg"] = avg_s * 1e3
     roof["kernel_launches_timed"] = kern_n
-    roof["kernel_share_of_step"] = kern_ms / ms
+    roof["kernel_share_of_step"] = kern_ms / kern_pass_ms
+    roof["kernel_timing"] = "separate pass after the timed region (launch-bound config)" if separate_pass else "inside the timed region"
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:

@@ -132,6 +132,67 @@ fitness_fp32_kernel(const float *__restrict__ ET, long long Npad, long long N, i
     }
 }
 
+// Small problems (configs 1-2) are launch-latency bound, so the tail of a generation is ONE single-CTA kernel:
+// a5 final reduction (same summation order as finalize_kernel, so the bits agree), a6 rank by counting
+// over shared-memory keys, a7 best / stop test.  One thread per chromosome; used for P <= 256, n_chunks*P <= 8192
+// (beyond that the multi-CTA rank is faster than one CTA's P^2 compares).
+constexpr int POST_SMALL_FLOATS = 8192;
+
+__global__ void __launch_bounds__(256, 1)
+post_small_kernel(const float *__restrict__ partial, int n_chunks, int Ppad, int P, long long N, int err,
+                  float *__restrict__ fit, int *__restrict__ order, DevState *state, float stop_error)
+{
+    if (state->stopped) return;            // single CTA: the flag this kernel may set is stop_request, read by later launches
+    __shared__ unsigned long long keys[256];
+    __shared__ float part[POST_SMALL_FLOATS];
+    const int p = threadIdx.x;
+    for (int i = p; i < n_chunks * P; i += blockDim.x)        // all slab sums in flight at once, then summed in order
+        part[i] = partial[(long long)(i / P) * Ppad + (i % P)];
+    __syncthreads();
+    unsigned long long mine = ~0ull;
+    float f = 0.f;
+    if (p < P) {
+        double tot = 0.0;
+        for (int r = 0; r < 32; ++r) {
+            double s = 0.0;
+            for (int ch = r; ch < n_chunks; ch += 32) s += (double)part[ch * P + p];
+            tot += s;
+        }
+        double v = tot / (double)N;
+        if (err == GAME_ERR_RMSE) v = sqrt(v);
+        f = (float)v;
+        fit[p] = f;
+        mine = ((unsigned long long)sort_key(f) << 32) | (unsigned)p;
+    }
+    keys[p] = mine;
+    __syncthreads();
+    if (p >= P) return;
+    int cnt = 0;
+#pragma unroll 8
+    for (int q = 0; q < P; ++q) cnt += keys[q] < mine;
+    order[cnt] = p;
+    if (cnt == 0) {
+        state->best_error = f;
+        state->best_index = p;
+        state->evals_done += 1;
+        if (stop_error >= 0.0f && f <= stop_error) state->stop_request = 1;
+    }
+}
+
+int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scratch, int *order, DevState *state,
+                float stop_error)
+{
+    if (P <= 256 && (long long)pi.n_chunks * P <= POST_SMALL_FLOATS) {
+        post_small_kernel<<<1, 256, 0, ctx->stream>>>(ctx->partial, pi.n_chunks, pi.Ppad, P, ctx->N, ctx->err, fit, order,
+                                                           state, stop_error);
+        GAME_LAUNCHED(ctx);
+        return GAME_OK;
+    }
+    int rc = launch_finalize(ctx, pi.n_chunks, pi.Ppad, P, fit, state);
+    if (rc) return rc;
+    return launch_rank(ctx, fit, P, rank_scratch, order, state, stop_error, true);
+}
+
 // fit[p] = (sum over chunks, ascending, in fp64) / N; RMSE takes the root (eq. 4-5).
 __global__ void finalize_kernel(const float *__restrict__ partial, int n_chunks, int Ppad, int P, long long N,
                                 int err, float *__restrict__ out, const DevState *state)
@@ -152,6 +213,89 @@ __global__ void finalize_kernel(const float *__restrict__ partial, int n_chunks,
         if (err == GAME_ERR_RMSE) f = sqrt(f);
         out[p] = (float)f;
     }
+}
+
+// ---- small problems (configs 1-2): latency, not throughput, decides ------------------------------------
+// The 128x128 tile above needs ~20 us per CTA whatever P is; when the whole grid is under two waves a
+// finer decomposition finishes sooner.  One CTA = one 128-pattern slab x 32 chromosomes, one THREAD = one
+// pattern: it streams its column of the term-major expansion (coalesced across the warp) against the 32
+// chromosomes staged in shared memory (broadcast reads), keeps 32 dot products in registers, applies the
+// activation and error, and the 32 per-pattern errors are summed over the slab's patterns by a fixed
+// butterfly (31 shuffles) and a 4-warp shared-memory pass.  Same partial[slab][p] layout as the big kernel.
+constexpr int SP = 32, SKC = 128;
+
+constexpr int SMALL_SMEM = SKC * SLAB * 4 + SKC * (SP + 4) * 4;      // E chunk [128][128] + C chunk [128][36]
+
+__global__ void __launch_bounds__(128)
+fitness_small_kernel(const float *__restrict__ ET, long long Npad, long long N, int K, const float *__restrict__ pop,
+                     int P, const float *__restrict__ tgt, FitnessCfg cfg, float *__restrict__ partial, int Ppad,
+                     const DevState *state)
+{
+    if (state && state->stopped) return;
+    extern __shared__ __align__(16) float small_smem[];
+    float (*Es)[SLAB] = reinterpret_cast<float (*)[SLAB]>(small_smem);                       // [k][n], as in ET
+    float (*Cs)[SP + 4] = reinterpret_cast<float (*)[SP + 4]>(small_smem + SKC * SLAB);      // [k][p]; +4: transposed
+    __shared__ float red[4][SP];                                                             // stores 4-way, not 32-way
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const long long n0 = (long long)blockIdx.x * SLAB;
+    const long long n = n0 + tid;
+    const int p0 = blockIdx.y * SP;
+    float acc[SP];
+#pragma unroll
+    for (int j = 0; j < SP; ++j) acc[j] = 0.f;
+    for (int k0 = 0; k0 < K; k0 += SKC) {
+        const int kc = min(SKC, K - k0);
+        __syncthreads();
+        // the whole E chunk in flight at once (cp.async, 16 B per request): one memory latency, not kc of them
+        for (int i = tid; i < kc * (SLAB / 4); i += 128) {
+            const int kk = i / (SLAB / 4), c4 = i % (SLAB / 4);
+            const float *src = ET + (long long)(k0 + kk) * Npad + n0 + c4 * 4;
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(&Es[kk][c4 * 4]);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+        }
+        for (int i = tid; i < SKC * SP; i += 128) {          // Cs[k][p] <- pop[p0+p][k0+k] (zero-filled outside), k fastest
+            const int pp = i / SKC, kk = i % SKC;
+            const bool in = p0 + pp < P && kk < kc;
+            const float *src = in ? pop + (long long)(p0 + pp) * K + k0 + kk : pop;
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(&Cs[kk][pp]);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(in ? 4 : 0) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();
+#pragma unroll 4
+        for (int kk = 0; kk < kc; ++kk) {
+            const float e = Es[kk][tid];
+#pragma unroll
+            for (int j = 0; j < SP; j += 4) {
+                const float4 c4 = *reinterpret_cast<const float4 *>(&Cs[kk][j]);
+                acc[j] = fmaf(e, c4.x, acc[j]);
+                acc[j + 1] = fmaf(e, c4.y, acc[j + 1]);
+                acc[j + 2] = fmaf(e, c4.z, acc[j + 2]);
+                acc[j + 3] = fmaf(e, c4.w, acc[j + 3]);
+            }
+        }
+    }
+    const bool valid = n < N;
+    const float t = tgt[n];
+#pragma unroll
+    for (int j = 0; j < SP; ++j) acc[j] = act_err(acc[j], t, valid, cfg.act, cfg.err, cfg.R);
+    // butterfly: after the step with offset o each lane holds half as many columns, summed over lane pairs;
+    // a + b is commutative, so every chromosome sees the same fixed tree whatever its column (DESIGN P20)
+#pragma unroll
+    for (int o = 16, w = SP / 2; o >= 1; o >>= 1, w >>= 1) {
+        const bool upper = (lane & o) != 0;
+#pragma unroll
+        for (int j = 0; j < w; ++j) {
+            float keep = upper ? acc[j + w] : acc[j];
+            float send = upper ? acc[j] : acc[j + w];
+            acc[j] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+        }
+    }
+    // lane l now owns column bitrev-free index: the kept halves follow the lane bits, i.e. column == lane
+    red[warp][lane] = acc[0];
+    __syncthreads();
+    if (tid < SP) partial[(long long)blockIdx.x * Ppad + p0 + tid] = red[0][tid] + red[1][tid] + red[2][tid] + red[3][tid];
 }
 
 static int pick_slabs_per_cta(const game_ctx *ctx, int P)
@@ -180,19 +324,36 @@ int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, co
     return GAME_OK;
 }
 
-int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state)
+int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer)
 {
     int Ppad = ((P + 255) / 256) * 256;
+    FitnessCfg cfg{ctx->act, ctx->err, ctx->R};
+    if ((long long)ctx->n_slabs * ((P + BP - 1) / BP) < 2LL * ctx->sm_count) {       // under two waves of big tiles
+        dim3 grid((unsigned)ctx->n_slabs, (unsigned)((P + SP - 1) / SP));
+        static bool attr_set = false;
+        if (!attr_set) {
+            GAME_CUDA(ctx, cudaFuncSetAttribute(fitness_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMALL_SMEM));
+            attr_set = true;
+        }
+        {
+            KernelTimer timer(ctx);
+            fitness_small_kernel<<<grid, 128, SMALL_SMEM, ctx->stream>>>(ctx->ET, ctx->Npad, ctx->N, ctx->K, pop, P, ctx->t, cfg,
+                                                              ctx->partial, Ppad, state);
+        }
+        GAME_LAUNCHED(ctx);
+        if (defer) { defer->n_chunks = ctx->n_slabs; defer->Ppad = Ppad; return GAME_OK; }
+        return launch_finalize(ctx, ctx->n_slabs, Ppad, P, out, state);
+    }
     int spc = pick_slabs_per_cta(ctx, P);
     int n_chunks = (ctx->n_slabs + spc - 1) / spc;
     dim3 grid((unsigned)n_chunks, (unsigned)((P + BP - 1) / BP));
-    FitnessCfg cfg{ctx->act, ctx->err, ctx->R};
     {
         KernelTimer timer(ctx);
         fitness_fp32_kernel<<<grid, NT, 0, ctx->stream>>>(ctx->ET, ctx->Npad, ctx->N, ctx->K, pop, P, ctx->t,
                                                           ctx->n_slabs, spc, cfg, ctx->partial, Ppad, state);
     }
     GAME_LAUNCHED(ctx);
+    if (defer) { defer->n_chunks = n_chunks; defer->Ppad = Ppad; return GAME_OK; }
     return launch_finalize(ctx, n_chunks, Ppad, P, out, state);
 }
 

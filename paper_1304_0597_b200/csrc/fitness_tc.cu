@@ -497,7 +497,7 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     return GAME_OK;
 }
 
-int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state)
+int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer)
 {
     const int Ppad = ((P + 255) / 256) * 256;
     const int cg = cta_group(ctx, Ppad);
@@ -524,6 +524,7 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
 #undef GAME_TC_MODE
     if (rc) return rc;
     ++ctx->launches;
+    if (defer) { defer->n_chunks = (int)(ctx->Npad256 / SLAB); defer->Ppad = Ppad; return GAME_OK; }
     return launch_finalize(ctx, (int)(ctx->Npad256 / SLAB), Ppad, P, out, state);
 }
 

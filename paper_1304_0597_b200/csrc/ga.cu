@@ -81,14 +81,6 @@ int launch_init_population(game_ctx *ctx, int mode, unsigned long long seed, int
 }
 
 // ---- a6: rank by counting.  key = (error, index) ascending, NaN as +inf, -0 as +0 (DESIGN G20) --------
-__device__ __forceinline__ uint32_t sort_key(float f)
-{
-    if (f != f) f = __int_as_float(0x7f800000);
-    f += 0.0f;                                   // -0 -> +0
-    uint32_t u = __float_as_uint(f);
-    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
-}
-
 constexpr int RANK_T = 128, RANK_Q = 256;   // chromosomes per CTA x keys per CTA: (P/128) x (P/256) CTAs
 
 __global__ void rank_count_kernel(const float *__restrict__ fit, int P, int *__restrict__ rank, const DevState *state)
@@ -125,6 +117,7 @@ __global__ void rank_scatter_kernel(const float *__restrict__ fit, int P, int *_
         float f = fit[p];
         state->best_error = f;
         state->best_index = p;
+        state->evals_done += 1;
         if (stop_error >= 0.0f && f <= stop_error) state->stop_request = 1;
     }
 }
@@ -230,6 +223,7 @@ __global__ void ga_step_kernel(StepArgs a, const int *__restrict__ order, const 
                                DevState *state, int *dbg)
 {
     const int K = a.K;
+    if (state) a.gen += (uint32_t)(state->evals_done - 1);     // written by the rank step of THIS generation, stable here
     const bool stopped = state && (state->stopped | state->stop_request);
     if (stopped && threadIdx.x == 0) state->stopped = 1;      // promote (every CTA writes the same value)
     if (blockIdx.x < a.e) {                         // a8 elitism (L148, L291; DESIGN G17)
@@ -275,7 +269,7 @@ __global__ void ga_step_kernel(StepArgs a, const int *__restrict__ order, const 
     }
 }
 
-int launch_ga_step(game_ctx *ctx, const game_ga_params *gp, unsigned long long seed, unsigned int gen,
+int launch_ga_step(game_ctx *ctx, const game_ga_params *gp, unsigned long long seed, unsigned int gen_base,
                    const int *order, const float *fit, const float *pop, float *next, DevState *state,
                    unsigned int *rw, unsigned long long *rprefix)
 {
@@ -283,7 +277,7 @@ int launch_ga_step(game_ctx *ctx, const game_ga_params *gp, unsigned long long s
     a.P = gp->P; a.K = ctx->K; a.e = gp->elitism; a.elite_mode = gp->elite_mode; a.selection = gp->selection;
     a.tsize = gp->tournament_size; a.npairs = (gp->P - gp->elitism + 1) / 2;
     a.pc = host_thr(gp->p_crossover); a.pm = host_thr(gp->p_mutation);
-    a.seed = seed; a.gen = gen;
+    a.seed = seed; a.gen = gen_base;
     if (gp->selection == GAME_SEL_ROULETTE) {
         roulette_kernel<<<1, 1024, 0, ctx->stream>>>(fit, order, gp->P, rw, rprefix, state);
         GAME_LAUNCHED(ctx);

@@ -85,14 +85,14 @@ static int resolve_path(const game_ctx *c, int P)
     return (can_tensor && P >= 256 && c->N >= 16384) ? GAME_PATH_TENSOR : GAME_PATH_FP32;
 }
 
-static int run_fitness(game_ctx *c, const float *pop, int P, float *out, const DevState *state)
+static int run_fitness(game_ctx *c, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer = nullptr)
 {
     int rc = ensure_scratch(c, P);
     if (rc) return rc;
     int path = resolve_path(c, P);
     if (path < 0) return fail(c, GAME_ERR_UNSUPPORTED, "tensor path unavailable for this dataset (not built, or |E| exceeds fp16 range)");
-    return path == GAME_PATH_TENSOR ? launch_fitness_tensor(c, pop, P, out, state)
-                                    : launch_fitness_fp32(c, pop, P, out, state);
+    return path == GAME_PATH_TENSOR ? launch_fitness_tensor(c, pop, P, out, state, defer)
+                                    : launch_fitness_fp32(c, pop, P, out, state, defer);
 }
 
 static int validate_params(game_ctx *c, const game_ga_params *g)
@@ -323,22 +323,69 @@ int game_evolve(game_ctx *c, int generations, unsigned long long seed, const gam
     GAME_CUDA(c, cudaMemsetAsync(c->state, 0, sizeof(DevState), c->stream));
     DevState h{};
     const bool can_stop = gp->stop_error >= 0.f;
-    for (int g = 0; g <= generations; ++g) {
-        rc = run_fitness(c, c->pop, P, c->fit, c->state);                                    // a1-a5
-        if (rc) return rc;
-        rc = launch_rank(c, c->fit, P, c->rank, c->order, c->state, gp->stop_error, true);    // a6, a7
-        if (rc) return rc;
-        if (g == generations) break;
-        if (can_stop && (g & 31) == 31) {        // poll the device-side stop flag now and then
-            GAME_CUDA(c, cudaMemcpyAsync(&h, c->state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
-            GAME_CUDA(c, cudaStreamSynchronize(c->stream));
-            if (h.stopped || h.stop_request) break;
-        }
-        rc = launch_ga_step(c, gp, seed, (unsigned int)(c->generation + g), c->order, c->fit, c->pop, c->pop_next,
-                            c->state, c->rw, c->rprefix);                                     // a8-a11
-        if (rc) return rc;
+    const unsigned int gen_base = (unsigned int)c->generation;      // the device adds its own evaluation counter
+    auto evaluate = [&]() -> int {                                   // a1-a5, then a5 tail + a6 + a7
+        PartialInfo pi{};
+        int r = run_fitness(c, c->pop, P, c->fit, c->state, &pi);
+        if (r) return r;
+        return launch_post(c, pi, P, c->fit, c->rank, c->order, c->state, gp->stop_error);
+    };
+    auto generation = [&]() -> int {
+        int r = evaluate();
+        if (r) return r;
+        r = launch_ga_step(c, gp, seed, gen_base, c->order, c->fit, c->pop, c->pop_next, c->state, c->rw, c->rprefix);   // a8-a11
+        if (r) return r;
         float *tmp = c->pop; c->pop = c->pop_next; c->pop_next = tmp;
+        return GAME_OK;
+    };
+    auto stopped_now = [&](bool &stop) -> int {                      // poll the device-side stop flag
+        GAME_CUDA(c, cudaMemcpyAsync(&h, c->state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+        GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+        stop = h.stopped || h.stop_request;
+        return GAME_OK;
+    };
+    int g = 0;
+    bool stop = false;
+    const bool capturable = c->stream != nullptr && c->stream != cudaStreamLegacy && c->stream != cudaStreamPerThread;
+    if (generations >= 8 && !c->timing && capturable) {
+        // Launch-latency matters for small problems: capture TWO generations (the population buffers swap
+        // back after two) into a CUDA graph and replay it.  Nothing in the captured kernels depends on host
+        // arguments that change per generation: the generation index and the stop flag live on the device.
+        rc = generation();                     // outside the graph: sets kernel attributes, sizes scratch
+        if (rc) return rc;
+        g = 1;
+        cudaGraph_t graph = nullptr;
+        cudaGraphExec_t exec = nullptr;
+        const long long before = c->launches;
+        GAME_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+        rc = generation();
+        if (!rc) rc = generation();
+        cudaError_t ce = cudaStreamEndCapture(c->stream, &graph);
+        const long long per_graph = c->launches - before;
+        c->launches = before;
+        if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (ce != cudaSuccess) return cuda_fail(c, ce, "cudaStreamEndCapture");
+        ce = cudaGraphInstantiate(&exec, graph, 0);
+        if (ce != cudaSuccess) { cudaGraphDestroy(graph); return cuda_fail(c, ce, "cudaGraphInstantiate"); }
+        for (int rep = 0; g + 2 <= generations && !stop; ++rep) {
+            ce = cudaGraphLaunch(exec, c->stream);
+            if (ce != cudaSuccess) break;
+            c->launches += per_graph;
+            g += 2;
+            if (can_stop && (rep & 15) == 15) { rc = stopped_now(stop); if (rc) break; }
+        }
+        cudaGraphExecDestroy(exec);
+        cudaGraphDestroy(graph);
+        if (ce != cudaSuccess) return cuda_fail(c, ce, "cudaGraphLaunch");
+        if (rc) return rc;
     }
+    for (; g < generations && !stop; ++g) {
+        rc = generation();
+        if (rc) return rc;
+        if (can_stop && (g & 31) == 31) { rc = stopped_now(stop); if (rc) return rc; }
+    }
+    rc = evaluate();                           // the returned fitness belongs to the returned population (G18)
+    if (rc) return rc;
     GAME_CUDA(c, cudaMemcpyAsync(&h, c->state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     GAME_CUDA(c, cudaStreamSynchronize(c->stream));
     c->generation += h.gens_run;

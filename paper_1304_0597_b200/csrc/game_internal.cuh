@@ -20,9 +20,23 @@ struct DevState {
     int stop_request;     // written by the stop test (a7) inside rank_scatter_kernel; the next ga_step_kernel promotes
                           // it to `stopped`, so no kernel ever tests a flag that its own launch may be writing
     int gens_run;         // evolution steps actually applied
+    int evals_done;       // fitness + rank evaluations completed; ga_step derives its generation index from it,
+                          // so a captured CUDA graph of the loop needs no per-generation host arguments
     float best_error;
     int best_index;
 };
+
+// where a fitness launch left its per-slab sums, when the caller fuses the final reduction with the rank
+struct PartialInfo { int n_chunks, Ppad; };
+
+// rank key: (error, index) ascending, NaN as +inf, -0 as +0 (DESIGN G20)
+__device__ __forceinline__ unsigned int sort_key(float f)
+{
+    if (f != f) f = __int_as_float(0x7f800000);
+    f += 0.0f;
+    unsigned int u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
 
 struct FitnessCfg {
     int act, err;
@@ -114,19 +128,23 @@ int launch_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out
 
 // fitness_fp32.cu
 size_t fitness_partial_floats(const game_ctx *ctx, int P);
-int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state);
+int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer);
 int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, const DevState *state);
+// a5 tail + a6 + a7 in one go: final reduction of the slab sums, rank, stop test (single CTA when small)
+int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scratch, int *order, DevState *state,
+                float stop_error);
 
 // fitness_tc.cu
 bool tensor_path_built();
 int tensor_prepare(game_ctx *ctx);                               // tensor maps etc. after load
-int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state);
+int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer);
 
 // ga.cu
 int launch_init_population(game_ctx *ctx, int mode, unsigned long long seed, int P, float *pop);
 int launch_rank(game_ctx *ctx, const float *fit, int P, int *rank_scratch, int *order, DevState *state,
                 float stop_error, bool update_state);
-int launch_ga_step(game_ctx *ctx, const game_ga_params *gp, unsigned long long seed, unsigned int gen,
+// generation index = gen_base (+ state->evals_done - 1 when state is given: the loop's device-side counter)
+int launch_ga_step(game_ctx *ctx, const game_ga_params *gp, unsigned long long seed, unsigned int gen_base,
                    const int *order, const float *fit, const float *pop, float *next, DevState *state,
                    unsigned int *rw, unsigned long long *rprefix);
 int launch_philox(game_ctx *ctx, unsigned long long seed, const unsigned int *ctr, int n, unsigned int *out);
