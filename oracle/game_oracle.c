@@ -135,6 +135,43 @@ void oracle_forward(int family, int degree, int F, int act, const float *X, long
     free(phi);
 }
 
+/* ---- test / run use cases (L127-L129) and the figures of merit of L301 ----------------------------------
+ * A pattern is classified GC (class 1) when act(z) > cut, and IS a GC when its target > 0.5.
+ * counts = {TP, FP, TN, FN}.  L301: accuracy = "fraction of patterns which are correctly classified
+ * (either GCs or non-GCs) with respect to the total" = (TP+TN)/N; completeness = "fraction of GCs which are
+ * correctly classified as such" = TP/(TP+FN); contamination = "fraction of non-GC objects which are
+ * erroneously classified as GCs" = FP/(FP+TN), read literally (DESIGN G23).  An empty denominator gives 0.
+ * near (optional) counts the patterns with |act(z) - cut| <= delta: a lower-precision implementation may
+ * legitimately classify those the other way. */
+void oracle_classify(int family, int degree, int F, int act, const float *X, const float *t, long long N,
+                     const float *genes, double cut, long long counts[4], double fom[3], long long *near,
+                     double delta)
+{
+    int K = oracle_num_terms(family, degree, F);
+    double *phi = (double *)malloc(sizeof(double) * (size_t)K);
+    long long tp = 0, fp = 0, tn = 0, fn = 0, nr = 0;
+    for (long long n = 0; n < N; ++n) {
+        expand_row(family, degree, F, X + n * F, phi);
+        double z = 0.0;
+        for (int k = 0; k < K; ++k) z += phi[k] * (double)genes[k];
+        double y = activate(act, z);
+        int pred = y > cut, truth = (double)t[n] > 0.5;
+        if (pred && truth) ++tp;
+        else if (pred && !truth) ++fp;
+        else if (!pred && !truth) ++tn;
+        else ++fn;
+        if (fabs(y - cut) <= delta) ++nr;
+    }
+    free(phi);
+    counts[0] = tp; counts[1] = fp; counts[2] = tn; counts[3] = fn;
+    if (fom) {
+        fom[0] = N > 0 ? (double)(tp + tn) / (double)N : 0.0;
+        fom[1] = tp + fn > 0 ? (double)tp / (double)(tp + fn) : 0.0;
+        fom[2] = fp + tn > 0 ? (double)fp / (double)(fp + tn) : 0.0;
+    }
+    if (near) *near = nr;
+}
+
 /* ---- a1..a5: fitness of every chromosome -------------------------------------------------
  * fit[p] = (1/N) sum_n e(t_n - act(z[n][p]))  (eq. 4); RMSE = sqrt (eq. 5).
  * e(r) = r^2 (eq. 3); TMSE (eq. 10, read per DESIGN G5 from the worked example

@@ -128,6 +128,21 @@ def fitness(family, degree, X, t, pop, act=SIGMOID, err=MSE, R=0.0, delta=None):
     return fit if delta is None else (fit, near)
 
 
+def classify(family, degree, X, t, genes, act=SIGMOID, cut=0.5, delta=0.0):
+    """oracle_classify: (counts[TP,FP,TN,FN], (accuracy, completeness, contamination), near) -- L301."""
+    X = _f32(X)
+    t = _f32(t)
+    genes = _f32(genes)
+    N, F = X.shape
+    counts = np.zeros(4, dtype=np.int64)
+    fom = np.zeros(3, dtype=np.float64)
+    near = C.c_longlong(0)
+    lib().oracle_classify(C.c_int(family), C.c_int(degree), C.c_int(F), C.c_int(act), _p(X, C.c_float),
+                          _p(t, C.c_float), C.c_longlong(N), _p(genes, C.c_float), C.c_double(cut),
+                          _p(counts, C.c_longlong), _p(fom, C.c_double), C.byref(near), C.c_double(delta))
+    return counts, fom, int(near.value)
+
+
 def philox4x32_10(key, ctr):
     """oracle_philox4x32_10: four uint32 words for (key[2], counter[4])."""
     k = np.asarray(key, dtype=np.uint32)

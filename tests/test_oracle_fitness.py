@@ -190,3 +190,36 @@ def test_p13_sigmoid(orc):
     big = np.array([[1.0, 0.0], [-1.0, 0.0]], dtype=np.float32) * 3e38
     f = orc.fitness(CHEB, 1, X, np.array([1.0], dtype=np.float32), big)
     assert f[0] == 0.0 and f[1] == 1.0 and not np.any(np.isnan(f))
+
+
+def test_p24_figures_of_merit(orc):
+    # L301 definitions on a hand-made case.  Identity activation, Chebyshev d=1, F=1: Out = c0 + c1*x, genes (0, 1)
+    # -> Out = x.  Patterns x = (0.9, 0.8, 0.7 | 0.6, 0.2, 0.1, -0.3, -0.5), truth (1,1,1 | 0 ...) with cut 0.5:
+    X = np.array([0.9, 0.8, 0.7, 0.6, 0.2, 0.1, -0.3, -0.5, 0.4, 0.3], dtype=np.float32)[:, None]
+    t = np.array([1, 1, 1, 0, 0, 0, 0, 0, 1, 1], dtype=np.float32)
+    g = np.array([0.0, 1.0], dtype=np.float32)
+    counts, fom, near = orc.classify(CHEB, 1, X, t, g, act=IDENTITY, cut=0.5)
+    # predicted GC: x > 0.5 -> first four.  TP = 3, FP = 1 (x=0.6), TN = 4, FN = 2 (x=0.4, 0.3)
+    assert counts.tolist() == [3, 1, 4, 2]
+    assert fom[0] == 7 / 10           # accuracy: correctly classified / total
+    assert fom[1] == 3 / 5            # completeness: GCs classified as such / all GCs
+    assert fom[2] == 1 / 5            # contamination: non-GCs classified as GC / all non-GCs (L301, literal)
+    assert near == 0
+    # the cut is exclusive (y > cut), and sigmoid(z) > 0.5 <=> z > 0
+    Xz = np.array([0.0, 1e-3, -1e-3], dtype=np.float32)[:, None]
+    c2, _, n2 = orc.classify(CHEB, 1, Xz, np.array([1, 1, 0], dtype=np.float32), g, act=SIGMOID, cut=0.5, delta=1e-6)
+    assert c2.tolist() == [1, 0, 1, 1] and n2 == 1
+    # degenerate denominators give 0, not NaN
+    c3, f3, _ = orc.classify(CHEB, 1, X[:3], t[:3], g, act=IDENTITY, cut=0.5)
+    assert c3.tolist() == [3, 0, 0, 0] and f3.tolist() == [1.0, 1.0, 0.0]
+    # consistency with forward(): counts recomputed from the oracle's own outputs
+    rng = np.random.default_rng(30)
+    Xr = rng.uniform(-1, 1, (500, 4)).astype(np.float32)
+    gr = rng.standard_normal(orc.num_terms(TRIG, 3, 4)).astype(np.float32)
+    tr = rng.integers(0, 2, 500).astype(np.float32)
+    _, y = orc.forward(TRIG, 3, Xr, gr)
+    cr, fr, _ = orc.classify(TRIG, 3, Xr, tr, gr)
+    pred, truth = y > 0.5, tr > 0.5
+    assert cr.tolist() == [int((pred & truth).sum()), int((pred & ~truth).sum()), int((~pred & ~truth).sum()),
+                           int((~pred & truth).sum())]
+    assert abs(fr[0] - np.mean(pred == truth)) < 1e-15
