@@ -104,6 +104,12 @@ int game_fitness_host(game_ctx *ctx, const float *pop, int P, float *out);
  * y_out[n] = act(z).  genes: K fp32, z_out / y_out: N fp32, either may be NULL.  DEV pointers. fp32. */
 int game_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out);
 
+/* Figures of merit of a trained chromosome on the loaded dataset (L301).  A pattern is classified as class 1
+ * when act(z) > cut and belongs to class 1 when its target > 0.5.  counts (DEV, 4 x int64) = {TP, FP, TN, FN};
+ * fom (DEV, 3 x double) = {accuracy (TP+TN)/N, completeness TP/(TP+FN), contamination FP/(FP+TN)}, 0 for an
+ * empty denominator.  genes: K fp32 DEV.  fp32 forward pass.  Asynchronous. */
+int game_classify(game_ctx *ctx, const float *genes, float cut, long long *counts, double *fom);
+
 /* Install a population (P x K fp32, DEV) instead of the random initial one; resets nothing else. */
 int game_set_population(game_ctx *ctx, const float *pop, int P);
 /* Set the absolute generation counter (checkpoint resume; Philox draws are keyed on it). */

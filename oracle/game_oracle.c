@@ -36,7 +36,7 @@
 #include <omp.h>
 #endif
 
-enum { FAM_TRIG = 0, FAM_CHEB = 1 };
+enum { FAM_TRIG = 0, FAM_CHEB = 1, FAM_TRIG_TIED = 2, FAM_POLY_TIED = 3 };
 enum { ACT_SIGMOID = 0, ACT_IDENTITY = 1 };
 enum { ERR_MSE = 0, ERR_TMSE = 1, ERR_RMSE = 2 };
 enum { SEL_TOURNAMENT = 0, SEL_ROULETTE = 1 };
@@ -79,11 +79,35 @@ int oracle_num_terms(int family, int degree, int F)
     if (F < 1 || degree < 1) return -1;
     if (family == FAM_TRIG) return F * (2 * degree + 1);
     if (family == FAM_CHEB) return F * (degree + 1);
+    if (family == FAM_TRIG_TIED) return 2 * degree + 1;   /* eq. 7 with B = 2: the paper's own chromosome (L105) */
+    if (family == FAM_POLY_TIED) return degree + 1;       /* eq. 7 with B = 1, g(x) = x (L89) */
     return -1;
+}
+
+/* Paper-literal models: ONE coefficient set shared by every feature (eq. 2 and eq. 9 as printed, L57, L100-L103):
+ *   TRIG_TIED: Out = a_0 + sum_m a_m sum_i cos(m f_i) + sum_m b_m sum_i sin(m f_i), genes [a_0, a_1..a_d, b_1..b_d];
+ *              the per-pattern sums of cosines and sines are the paper's two precomputed vectors (L254).
+ *   POLY_TIED: Out = a_0 + sum_j a_j sum_i f_i^j (eq. 2 with g(x) = x, powers), genes [a_0..a_d].
+ * The constant a_0 appears once, not once per feature. */
+static void expand_row_tied(int family, int d, int F, const float *x, double *phi)
+{
+    int K = family == FAM_TRIG_TIED ? 2 * d + 1 : d + 1;
+    for (int k = 0; k < K; ++k) phi[k] = 0.0;
+    phi[0] = 1.0;
+    for (int i = 0; i < F; ++i) {
+        double xi = (double)x[i];
+        if (family == FAM_TRIG_TIED) {
+            for (int m = 1; m <= d; ++m) { phi[m] += cos((double)m * xi); phi[d + m] += sin((double)m * xi); }
+        } else {
+            double pw = 1.0;
+            for (int j = 1; j <= d; ++j) { pw *= xi; phi[j] += pw; }
+        }
+    }
 }
 
 static void expand_row(int family, int d, int F, const float *x, double *phi)
 {
+    if (family == FAM_TRIG_TIED || family == FAM_POLY_TIED) { expand_row_tied(family, d, F, x, phi); return; }
     for (int i = 0; i < F; ++i) {
         double xi = (double)x[i];
         if (family == FAM_TRIG) {

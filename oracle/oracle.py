@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "game_oracle.c")
 _LIB = os.path.join(_HERE, "libgame_oracle.so")
 
-TRIG, CHEB = 0, 1
+TRIG, CHEB, TRIG_TIED, POLY_TIED = 0, 1, 2, 3
 SIGMOID, IDENTITY = 0, 1
 MSE, TMSE, RMSE = 0, 1, 2
 TOURNAMENT, ROULETTE = 0, 1

@@ -26,7 +26,7 @@ ERROR_NAMES = {1: "INVALID_ARG", 2: "NOT_LOADED", 3: "ALLOC", 4: "CUDA", 5: "UNS
 SYMBOLS = [
     "game_create", "game_destroy", "game_num_terms", "game_generation", "game_last_error",
     "game_set_stream", "game_set_activation", "game_set_error", "game_set_path", "game_resolved_path",
-    "game_load", "game_load_host", "game_fitness", "game_fitness_host", "game_predict",
+    "game_load", "game_load_host", "game_fitness", "game_fitness_host", "game_predict", "game_classify",
     "game_set_population", "game_set_generation", "game_evolve", "game_get_population",
     "game_get_population_host", "game_rank", "game_ga_step", "game_init_population", "game_philox",
     "game_launch_count", "game_set_kernel_timing", "game_get_kernel_timing",
@@ -82,6 +82,7 @@ def load_library():
         L.game_fitness.argtypes = [vp, vp, i, vp]
         L.game_fitness_host.argtypes = [vp, vp, i, vp]
         L.game_predict.argtypes = [vp, vp, vp, vp]
+        L.game_classify.argtypes = [vp, vp, C.c_float, vp, vp]
         L.game_set_population.argtypes = [vp, vp, i]
         L.game_set_generation.argtypes = [vp, ll]
         L.game_evolve.argtypes = [vp, i, u64, C.POINTER(game_ga_params), C.POINTER(game_result)]
@@ -222,6 +223,13 @@ class Game:
         y = t.empty(self.N, dtype=t.float32, device=genes.device) if want_y else None
         self._ck(self._L.game_predict(self._h, _dev(genes, t.float32), _dev(z), _dev(y)))
         return z, y
+
+    def classify(self, genes, cut=0.5):
+        t = self._torch
+        counts = t.empty(4, dtype=t.int64, device=genes.device)
+        fom = t.empty(3, dtype=t.float64, device=genes.device)
+        self._ck(self._L.game_classify(self._h, _dev(genes, t.float32), cut, _dev(counts), _dev(fom)))
+        return counts, fom
 
     def set_population(self, pop):
         self._ck(self._L.game_set_population(self._h, _dev(pop, self._torch.float32), pop.shape[0]))

@@ -107,6 +107,52 @@ __global__ void predict_kernel(const float *__restrict__ ET, long long Npad, lon
     if (y_out) y_out[n] = act == GAME_ACT_SIGMOID ? 1.0f / (1.0f + expf(-z)) : z;
 }
 
+// Figures of merit of the test / run use cases: forward pass as above, class = act(z) > cut,
+// truth = target > 0.5, counts {TP, FP, TN, FN} by integer atomics (exact, order-independent), then
+// accuracy (TP+TN)/N, completeness TP/(TP+FN), contamination FP/(FP+TN) (DESIGN G23) by the last CTA.
+__global__ void classify_kernel(const float *__restrict__ ET, long long Npad, long long N, int K,
+                                const float *__restrict__ genes, const float *__restrict__ tgt, int act, float cut,
+                                unsigned long long *counts, double *fom, unsigned int *ticket)
+{
+    extern __shared__ float g[];
+    __shared__ unsigned int sc[4];
+    for (int k = threadIdx.x; k < K; k += blockDim.x) g[k] = genes[k];
+    if (threadIdx.x < 4) sc[threadIdx.x] = 0;
+    __syncthreads();
+    long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n < N) {
+        float z = 0.f;
+        for (int k = 0; k < K; ++k) z = fmaf(ET[(long long)k * Npad + n], g[k], z);
+        float y = act == GAME_ACT_SIGMOID ? 1.0f / (1.0f + expf(-z)) : z;
+        bool pred = y > cut, truth = tgt[n] > 0.5f;
+        atomicAdd(&sc[pred ? (truth ? 0 : 1) : (truth ? 3 : 2)], 1u);
+    }
+    __syncthreads();
+    if (threadIdx.x < 4 && sc[threadIdx.x]) atomicAdd(&counts[threadIdx.x], (unsigned long long)sc[threadIdx.x]);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0 && atomicAdd(ticket, 1u) == gridDim.x - 1) {      // last CTA: every count has landed
+        __threadfence();
+        volatile unsigned long long *c = counts;
+        double tp = (double)c[0], fp = (double)c[1], tn = (double)c[2], fn = (double)c[3];
+        fom[0] = N > 0 ? (tp + tn) / (double)N : 0.0;
+        fom[1] = tp + fn > 0 ? tp / (tp + fn) : 0.0;
+        fom[2] = fp + tn > 0 ? fp / (fp + tn) : 0.0;
+        *ticket = 0;
+    }
+}
+
+int launch_classify(game_ctx *ctx, const float *genes, float cut, long long *counts, double *fom, unsigned int *ticket)
+{
+    GAME_CUDA(ctx, cudaMemsetAsync(counts, 0, 4 * sizeof(long long), ctx->stream));
+    int blocks = (int)((ctx->N + 255) / 256);
+    classify_kernel<<<blocks, 256, ctx->K * sizeof(float), ctx->stream>>>(ctx->ET, ctx->Npad, ctx->N, ctx->K, genes, ctx->t,
+                                                                         ctx->act, cut, (unsigned long long *)counts, fom,
+                                                                         ticket);
+    GAME_LAUNCHED(ctx);
+    return GAME_OK;
+}
+
 int launch_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out)
 {
     int blocks = (int)((ctx->N + 255) / 256);

@@ -184,8 +184,9 @@ int game_create(int family, int degree, int F, game_ctx **out)
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
-    if (e == cudaSuccess) e = cudaMalloc(&c->state, sizeof(DevState));
-    if (e == cudaSuccess) e = cudaMemset(c->state, 0, sizeof(DevState));
+    if (e == cudaSuccess) e = cudaMalloc(&c->state, sizeof(DevState) + 16);
+    if (e == cudaSuccess) e = cudaMemset(c->state, 0, sizeof(DevState) + 16);
+    c->ticket = reinterpret_cast<unsigned int *>(c->state + 1);
     if (e != cudaSuccess) {       // no CPU fallback: without a device there is no context
         cudaGetLastError();
         delete c;
@@ -284,6 +285,14 @@ int game_predict(game_ctx *c, const float *genes, float *z_out, float *y_out)
     if (!c->N) return fail(c, GAME_ERR_NOT_LOADED, "game_predict before game_load");
     if (!genes) return fail(c, GAME_ERR_INVALID_ARG, "game_predict: genes is NULL");
     return launch_predict(c, genes, z_out, y_out);
+}
+
+int game_classify(game_ctx *c, const float *genes, float cut, long long *counts, double *fom)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!c->N) return fail(c, GAME_ERR_NOT_LOADED, "game_classify before game_load");
+    if (!genes || !counts || !fom) return fail(c, GAME_ERR_INVALID_ARG, "game_classify: NULL pointer");
+    return launch_classify(c, genes, cut, counts, fom, c->ticket);
 }
 
 int game_set_population(game_ctx *c, const float *pop, int P)

@@ -73,6 +73,7 @@ struct game_ctx {
     unsigned long long *rprefix = nullptr;   // roulette inclusive prefix sums
     size_t pop_cap = 0;                      // capacity in chromosomes of the buffers above
     game::DevState *state = nullptr;
+    unsigned int *ticket = nullptr;          // last-CTA ticket for classify_kernel (lives behind `state`)
 
     // scratch
     float *partial = nullptr;  // n_chunks x Ppad per-chunk error sums
@@ -125,6 +126,7 @@ int launch_check_finite(game_ctx *ctx, const float *X, long long nX, const float
 int launch_expand_fp32(game_ctx *ctx);      // X -> ET
 int launch_expand_fp16(game_ctx *ctx, float *maxabs_dev);   // X -> E16
 int launch_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out);
+int launch_classify(game_ctx *ctx, const float *genes, float cut, long long *counts, double *fom, unsigned int *ticket);
 
 // fitness_fp32.cu
 size_t fitness_partial_floats(const game_ctx *ctx, int P);

@@ -212,6 +212,29 @@ def test_predict_parity(orc):
     assert np.allclose(y.cpu().numpy(), yr, rtol=1e-5, atol=1e-6)
 
 
+def test_classify_figures_of_merit(orc):
+    # L301: counts are integers decided by a float (y > cut).  The kernel decides in fp32, the oracle in fp64,
+    # so patterns the oracle finds within delta of the cut may fall either way; everything else must agree.
+    for cfg, scale in ((1, 1.0), (3, 0.05)):
+        w = wl.config(cfg)
+        fam, d = w.family, w.degree
+        X, t, c0 = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+        rng = np.random.default_rng(26)
+        genes = c0 if c0 is not None else (rng.standard_normal(w.K) * scale).astype(np.float32)
+        ctx = make_ctx(fam, d, X, t)
+        counts, fom = ctx.classify(dev(genes), 0.5)
+        counts, fom = counts.cpu().numpy(), fom.cpu().numpy()
+        ref_c, ref_f, near = orc.classify(fam, d, X, t, genes, cut=0.5, delta=1e-5)
+        assert counts.sum() == w.N == ref_c.sum()
+        assert np.abs(counts - ref_c).max() <= near, (counts, ref_c, near)
+        # the ratios are exactly those of the kernel's own counts, and within near/N of the oracle's
+        tp, fp, tn, fn = [float(v) for v in counts]
+        assert fom[0] == (tp + tn) / w.N and fom[1] == tp / (tp + fn) and fom[2] == fp / (fp + tn)
+        assert np.abs(fom - ref_f).max() <= (near + 1e-9) / min(tp + fn, fp + tn)
+        if c0 is not None:      # planted labels with 10 % flips: accuracy ~ 0.9
+            assert 0.85 < fom[0] < 0.95
+
+
 def test_error_paths():
     ctx = g.Game(TRIG, 2, 3)
     pop = torch.zeros((4, ctx.K), device="cuda")
