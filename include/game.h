@@ -32,7 +32,11 @@ typedef struct game_ctx game_ctx; /* opaque */
 enum { GAME_OK = 0, GAME_ERR_INVALID_ARG = 1, GAME_ERR_NOT_LOADED = 2, GAME_ERR_ALLOC = 3,
        GAME_ERR_CUDA = 4, GAME_ERR_UNSUPPORTED = 5, GAME_ERR_NONFINITE_INPUT = 6 };
 
-enum { GAME_TRIG = 0, GAME_CHEB = 1 };                 /* expansion family: eq. 8-9 (L95-L103) / eq. 1 with g^j = T_j */
+/* Expansion family.  TRIG / CHEB: one coefficient per (feature, term), K = F(2d+1) / F(d+1) (eq. 8-9 L95-L103 /
+ * eq. 1 with g^j = T_j; DESIGN G1).  TRIG_TIED / POLY_TIED: the paper-literal models, one coefficient set shared
+ * by all features acting on per-pattern sums over features (eq. 9 / eq. 2 as printed, L57, L100-L105, L254):
+ * K = 2d+1 genes [a_0, a_1..a_d, b_1..b_d] on (1, sum_i cos(m f_i), sum_i sin(m f_i)); K = d+1 genes on sum_i f_i^j. */
+enum { GAME_TRIG = 0, GAME_CHEB = 1, GAME_TRIG_TIED = 2, GAME_POLY_TIED = 3 };
 enum { GAME_ACT_SIGMOID = 0, GAME_ACT_IDENTITY = 1 };  /* DESIGN G4; identity is the paper-literal eq. 2 */
 enum { GAME_ERR_MSE = 0, GAME_ERR_TMSE = 1, GAME_ERR_RMSE = 2 };   /* eq. 4, eq. 10, eq. 5 (L71-L75, L113) */
 enum { GAME_SEL_TOURNAMENT = 0, GAME_SEL_ROULETTE = 1 };           /* L147, L290; DESIGN G14 */

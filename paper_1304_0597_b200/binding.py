@@ -13,7 +13,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgame_b200.so")
 
-GAME_TRIG, GAME_CHEB = 0, 1
+GAME_TRIG, GAME_CHEB, GAME_TRIG_TIED, GAME_POLY_TIED = 0, 1, 2, 3
 GAME_ACT_SIGMOID, GAME_ACT_IDENTITY = 0, 1
 GAME_ERR_MSE, GAME_ERR_TMSE, GAME_ERR_RMSE = 0, 1, 2
 GAME_SEL_TOURNAMENT, GAME_SEL_ROULETTE = 0, 1

@@ -73,8 +73,57 @@ __global__ void expand_kernel(const float *__restrict__ X, long long N, int F, i
     }
 }
 
+// Paper-literal tied families (eq. 2 / eq. 9 as printed, L57, L100-L103): one coefficient set for all features,
+// so a term is a per-pattern SUM over features -- the "sums of sines and cosines ... stored in two vectors"
+// the paper precomputes (L254).  One thread per pattern, fp64 sums in ascending feature order.
+template <typename OutT, bool PATTERN_MAJOR>
+__global__ void expand_tied_kernel(const float *__restrict__ X, long long N, int F, int family, int d,
+                                   OutT *__restrict__ E, long long ld, float *maxabs)
+{
+    long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    float local_max = 0.f;
+    if (n < N) {
+        double sum[65];
+        const int K = family == GAME_TRIG_TIED ? 2 * d + 1 : d + 1;
+        for (int k = 0; k < K; ++k) sum[k] = 0.0;
+        sum[0] = 1.0;
+        for (int i = 0; i < F; ++i) {
+            double x = (double)X[n * F + i];
+            if (family == GAME_TRIG_TIED) {
+                for (int m = 1; m <= d; ++m) {
+                    double s, c;
+                    sincos((double)m * x, &s, &c);
+                    sum[m] += c;
+                    sum[d + m] += s;
+                }
+            } else {
+                double pw = 1.0;
+                for (int j = 1; j <= d; ++j) { pw *= x; sum[j] += pw; }
+            }
+        }
+        for (int k = 0; k < K; ++k) {
+            float f = (float)sum[k];
+            local_max = fmaxf(local_max, fabsf(f));
+            if (PATTERN_MAJOR) E[(((n >> 8) * (ld >> 6) + (k >> 6)) << 14) + ((n & 255) << 6) + (k & 63)] = (OutT)f;
+            else E[(long long)k * ld + n] = (OutT)f;
+        }
+    }
+    if (maxabs) {
+        for (int o = 16; o; o >>= 1) local_max = fmaxf(local_max, __shfl_xor_sync(0xffffffffu, local_max, o));
+        if ((threadIdx.x & 31) == 0 && local_max > 0.f) atomicMax((int *)maxabs, __float_as_int(local_max));
+    }
+}
+
+static bool tied(const game_ctx *ctx) { return ctx->family == GAME_TRIG_TIED || ctx->family == GAME_POLY_TIED; }
+
 int launch_expand_fp32(game_ctx *ctx)
 {
+    if (tied(ctx)) {
+        expand_tied_kernel<float, false><<<(unsigned)((ctx->N + 127) / 128), 128, 0, ctx->stream>>>(
+            ctx->X, ctx->N, ctx->F, ctx->family, ctx->degree, ctx->ET, ctx->Npad, nullptr);
+        GAME_LAUNCHED(ctx);
+        return GAME_OK;
+    }
     dim3 grid((unsigned)((ctx->N + 255) / 256), (unsigned)ctx->F);
     expand_kernel<float, false><<<grid, 256, 0, ctx->stream>>>(ctx->X, ctx->N, ctx->F, ctx->family, ctx->degree,
                                                                 ctx->ET, ctx->Npad, nullptr);
@@ -84,6 +133,12 @@ int launch_expand_fp32(game_ctx *ctx)
 
 int launch_expand_fp16(game_ctx *ctx, float *maxabs_dev)
 {
+    if (tied(ctx)) {
+        expand_tied_kernel<__half, true><<<(unsigned)((ctx->N + 127) / 128), 128, 0, ctx->stream>>>(
+            ctx->X, ctx->N, ctx->F, ctx->family, ctx->degree, ctx->E16, ctx->Kpad, maxabs_dev);
+        GAME_LAUNCHED(ctx);
+        return GAME_OK;
+    }
     dim3 grid((unsigned)((ctx->N + 255) / 256), (unsigned)ctx->F);
     expand_kernel<__half, true><<<grid, 256, 0, ctx->stream>>>(ctx->X, ctx->N, ctx->F, ctx->family, ctx->degree,
                                                                 ctx->E16, ctx->Kpad, maxabs_dev);

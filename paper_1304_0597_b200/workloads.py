@@ -14,7 +14,7 @@ from dataclasses import dataclass, field, replace
 
 import numpy as np
 
-TRIG, CHEB = 0, 1
+TRIG, CHEB, TRIG_TIED, POLY_TIED = 0, 1, 2, 3
 SIGMOID, IDENTITY = 0, 1
 MSE, TMSE, RMSE = 0, 1, 2
 
@@ -44,6 +44,10 @@ class Workload:
 
     @property
     def K(self):
+        if self.family == TRIG_TIED:      # paper-literal eq. 7: (B*d)+1 genes with B = 2
+            return 2 * self.degree + 1
+        if self.family == POLY_TIED:
+            return self.degree + 1
         return self.F * (2 * self.degree + 1 if self.family == TRIG else self.degree + 1)
 
     def scaled(self, N=None, P=None, generations=None):
@@ -64,6 +68,15 @@ CONFIGS = [
 ]
 
 
+def paper_literal(degree=4, N=2100, generations=4000):
+    """The paper's own experiment shape (L187, L273, L282-L291, eq. 6-7): 2100 patterns x 11 features, tied
+    trigonometric model with 2d+1 genes, population 2*11+1 = 23, tournament 4, crossover 0.9, mutation 0.2,
+    elitism 2, TMSE 0.49, normal initial population.  Identity output as eq. 9 prints it.  Larger N replicates
+    the 2100 rows, as the paper's scaling runs do (L326)."""
+    return Workload("paper-literal-d%d" % degree, N, 11, TRIG_TIED, degree, 23, generations, 1, "planted_binary",
+                    flip=0.10, act=IDENTITY, tournament_size=4, p_mutation=0.2, extra={"base_rows": 2100})
+
+
 def config(i):
     """1-based, as BASELINE.json / SURVEY.md number them."""
     return CONFIGS[i - 1]
@@ -74,6 +87,11 @@ def make(w, forward=None):
 
     Draw order per recipe is fixed; the same bytes go to the oracle and to the GPU library.
     """
+    base = w.extra.get("base_rows")
+    if base and w.N > base:             # the paper's scaling construction: replicate the catalogue's rows (L326)
+        X, t, c0 = make(replace(w, N=base), forward)
+        reps = -(-w.N // base)
+        return np.tile(X, (reps, 1))[:w.N].copy(), np.tile(t, reps)[:w.N].copy(), c0
     rng = np.random.default_rng(w.seed)
     N, F, K = w.N, w.F, w.K
     if w.kind == "mixture":
@@ -87,7 +105,7 @@ def make(w, forward=None):
     if w.kind == "planted_binary":
         c0 = rng.standard_normal(K).astype(np.float32)
         z, _ = forward(X, c0)
-        t = (np.asarray(z, dtype=np.float64) > 0.0)
+        t = (np.asarray(z, dtype=np.float64) > (0.0 if w.act == SIGMOID else 0.5))     # output above one half
         flips = rng.random(N) < w.flip
         t = np.where(flips, ~t, t)
         return X, t.astype(np.float32), c0

@@ -379,3 +379,26 @@ def test_full_size_sampled(orc, cfg, nsample):
     # properties that hold at any size: elites are copies of the previous winner -> rows 0,1 identical
     assert np.array_equal(pop[0], pop[1]) and fit[0] == fit[1]
     assert np.all(np.abs(pop) <= 1.0) and np.all(np.isfinite(fit)) and np.all(fit >= 0)
+
+
+# ---- the paper-literal tied-coefficient models ------------------------------------------
+@pytest.mark.parametrize("fam,d", [(2, 1), (2, 8), (3, 1), (3, 6)])
+def test_tied_families_fitness(orc, fam, d):
+    rng = np.random.default_rng(27)
+    N, F, P = 2100, 11, 23
+    X = rng.uniform(-1, 1, (N, F)).astype(np.float32)
+    t = rng.integers(0, 2, N).astype(np.float32)
+    K = orc.num_terms(fam, d, F)
+    pop = rng.uniform(-1, 1, (P, K)).astype(np.float32)
+    for act, err, R in ((IDENTITY, MSE, 0.0), (IDENTITY, TMSE, 0.49), (SIGMOID, TMSE, 0.49), (SIGMOID, RMSE, 0.0)):
+        ctx = make_ctx(fam, d, X, t, act, err, R)
+        assert ctx.K == K and ctx.resolved_path(P) == g.GAME_PATH_FP32
+        got = ctx.fitness(dev(pop)).cpu().numpy()
+        check_fitness(orc, got, fam, d, X, t, pop, act, err, R, g.GAME_PATH_FP32, "tied fam %d d %d" % (fam, d))
+
+
+def test_trajectory_paper_literal(orc):
+    # the paper's own experiment shape and settings (eq. 6-7) on stand-in data, 40 generations
+    trajectory(orc, wl.paper_literal(degree=4), 40)
+    # and on row-replicated data (L326): same shape of run, 4x the rows
+    trajectory(orc, wl.paper_literal(degree=2, N=8400), 6)
