@@ -228,58 +228,70 @@ constexpr int SMALL_SMEM = SKC * SLAB * 4 + SKC * (SP + 4) * 4;      // E chunk 
 
 __global__ void __launch_bounds__(128)
 fitness_small_kernel(const float *__restrict__ ET, long long Npad, long long N, int K, const float *__restrict__ pop,
-                     int P, const float *__restrict__ tgt, FitnessCfg cfg, float *__restrict__ partial, int Ppad,
-                     const DevState *state)
+                     int P, const float *__restrict__ tgt, int n_slabs, int spc, int kcap, FitnessCfg cfg,
+                     float *__restrict__ partial, int Ppad, const DevState *state)
 {
     if (state && state->stopped) return;
     extern __shared__ __align__(16) float small_smem[];
     float (*Es)[SLAB] = reinterpret_cast<float (*)[SLAB]>(small_smem);                       // [k][n], as in ET
-    float (*Cs)[SP + 4] = reinterpret_cast<float (*)[SP + 4]>(small_smem + SKC * SLAB);      // [k][p]; +4: transposed
+    float (*Cs)[SP + 4] = reinterpret_cast<float (*)[SP + 4]>(small_smem + kcap * SLAB);     // [k][p]; +4: transposed
     __shared__ float red[4][SP];                                                             // stores 4-way, not 32-way
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const long long n0 = (long long)blockIdx.x * SLAB;
-    const long long n = n0 + tid;
     const int p0 = blockIdx.y * SP;
-    float acc[SP];
-#pragma unroll
-    for (int j = 0; j < SP; ++j) acc[j] = 0.f;
-    for (int k0 = 0; k0 < K; k0 += SKC) {
-        const int kc = min(SKC, K - k0);
-        __syncthreads();
-        // the whole E chunk in flight at once (cp.async, 16 B per request): one memory latency, not kc of them
-        for (int i = tid; i < kc * (SLAB / 4); i += 128) {
-            const int kk = i / (SLAB / 4), c4 = i % (SLAB / 4);
-            const float *src = ET + (long long)(k0 + kk) * Npad + n0 + c4 * 4;
-            const unsigned dst = (unsigned)__cvta_generic_to_shared(&Es[kk][c4 * 4]);
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-        }
-        for (int i = tid; i < SKC * SP; i += 128) {          // Cs[k][p] <- pop[p0+p][k0+k] (zero-filled outside), k fastest
-            const int pp = i / SKC, kk = i % SKC;
+    const bool one_chunk = K <= kcap;          // then the chromosomes are staged once for all of this CTA's slabs
+    auto stage_C = [&](int k0, int kc) {       // Cs[k][p] <- pop[p0+p][k0+k] (zero-filled outside), k fastest
+        for (int i = tid; i < kcap * SP; i += 128) {
+            const int pp = i / kcap, kk = i % kcap;
             const bool in = p0 + pp < P && kk < kc;
             const float *src = in ? pop + (long long)(p0 + pp) * K + k0 + kk : pop;
             const unsigned dst = (unsigned)__cvta_generic_to_shared(&Cs[kk][pp]);
             asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(in ? 4 : 0) : "memory");
         }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-        asm volatile("cp.async.wait_group 0;" ::: "memory");
-        __syncthreads();
-#pragma unroll 4
-        for (int kk = 0; kk < kc; ++kk) {
-            const float e = Es[kk][tid];
+    };
+    if (one_chunk) stage_C(0, K);
+    float esum[SP];
 #pragma unroll
-            for (int j = 0; j < SP; j += 4) {
-                const float4 c4 = *reinterpret_cast<const float4 *>(&Cs[kk][j]);
-                acc[j] = fmaf(e, c4.x, acc[j]);
-                acc[j + 1] = fmaf(e, c4.y, acc[j + 1]);
-                acc[j + 2] = fmaf(e, c4.z, acc[j + 2]);
-                acc[j + 3] = fmaf(e, c4.w, acc[j + 3]);
+    for (int j = 0; j < SP; ++j) esum[j] = 0.f;
+    const int slab_hi = min((int)(blockIdx.x + 1) * spc, n_slabs);
+    for (int slab = blockIdx.x * spc; slab < slab_hi; ++slab) {
+        const long long n0 = (long long)slab * SLAB;
+        const long long n = n0 + tid;
+        float acc[SP];
+#pragma unroll
+        for (int j = 0; j < SP; ++j) acc[j] = 0.f;
+        for (int k0 = 0; k0 < K; k0 += kcap) {
+            const int kc = min(kcap, K - k0);
+            __syncthreads();
+            // the whole E chunk in flight at once (cp.async, 16 B per request): one memory latency, not kc of them
+            for (int i = tid; i < kc * (SLAB / 4); i += 128) {
+                const int kk = i / (SLAB / 4), c4 = i % (SLAB / 4);
+                const float *src = ET + (long long)(k0 + kk) * Npad + n0 + c4 * 4;
+                const unsigned dst = (unsigned)__cvta_generic_to_shared(&Es[kk][c4 * 4]);
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+            }
+            if (!one_chunk) stage_C(k0, kc);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncthreads();
+#pragma unroll 4
+            for (int kk = 0; kk < kc; ++kk) {
+                const float e = Es[kk][tid];
+#pragma unroll
+                for (int j = 0; j < SP; j += 4) {
+                    const float4 c4 = *reinterpret_cast<const float4 *>(&Cs[kk][j]);
+                    acc[j] = fmaf(e, c4.x, acc[j]);
+                    acc[j + 1] = fmaf(e, c4.y, acc[j + 1]);
+                    acc[j + 2] = fmaf(e, c4.z, acc[j + 2]);
+                    acc[j + 3] = fmaf(e, c4.w, acc[j + 3]);
+                }
             }
         }
-    }
-    const bool valid = n < N;
-    const float t = tgt[n];
+        const bool valid = n < N;
+        const float t = tgt[n];
 #pragma unroll
-    for (int j = 0; j < SP; ++j) acc[j] = act_err(acc[j], t, valid, cfg.act, cfg.err, cfg.R);
+        for (int j = 0; j < SP; ++j) esum[j] += act_err(acc[j], t, valid, cfg.act, cfg.err, cfg.R);
+    }
+    float (&acc)[SP] = esum;
     // butterfly: after the step with offset o each lane holds half as many columns, summed over lane pairs;
     // a + b is commutative, so every chromosome sees the same fixed tree whatever its column (DESIGN P20)
 #pragma unroll
@@ -328,8 +340,15 @@ int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, cons
 {
     int Ppad = ((P + 255) / 256) * 256;
     FitnessCfg cfg{ctx->act, ctx->err, ctx->R};
-    if ((long long)ctx->n_slabs * ((P + BP - 1) / BP) < 2LL * ctx->sm_count) {       // under two waves of big tiles
-        dim3 grid((unsigned)ctx->n_slabs, (unsigned)((P + SP - 1) / SP));
+    // under two waves of big tiles, or so few chromosomes that a 128-wide tile would mostly compute padding
+    if ((long long)ctx->n_slabs * ((P + BP - 1) / BP) < 2LL * ctx->sm_count || P <= 2 * SP) {
+        const int ptiles = (P + SP - 1) / SP;
+        long long spc_ll = ((long long)ctx->n_slabs * ptiles) / ((long long)ctx->sm_count * 32);
+        const int spc = (int)(spc_ll < 1 ? 1 : spc_ll > 64 ? 64 : spc_ll);
+        const int n_chunks = (ctx->n_slabs + spc - 1) / spc;
+        const int kcap = ctx->K < SKC ? ctx->K : SKC;
+        const int smem = kcap * (SLAB + SP + 4) * 4;
+        dim3 grid((unsigned)n_chunks, (unsigned)ptiles);
         static bool attr_set = false;
         if (!attr_set) {
             GAME_CUDA(ctx, cudaFuncSetAttribute(fitness_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMALL_SMEM));
@@ -337,12 +356,12 @@ int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, cons
         }
         {
             KernelTimer timer(ctx);
-            fitness_small_kernel<<<grid, 128, SMALL_SMEM, ctx->stream>>>(ctx->ET, ctx->Npad, ctx->N, ctx->K, pop, P, ctx->t, cfg,
-                                                              ctx->partial, Ppad, state);
+            fitness_small_kernel<<<grid, 128, smem, ctx->stream>>>(ctx->ET, ctx->Npad, ctx->N, ctx->K, pop, P, ctx->t,
+                                                                   ctx->n_slabs, spc, kcap, cfg, ctx->partial, Ppad, state);
         }
         GAME_LAUNCHED(ctx);
-        if (defer) { defer->n_chunks = ctx->n_slabs; defer->Ppad = Ppad; return GAME_OK; }
-        return launch_finalize(ctx, ctx->n_slabs, Ppad, P, out, state);
+        if (defer) { defer->n_chunks = n_chunks; defer->Ppad = Ppad; return GAME_OK; }
+        return launch_finalize(ctx, n_chunks, Ppad, P, out, state);
     }
     int spc = pick_slabs_per_cta(ctx, P);
     int n_chunks = (ctx->n_slabs + spc - 1) / spc;
