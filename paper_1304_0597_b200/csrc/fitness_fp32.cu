@@ -215,6 +215,43 @@ __global__ void finalize_kernel(const float *__restrict__ partial, int n_chunks,
     }
 }
 
+// Many slabs, few chromosomes (config 4: 7814 x 256): one CTA per 32 chromosomes would leave the GPU idle, so the
+// slab axis is split over FIN_SPLIT CTAs that each total a contiguous range in fp64, and a second tiny kernel adds
+// the FIN_SPLIT totals in ascending order.  Fixed order again: reproducible, and the same for every caller.
+__global__ void finalize_split_kernel(const float *__restrict__ partial, int n_chunks, int Ppad, int P,
+                                      double *__restrict__ fin2, const DevState *state)
+{
+    if (state && state->stopped) return;
+    __shared__ double red[32][33];
+    const int c = threadIdx.x, r = threadIdx.y;
+    const int p = blockIdx.x * 32 + c;
+    const int len = (n_chunks + FIN_SPLIT - 1) / FIN_SPLIT;
+    const int lo = blockIdx.y * len, hi = min(lo + len, n_chunks);
+    double s = 0.0;
+    if (p < P)
+        for (int ch = lo + r; ch < hi; ch += 32) s += (double)partial[(long long)ch * Ppad + p];
+    red[r][c] = s;
+    __syncthreads();
+    if (r == 0 && p < P) {
+        double tot = 0.0;
+        for (int q = 0; q < 32; ++q) tot += red[q][c];
+        fin2[(long long)blockIdx.y * Ppad + p] = tot;
+    }
+}
+
+__global__ void finalize_merge_kernel(const double *__restrict__ fin2, int Ppad, int P, long long N, int err,
+                                      float *__restrict__ out, const DevState *state)
+{
+    if (state && state->stopped) return;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    double tot = 0.0;
+    for (int y = 0; y < FIN_SPLIT; ++y) tot += fin2[(long long)y * Ppad + p];
+    double f = tot / (double)N;
+    if (err == GAME_ERR_RMSE) f = sqrt(f);
+    out[p] = (float)f;
+}
+
 // ---- small problems (configs 1-2): latency, not throughput, decides ------------------------------------
 // The 128x128 tile above needs ~20 us per CTA whatever P is; when the whole grid is under two waves a
 // finer decomposition finishes sooner.  One CTA = one 128-pattern slab x 32 chromosomes, one THREAD = one
@@ -330,6 +367,14 @@ size_t fitness_partial_floats(const game_ctx *ctx, int P)
 int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, const DevState *state)
 {
     dim3 block(32, 32);
+    if (n_chunks >= 1024 && (P + 31) / 32 < 2 * ctx->sm_count) {
+        dim3 grid((P + 31) / 32, FIN_SPLIT);
+        finalize_split_kernel<<<grid, block, 0, ctx->stream>>>(ctx->partial, n_chunks, Ppad, P, ctx->fin2, state);
+        GAME_LAUNCHED(ctx);
+        finalize_merge_kernel<<<(P + 255) / 256, 256, 0, ctx->stream>>>(ctx->fin2, Ppad, P, ctx->N, ctx->err, out, state);
+        GAME_LAUNCHED(ctx);
+        return GAME_OK;
+    }
     finalize_kernel<<<(P + 31) / 32, block, 0, ctx->stream>>>(ctx->partial, n_chunks, Ppad, P, ctx->N, ctx->err, out,
                                                                state);
     GAME_LAUNCHED(ctx);

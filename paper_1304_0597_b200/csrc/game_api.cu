@@ -67,6 +67,12 @@ static int ensure_scratch(game_ctx *c, int P)
         GAME_CUDA(c, cudaMalloc(&c->partial, need * sizeof(float)));
         c->partial_cap = need;
     }
+    size_t need2 = (size_t)FIN_SPLIT * ((P + 255) / 256) * 256;
+    if (need2 > c->fin2_cap) {
+        dfree(c->fin2);
+        GAME_CUDA(c, cudaMalloc(&c->fin2, need2 * sizeof(double)));
+        c->fin2_cap = need2;
+    }
     size_t need16 = (size_t)((P + 255) / 256) * 256 * (size_t)c->Kpad;
     if (c->tensor_ok && need16 > c->c16_cap) {
         dfree(c->C16);
@@ -205,7 +211,7 @@ void game_destroy(game_ctx *c)
     cudaStreamSynchronize(c->stream);
     free_dataset(c);
     free_population(c);
-    dfree(c->partial); dfree(c->C16); dfree(c->stage_pop); dfree(c->stage_fit); dfree(c->state);
+    dfree(c->partial); dfree(c->fin2); dfree(c->C16); dfree(c->stage_pop); dfree(c->stage_fit); dfree(c->state);
     free(c->tmap_E); free(c->tmap_C);
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     delete c;

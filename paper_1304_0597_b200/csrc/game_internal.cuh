@@ -12,6 +12,7 @@
 namespace game {
 
 constexpr int SLAB = 128;        // patterns per n-slab: unit of the per-chromosome partial sums
+constexpr int FIN_SPLIT = 64;     // CTAs along the slab axis in the two-pass final reduction
 constexpr int TC_KBLK = 64;      // fp16 elements per 128-byte swizzled smem row (tensor path k-block)
 
 // Device-resident loop state, so a generation needs no host round trip.
@@ -78,6 +79,8 @@ struct game_ctx {
     // scratch
     float *partial = nullptr;  // n_chunks x Ppad per-chunk error sums
     size_t partial_cap = 0;
+    double *fin2 = nullptr;    // FIN_SPLIT x Ppad partial totals of the two-pass final reduction
+    size_t fin2_cap = 0;
     __half *C16 = nullptr;     // Ppad128 x Kpad fp16 population copy (TENSOR path)
     size_t c16_cap = 0;
     float *stage_pop = nullptr, *stage_fit = nullptr;   // device staging for *_host calls
