@@ -40,27 +40,32 @@ __global__ void expand_kernel(const float *__restrict__ X, long long N, int F, i
         double x = (double)X[n * F + i];
         int B = family == GAME_TRIG ? 2 * d + 1 : d + 1;
         int k0 = i * B;
-        auto put = [&](int k, double v) {
+        auto put = [&](int m, double v) {      // m: index inside feature i's block, ABI order
             float f = (float)v;
             local_max = fmaxf(local_max, fabsf(f));
-            // TENSOR path: tile-blocked [n/256][k/64][256][64] so that every TMA box is one contiguous 32 KB run
-            if (PATTERN_MAJOR) E[(((n >> 8) * (ld >> 6) + (k >> 6)) << 14) + ((n & 255) << 6) + (k & 63)] = (OutT)f;
-            else E[(long long)k * ld + n] = (OutT)f;
+            if (PATTERN_MAJOR) {
+                // TENSOR path: permuted term order (tc_position), tile-blocked [n/256][k/64][256][64] so that every
+                // TMA box is one contiguous 32 KB run
+                const long long k = tc_position(family, d, i, m);
+                E[(((n >> 8) * (ld >> 6) + (k >> 6)) << 14) + ((n & 255) << 6) + (k & 63)] = (OutT)f;
+            } else {
+                E[(long long)(k0 + m) * ld + n] = (OutT)f;
+            }
         };
-        put(k0, 1.0);
+        put(0, 1.0);
         if (family == GAME_TRIG) {
             for (int m = 1; m <= d; ++m) {
                 double s, c;
                 sincos((double)m * x, &s, &c);
-                put(k0 + m, c);
-                put(k0 + d + m, s);
+                put(m, c);
+                put(d + m, s);
             }
         } else {
             double tm1 = 1.0, t0 = x;
-            if (d >= 1) put(k0 + 1, x);
+            if (d >= 1) put(1, x);
             for (int m = 2; m <= d; ++m) {
                 double t1 = 2.0 * x * t0 - tm1;
-                put(k0 + m, t1);
+                put(m, t1);
                 tm1 = t0;
                 t0 = t1;
             }

@@ -384,15 +384,20 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
 }
 
 // pop fp32 [P][K] -> C16 fp16 [Ppad][Kpad] (round to nearest even, clamped to the finite fp16 range)
-__global__ void pop_to_f16_kernel(const float *__restrict__ pop, int P, int K, int Kpad, __half *__restrict__ C16,
-                                  const DevState *state)
+__global__ void pop_to_f16_kernel(const float *__restrict__ pop, int P, int K, int Kpad, int family, int d,
+                                  __half *__restrict__ C16, const DevState *state)
 {
     if (state && state->stopped) return;
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= (long long)P * K) return;
     int p = (int)(i / K), k = (int)(i % K);
     float v = fminf(fmaxf(pop[i], -65504.f), 65504.f);
-    C16[(long long)p * Kpad + k] = __float2half_rn(v);
+    int pos = k;
+    if (tc_permuted(family)) {              // ABI order k = i*B + m  ->  the tensor path's term order
+        const int B = tc_terms_per_feature(family, d);
+        pos = tc_position(family, d, k / B, k % B);
+    }
+    C16[(long long)p * Kpad + pos] = __float2half_rn(v);
 }
 
 // ---- host side ------------------------------------------------------------------------------------------
@@ -504,7 +509,8 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     const int n_tiles = (int)(ctx->Npad256 / BN);
     const int m_blocks = Ppad / (BM * cg);
     long long n = (long long)P * ctx->K;
-    pop_to_f16_kernel<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(pop, P, ctx->K, ctx->Kpad, ctx->C16, state);
+    pop_to_f16_kernel<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(pop, P, ctx->K, ctx->Kpad, ctx->family, ctx->degree,
+                                                                            ctx->C16, state);
     GAME_LAUNCHED(ctx);
     int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_C, ctx->C16, Ppad, ctx->Kpad, BM);
     if (rc) return rc;

@@ -189,7 +189,7 @@ int game_create(int family, int degree, int F, game_ctx **out)
     c->family = family; c->degree = degree; c->F = F;
     c->K = family == GAME_TRIG ? F * (2 * degree + 1) : family == GAME_CHEB ? F * (degree + 1)
          : family == GAME_TRIG_TIED ? 2 * degree + 1 : degree + 1;
-    c->Kpad = ((c->K + TC_KBLK - 1) / TC_KBLK) * TC_KBLK;
+    c->Kpad = ((tc_num_positions(family, degree, F, c->K) + TC_KBLK - 1) / TC_KBLK) * TC_KBLK;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);

@@ -39,6 +39,29 @@ __device__ __forceinline__ unsigned int sort_key(float f)
     return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
 
+// ---- term order of the TENSOR path's operands ---------------------------------------------------------------
+// A contraction does not care in which order its terms are stored as long as both operands agree, so E16 and C16
+// use an order that an in-kernel generator can stream: features in groups of 8, and inside a group one 8-wide
+// chunk (16 bytes of fp16 = one swizzle chunk) per term type, the 8 lanes of the chunk being the group's features:
+//     position = ((i / 8) * T + tau) * 8 + (i % 8),      T = terms per feature (2d+1 or d+1)
+// tau: Chebyshev T_0..T_d in order; trigonometric 1, cos x, sin x, cos 2x, sin 2x, ... so that (cos, sin) of one
+// multiple sit in adjacent chunks and one packed recurrence step yields both.  Features are padded to a multiple
+// of 8 (zero genes).  The tied families keep their natural order.  The ABI's order (L105) is untouched: only the
+// fp16 copies are permuted, by pop_to_f16_kernel and the expansion kernels.
+__host__ __device__ inline bool tc_permuted(int family) { return family == GAME_TRIG || family == GAME_CHEB; }
+__host__ __device__ inline int tc_terms_per_feature(int family, int d) { return family == GAME_TRIG ? 2 * d + 1 : d + 1; }
+__host__ __device__ inline int tc_num_positions(int family, int d, int F, int K)
+{
+    return tc_permuted(family) ? ((F + 7) / 8) * 8 * tc_terms_per_feature(family, d) : K;
+}
+// m = index inside the feature's block in the ABI's order [a_0, a_1..a_d, b_1..b_d]
+__host__ __device__ inline int tc_position(int family, int d, int i, int m)
+{
+    const int T = tc_terms_per_feature(family, d);
+    const int tau = family == GAME_TRIG ? (m == 0 ? 0 : (m <= d ? 2 * m - 1 : 2 * (m - d))) : m;
+    return ((i >> 3) * T + tau) * 8 + (i & 7);
+}
+
 struct FitnessCfg {
     int act, err;
     float R;
