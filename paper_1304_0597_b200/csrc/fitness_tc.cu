@@ -29,15 +29,15 @@ constexpr int BN = 256;            // patterns per tile    = TMEM columns of one
 constexpr int BKB = TC_KBLK;       // 64 fp16 = one 128-byte swizzle row per k-block
 constexpr int UMMA_K = 16;
 constexpr int A_BYTES = BM * BKB * 2;
-constexpr int N_EPI_WARPS = 8;
-constexpr int TC_THREADS = 64 + 32 * N_EPI_WARPS;
+constexpr int WARP_TMA = 0, WARP_MMA = 1, WARP_EPI0 = 2;      // warp roles; the epilogue warps follow (EW = 8 or 16 of them)
 
 template <int CG> struct Cfg {
     static constexpr int BNL = BN / CG;                 // pattern rows this CTA stages
     static constexpr int B_BYTES = BNL * BKB * 2;
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
     static constexpr int STAGES = CG == 1 ? 4 : 6;
-    static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/ + 2 * BN * 4 /*targets*/;
+    static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/ + 3 * BN * 4 /*targets*/
+                              + 2 * 4 * BM * 4 /*per-column-block error sums of two tiles*/;
 };
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------
@@ -69,6 +69,14 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
                      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
         if (spin > (1u << 22)) __trap();      // a protocol bug must fail loudly, not hang the device
     }
+}
+// non-blocking: has the phase with this parity completed?
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
@@ -153,6 +161,11 @@ __host__ __device__ constexpr uint32_t make_idesc(int M, int N)
 
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
 {
+#ifdef GAME_PROBE_SKIP_LDTM      // measurement probe only (never defined in the product build): no TMEM read
+#pragma unroll
+    for (int i = 0; i < 32; ++i) v[i] = (taddr + i) & 0x3fffffffu;
+    return;
+#endif
     asm volatile(
         "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
         "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
@@ -163,7 +176,19 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
           "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
         : "r"(taddr) : "memory");
 }
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// Wait for this warp's outstanding TMEM loads.  The loaded registers pass through the statement as in/out operands, so
+// the compiler can neither read them before the wait nor start on them early: consumers stay BELOW this point and the
+// evaluation of the previous chunk stays ABOVE the next tmem_ld32 into the same registers.  Without that tie ptxas
+// interleaves the two chunks and the warp blocks on the load it was meant to overlap (measured: config 3, K = 112).
+__device__ __forceinline__ void tmem_ld_wait(uint32_t (&v)[32])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(v[0]), "+r"(v[1]), "+r"(v[2]), "+r"(v[3]), "+r"(v[4]), "+r"(v[5]), "+r"(v[6]), "+r"(v[7]),
+                   "+r"(v[8]), "+r"(v[9]), "+r"(v[10]), "+r"(v[11]), "+r"(v[12]), "+r"(v[13]), "+r"(v[14]), "+r"(v[15]),
+                   "+r"(v[16]), "+r"(v[17]), "+r"(v[18]), "+r"(v[19]), "+r"(v[20]), "+r"(v[21]), "+r"(v[22]), "+r"(v[23]),
+                   "+r"(v[24]), "+r"(v[25]), "+r"(v[26]), "+r"(v[27]), "+r"(v[28]), "+r"(v[29]), "+r"(v[30]), "+r"(v[31])
+                 :: "memory");
+}
 
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
@@ -176,7 +201,8 @@ __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.
 //     indistinguishable from mode 0's (both dominated by the fp16 operand rounding, max 5e-4 relative, no
 //     bias), and the MUFU-bound config 3 runs 1.4x faster, so it is the default.  A packed
 //     tanh.approx.f16x2 form (0.5 MUFU per evaluation) was measured too: biased by -2e-4 and slower; dropped.
-// In mode 2 the staged targets are t - 0.5, so r = (t - 0.5) - 0.5 tanh(z/2) is one FFMA.
+// In mode 2 the staged targets are t - 0.5 and the fp16 genes are pre-halved (a power-of-two scale: the same
+// rounding), so the accumulator is z/2 and r = (t - 0.5) - 0.5 tanh(z/2) is one MUFU + one FFMA.
 // Arithmetic is issued two evaluations at a time with the packed fp32 instructions of sm_100
 // (FMUL2 / FFMA2), which halves the FMA-pipe issue slots the epilogue needs.
 constexpr int MODE_SIG_EXACT = 0, MODE_IDENTITY = 1, MODE_SIG_TANH32 = 2;
@@ -193,49 +219,41 @@ template <int ACT> __device__ __forceinline__ float2 residual2(float2 z, float2 
     } else if (ACT == MODE_IDENTITY) {
         return __ffma2_rn(z, make_float2(-1.0f, -1.0f), t);
     } else {
-        float2 h = __fmul2_rn(z, make_float2(0.5f, 0.5f));
-        return __ffma2_rn(make_float2(tanh_approx(h.x), tanh_approx(h.y)), make_float2(-0.5f, -0.5f), t);
+        // the accumulator already holds z/2: pop_to_f16_kernel halves the genes (exact in fp16) in this mode
+        return __ffma2_rn(make_float2(tanh_approx(z.x), tanh_approx(z.y)), make_float2(-0.5f, -0.5f), t);
     }
 }
 
-// acc += e(r) for two evaluations; TMSE zeroes residuals inside the tube first (|r| <= R -> 0)
+// acc += e(r) for two evaluations; TMSE zeroes residuals inside the tube first (|r| <= R -> 0).  The tube test is
+// one FSET per evaluation (a 1.0 / 0.0 mask) folded in by a packed multiply, instead of a compare + select pair.
 template <bool TMSE> __device__ __forceinline__ void accumulate2(float2 r, float R, float2 &acc)
 {
     if (TMSE) {
-        r.x = fabsf(r.x) > R ? r.x : 0.f;
-        r.y = fabsf(r.y) > R ? r.y : 0.f;
+        const float2 m = make_float2(fabsf(r.x) > R ? 1.0f : 0.0f, fabsf(r.y) > R ? 1.0f : 0.0f);
+        acc = __ffma2_rn(__fmul2_rn(r, m), r, acc);
+    } else {
+        acc = __ffma2_rn(r, r, acc);
     }
-    acc = __ffma2_rn(r, r, acc);
 }
 
-// 32 consecutive accumulator columns of this thread's chromosome against 32 staged targets
+// 32 consecutive accumulator columns of this thread's chromosome against 32 staged targets; four independent
+// running sums so the additions do not form one dependent chain
 template <int ACT, bool TMSE>
-__device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const float *ts, float R, float2 &acc)
+__device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const float *ts, float R, float2 (&acc)[4])
 {
 #pragma unroll
     for (int j = 0; j < 32; j += 4) {
         const float4 t4 = *reinterpret_cast<const float4 *>(ts + j);
-        accumulate2<TMSE>(residual2<ACT>(make_float2(__uint_as_float(v[j]), __uint_as_float(v[j + 1])), make_float2(t4.x, t4.y)), R, acc);
-        accumulate2<TMSE>(residual2<ACT>(make_float2(__uint_as_float(v[j + 2]), __uint_as_float(v[j + 3])), make_float2(t4.z, t4.w)), R, acc);
-    }
-}
-
-// ragged tail: only the first `valid` of the 32 columns count
-template <int ACT, bool TMSE>
-__device__ __forceinline__ void epilogue_chunk_masked(const uint32_t (&v)[32], const float *ts, float R, int valid, float2 &acc)
-{
-#pragma unroll
-    for (int j = 0; j < 32; j += 2) {
-        float2 r = residual2<ACT>(make_float2(__uint_as_float(v[j]), __uint_as_float(v[j + 1])), make_float2(ts[j], ts[j + 1]));
-        r.x = j < valid ? r.x : 0.f;
-        r.y = j + 1 < valid ? r.y : 0.f;
-        accumulate2<TMSE>(r, R, acc);
+        accumulate2<TMSE>(residual2<ACT>(make_float2(__uint_as_float(v[j]), __uint_as_float(v[j + 1])), make_float2(t4.x, t4.y)), R,
+                          acc[(j >> 1) & 3]);
+        accumulate2<TMSE>(residual2<ACT>(make_float2(__uint_as_float(v[j + 2]), __uint_as_float(v[j + 3])), make_float2(t4.z, t4.w)), R,
+                          acc[((j >> 1) + 1) & 3]);
     }
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------
-template <int CG, int ACT, bool TMSE>
-__global__ void __launch_bounds__(TC_THREADS, 1)
+template <int CG, int ACT, bool TMSE, int EW>
+__global__ void __launch_bounds__(64 + 32 * EW, 1)
 fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmE,
                   int n_tiles, int m_blocks, int k_blocks, long long N, const float *__restrict__ tgt, float R,
                   float *__restrict__ partial, int Ppad, const DevState *state)
@@ -253,7 +271,8 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     auto tempty_bar = [&](int a) { return bar0 + 8u * (2 * C::STAGES + 2 + a); };
     const uint32_t tmem_slot = bar0 + 8u * (2 * C::STAGES + 4);
     volatile uint32_t *tmem_slot_g = reinterpret_cast<volatile uint32_t *>(gbase + C::STAGES * C::STAGE_BYTES + 8 * (2 * C::STAGES + 4));
-    float *tgt_s = reinterpret_cast<float *>(gbase + C::STAGES * C::STAGE_BYTES + 256);   // [2][BN]
+    float *tgt_s = reinterpret_cast<float *>(gbase + C::STAGES * C::STAGE_BYTES + 256);   // [3][BN]
+    float *sum_s = tgt_s + 3 * BN;                                                        // [2][4][BM]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint32_t cta_rank = 0;
@@ -263,19 +282,19 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < C::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-        for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), CG * N_EPI_WARPS); }
+        for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), CG * EW); }
         fence_barrier_init();
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmC) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmE) : "memory");
     }
-    if (warp == 1) tmem_alloc<CG>(tmem_slot, 512);
+    if (warp == WARP_MMA) tmem_alloc<CG>(tmem_slot, 512);
     tc_fence_before();
     if (CG == 2) { asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory"); }
     else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_g;
 
-    if (warp == 0) {
+    if (warp == WARP_TMA) {
         // ===== TMA producer =====
         if (lane == 0) {
             int s = 0; uint32_t ph = 0;
@@ -293,7 +312,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                 }
             }
         }
-    } else if (warp == 1) {
+    } else if (warp == WARP_MMA) {
         // ===== MMA issuer (one thread; leader CTA only when paired) =====
         if (lane == 0 && cta_rank == 0) {
             constexpr uint32_t idesc = make_idesc(BM * CG, BN);
@@ -322,57 +341,100 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
         }
     } else {
         // ===== epilogue warps =====
-        const int ew = warp - 2;
-        const int quarter = warp & 3;          // TMEM lane quarter this warp may touch
-        const int half = ew >> 2;              // which 128 columns of the 256-column tile
-        const int et = threadIdx.x - 64;
-        int acc = 0; uint32_t aph = 0;
+        // EW warps: warp w may touch TMEM lanes 32*(w%4).., so four warps cover the 128 chromosomes and EW/4 such
+        // groups split the tile's 256 pattern columns.  16 warps (4 per scheduler) keep the MUFU pipe fed where the
+        // epilogue is the bound (shallow K); 8 leave more registers per thread.
+        constexpr int NCB = EW / 4;                 // column blocks per tile
+        constexpr int CBW = BN / NCB;               // columns per block: 128 or 64
+        constexpr int NCH = CBW / 32;               // 32-column chunks per tile and warp: 4 or 2 (even)
+        const int ew = warp - WARP_EPI0;
+        const int quarter = warp & 3;               // TMEM lane quarter this warp may touch
+        const int cb = ew >> 2;                     // which column block of the 256-column tile
+        const int et = threadIdx.x - 32 * WARP_EPI0;
+        // One continuous stream of 32-column chunks: the TMEM load of the next chunk -- the next TILE's first chunk
+        // included -- is in flight while the current one is evaluated.  Targets are staged one tile ahead in a ring
+        // of three buffers: the buffer written during tile i was last read in tile i-2, and the one barrier per tile
+        // separates the two.  Patterns beyond N carry the target that makes their residual exactly zero (their
+        // expansion rows are zero, so z = 0): no masked code path.  The column blocks' sums of a tile meet in shared
+        // memory and are added in fixed order by block 0's warps one tile later: one partial row per 256 patterns.
+        constexpr float tbias = ACT == MODE_SIG_TANH32 ? 0.5f : 0.f;           // staged target = t - tbias
+        constexpr float tneutral = ACT == MODE_SIG_EXACT ? 0.5f : 0.f;         // staged target of a padding pattern
+        // raw target of this thread's pattern in `tile` (tneutral + tbias for a padding pattern); the bias comes
+        // off when the value is staged one tile later, so nothing waits on the load where it is issued
+        auto fetch_target = [&](int tile) -> float {
+            const long long n = (long long)(tile / m_blocks) * BN + et;
+            return (et < BN && n < N) ? tgt[n] : tneutral + tbias;
+        };
+        auto epi_barrier = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(32 * EW) : "memory"); };
+        const int row = quarter * 32 + lane;        // chromosome row inside the 128-row block
+        long long prev_off = -1;                    // where the previous tile's sum goes in `partial`
+        auto flush = [&](int buf) {                 // block 0's warps: add the tile's column-block sums, ascending
+            if (cb == 0 && prev_off >= 0) {
+                const float *ss = sum_s + buf * 4 * BM + row;
+                float s = ss[0];
+#pragma unroll
+                for (int j = 1; j < NCB; ++j) s += ss[j * BM];
+                partial[prev_off] = s;
+            }
+        };
+        const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(cb * CBW);
+        int acc = 0; uint32_t aph = 0; int tb = 0, sb = 0;
+        uint32_t va[32], vb[32];
+        float t_next = 0.f;
+        if (pair < total_tiles) {
+            if (et < BN) tgt_s[et] = fetch_target(pair) - tbias;
+            if (pair + n_pairs < total_tiles) t_next = fetch_target(pair + n_pairs);
+            epi_barrier();
+            mbar_wait(tfull_bar(0), 0);
+            tc_fence_after();
+            tmem_ld32(lane_addr, va);
+        }
         for (int tile = pair; tile < total_tiles; tile += n_pairs) {
             const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
-            const long long n0 = (long long)n_tile * BN;
-            tgt_s[acc * BN + et] = tgt[n0 + et] - (ACT == MODE_SIG_TANH32 ? 0.5f : 0.f);
-            asm volatile("bar.sync 1, %0;" ::"n"(32 * N_EPI_WARPS) : "memory");
-            long long rem = N - (n0 + half * 128);
-            const int valid = rem >= 128 ? 128 : (rem > 0 ? (int)rem : 0);
-            mbar_wait(tfull_bar(acc), aph);
-            tc_fence_after();
-            const uint32_t t0 = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(acc * BN + half * 128);
-            const float *ts = tgt_s + acc * BN + half * 128;
-            float2 acc2 = make_float2(0.f, 0.f);
-            if (valid == 128) {
-                // software pipeline: the TMEM load of chunk c+1 is in flight while chunk c is evaluated
-                uint32_t va[32], vb[32];
-                tmem_ld32(t0, va);
-                tmem_ld_wait();
-                tmem_ld32(t0 + 32, vb);
-                epilogue_chunk<ACT, TMSE>(va, ts, R, acc2);
-                tmem_ld_wait();
-                tmem_ld32(t0 + 64, va);
-                epilogue_chunk<ACT, TMSE>(vb, ts + 32, R, acc2);
-                tmem_ld_wait();
-                tmem_ld32(t0 + 96, vb);
-                epilogue_chunk<ACT, TMSE>(va, ts + 64, R, acc2);
-                tmem_ld_wait();
-                epilogue_chunk<ACT, TMSE>(vb, ts + 96, R, acc2);
-            } else {
-#pragma unroll 1
-                for (int c = 0; c * 32 < valid; ++c) {
-                    uint32_t v[32];
-                    tmem_ld32(t0 + c * 32, v);
-                    tmem_ld_wait();
-                    epilogue_chunk_masked<ACT, TMSE>(v, ts + c * 32, R, valid - c * 32, acc2);
+            const bool has_next = tile + n_pairs < total_tiles;
+            const uint32_t t0 = lane_addr + (uint32_t)(acc * BN);
+            const float *ts = tgt_s + tb * BN + cb * CBW;
+            const int tbn = tb == 2 ? 0 : tb + 1;
+            float2 acc2[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) {
+                uint32_t (&cur)[32] = (c & 1) ? vb : va;
+                uint32_t (&nxt)[32] = (c & 1) ? va : vb;
+                tmem_ld_wait(cur);
+                if (c + 1 < NCH) {
+                    tmem_ld32(t0 + 32 * (c + 1), nxt);
+                } else {
+                    // every TMEM read of this tile's accumulator has completed: hand it back to the MMA warp
+                    // BEFORE waiting for the next one
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) {
+                        if (CG == 1) mbar_arrive(tempty_bar(acc));
+                        else mbar_arrive_cluster(tempty_bar(acc), 0);
+                    }
+                    if (has_next && et < BN) tgt_s[tbn * BN + et] = t_next - tbias;
+                    if (tile + 2 * n_pairs < total_tiles) t_next = fetch_target(tile + 2 * n_pairs);
+                    epi_barrier();
+                    flush(sb ^ 1);
+                    if (has_next) {                   // uniform over the CTA's epilogue warps
+                        mbar_wait(tfull_bar(acc ^ 1), acc ? aph ^ 1 : aph);
+                        tc_fence_after();
+                        tmem_ld32(lane_addr + (uint32_t)((acc ^ 1) * BN), nxt);
+                    }
                 }
+#ifndef GAME_PROBE_NO_EPI
+                epilogue_chunk<ACT, TMSE>(cur, ts + 32 * c, R, acc2);
+#endif
             }
-            const float sum = acc2.x + acc2.y;
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) {
-                if (CG == 1) mbar_arrive(tempty_bar(acc));
-                else mbar_arrive_cluster(tempty_bar(acc), 0);
-            }
-            const int p = (m_blk * CG + (int)cta_rank) * BM + quarter * 32 + lane;
-            partial[(long long)(n_tile * 2 + half) * Ppad + p] = sum;
+            sum_s[(sb * 4 + cb) * BM + row] = ((acc2[0].x + acc2[0].y) + (acc2[1].x + acc2[1].y)) + ((acc2[2].x + acc2[2].y) + (acc2[3].x + acc2[3].y));
+            prev_off = (long long)n_tile * Ppad + (m_blk * CG + (int)cta_rank) * BM + row;
+            tb = tbn;
+            sb ^= 1;
             if (++acc == 2) { acc = 0; aph ^= 1; }
+        }
+        if (pair < total_tiles) {
+            epi_barrier();
+            flush(sb ^ 1);
         }
     }
 
@@ -380,18 +442,19 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     tc_fence_before();
     if (CG == 2) { asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory"); }
     else __syncthreads();
-    if (warp == 1) { __syncwarp(); tc_fence_after(); tmem_dealloc<CG>(tmem_base, 512); }
+    if (warp == WARP_MMA) { __syncwarp(); tc_fence_after(); tmem_dealloc<CG>(tmem_base, 512); }
 }
 
-// pop fp32 [P][K] -> C16 fp16 [Ppad][Kpad] (round to nearest even, clamped to the finite fp16 range)
-__global__ void pop_to_f16_kernel(const float *__restrict__ pop, int P, int K, int Kpad, int family, int d,
+// pop fp32 [P][K] -> C16 fp16 [Ppad][Kpad] (round to nearest even, clamped to the finite fp16 range), times `scale`
+// (1 or 0.5: exact, see the epilogue modes)
+__global__ void pop_to_f16_kernel(const float *__restrict__ pop, int P, int K, int Kpad, int family, int d, float scale,
                                   __half *__restrict__ C16, const DevState *state)
 {
     if (state && state->stopped) return;
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= (long long)P * K) return;
     int p = (int)(i / K), k = (int)(i % K);
-    float v = fminf(fmaxf(pop[i], -65504.f), 65504.f);
+    float v = fminf(fmaxf(pop[i], -65504.f), 65504.f) * scale;
     int pos = k;
     if (tc_permuted(family)) {              // ABI order k = i*B + m  ->  the tensor path's term order
         const int B = tc_terms_per_feature(family, d);
@@ -450,6 +513,20 @@ static int cta_group(const game_ctx *ctx, int Ppad)
     return (ctx->Kpad >= 512 && Ppad >= 1024) ? 2 : 1;
 }
 
+// Epilogue warps per CTA: 8.  16 (four per scheduler, 96 registers each) were measured on B200 and lose everywhere
+// (config 3: 0.177 vs 0.154 ms; config 5: 2.32 vs 2.23 ms); GAME_TC_EPI_WARPS=16 keeps that variant measurable.
+static int epilogue_warps(const game_ctx *ctx)
+{
+    static int forced = -1;
+    if (forced < 0) {
+        const char *e = getenv("GAME_TC_EPI_WARPS");
+        forced = e ? (atoi(e) == 16 ? 16 : 8) : 0;
+    }
+    if (forced) return forced;
+    (void)ctx;
+    return 8;
+}
+
 // Which logistic form the epilogue uses: mode 2 unless GAME_TC_SIGMOID=0 (measurement knob).
 static int sigmoid_mode()
 {
@@ -474,11 +551,11 @@ int tensor_prepare(game_ctx *ctx)
     return GAME_OK;
 }
 
-template <int CG, int ACT, bool TMSE>
+template <int CG, int ACT, bool TMSE, int EW>
 static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, const DevState *state)
 {
     using C = Cfg<CG>;
-    auto kern = fitness_tc_kernel<CG, ACT, TMSE>;
+    auto kern = fitness_tc_kernel<CG, ACT, TMSE, EW>;
     static bool attr_set = false;
     if (!attr_set) {
         GAME_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
@@ -489,7 +566,7 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     if (pairs > total) pairs = (int)total;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)(pairs * CG));
-    cfg.blockDim = dim3(TC_THREADS);
+    cfg.blockDim = dim3(64 + 32 * EW);
     cfg.dynamicSmemBytes = C::SMEM;
     cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
@@ -509,16 +586,19 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     const int n_tiles = (int)(ctx->Npad256 / BN);
     const int m_blocks = Ppad / (BM * cg);
     long long n = (long long)P * ctx->K;
+    const bool tmse = ctx->err == GAME_ERR_TMSE;
+    const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : sigmoid_mode();
+    const int ew = epilogue_warps(ctx);
     pop_to_f16_kernel<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(pop, P, ctx->K, ctx->Kpad, ctx->family, ctx->degree,
-                                                                            ctx->C16, state);
+                                                                            mode == MODE_SIG_TANH32 ? 0.5f : 1.0f, ctx->C16, state);
     GAME_LAUNCHED(ctx);
     int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_C, ctx->C16, Ppad, ctx->Kpad, BM);
     if (rc) return rc;
-    const bool tmse = ctx->err == GAME_ERR_TMSE;
-    const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : sigmoid_mode();
+#define GAME_TC_EW(CGV, M, T)                                                                    \
+    rc = ew == 16 ? launch_variant<CGV, M, T, 16>(ctx, n_tiles, m_blocks, Ppad, state)           \
+                  : launch_variant<CGV, M, T, 8>(ctx, n_tiles, m_blocks, Ppad, state)
 #define GAME_TC_MODE(CGV, M)                                                                     \
-    rc = tmse ? launch_variant<CGV, M, true>(ctx, n_tiles, m_blocks, Ppad, state)                \
-              : launch_variant<CGV, M, false>(ctx, n_tiles, m_blocks, Ppad, state)
+    if (tmse) { GAME_TC_EW(CGV, M, true); } else { GAME_TC_EW(CGV, M, false); }
 #define GAME_TC_DISPATCH(CGV)                                                                    \
     switch (mode) {                                                                              \
     case MODE_IDENTITY: GAME_TC_MODE(CGV, MODE_IDENTITY); break;                                 \
@@ -528,10 +608,11 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     if (cg == 2) { GAME_TC_DISPATCH(2); } else { GAME_TC_DISPATCH(1); }
 #undef GAME_TC_DISPATCH
 #undef GAME_TC_MODE
+#undef GAME_TC_EW
     if (rc) return rc;
     ++ctx->launches;
-    if (defer) { defer->n_chunks = (int)(ctx->Npad256 / SLAB); defer->Ppad = Ppad; return GAME_OK; }
-    return launch_finalize(ctx, (int)(ctx->Npad256 / SLAB), Ppad, P, out, state);
+    if (defer) { defer->n_chunks = n_tiles; defer->Ppad = Ppad; return GAME_OK; }     // one partial row per 256-pattern tile
+    return launch_finalize(ctx, n_tiles, Ppad, P, out, state);
 }
 
 }  // namespace game
