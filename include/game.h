@@ -45,6 +45,7 @@ enum { GAME_ELITE_COPIES_OF_BEST = 0, GAME_ELITE_TOP_E = 1 };      /* L148; DESI
 /* Fitness kernel choice.  FP32: FFMA contraction, |rel err| <= 1e-5 class.  TENSOR: tcgen05 fp16-input /
  * fp32-accumulate MMA (same 11-bit significand as TF32), 1e-3 class.  AUTO picks by problem shape. */
 enum { GAME_PATH_AUTO = 0, GAME_PATH_FP32 = 1, GAME_PATH_TENSOR = 2 };
+enum { GAME_EXPAND_AUTO = 0, GAME_EXPAND_MATERIALIZED = 1, GAME_EXPAND_REGENERATED = 2 };
 
 /* GA parameters (L275-L291).  Probabilities are per parent pair (crossover, DESIGN G15) and per gene
  * (mutation, DESIGN G16).  stop_error < 0 disables the error-threshold stop (L219, L287). */
@@ -85,6 +86,18 @@ int game_set_error(game_ctx *ctx, int err_type, float tmse_R);   /* default MSE;
 int game_set_path(game_ctx *ctx, int path);                      /* default GAME_PATH_AUTO */
 /* Which path the next fitness call will take for population size P: GAME_PATH_FP32 or GAME_PATH_TENSOR. */
 int game_resolved_path(const game_ctx *ctx, int P);
+/* a1, TENSOR path only: where the fused fitness kernel takes the expansion from (north_star (1)).
+ *   GAME_EXPAND_MATERIALIZED  streams the fp16 expansion matrix built once by game_load (L254's hoisting);
+ *   GAME_EXPAND_REGENERATED   recomputes each 256-pattern tile of it from X inside the kernel, straight into shared
+ *                             memory, with the population's fp16 copy resident there.  Available for the per-feature
+ *                             families when P <= 256 and K (padded to 64 per 8 features) <= 576, and for the
+ *                             trigonometric family only when max|X| <= pi; otherwise the fitness call fails with
+ *                             GAME_ERR_UNSUPPORTED;
+ *   GAME_EXPAND_AUTO          (default) the faster of the two as measured on B200.
+ * game_resolved_expansion: which of the two a TENSOR-path fitness call on P chromosomes will use, or -1 if the
+ * requested one is unavailable. */
+int game_set_expansion(game_ctx *ctx, int mode);
+int game_resolved_expansion(const game_ctx *ctx, int P);
 
 /* a0 + a1: load the dataset and expand it (L254: "calculate the time consuming trigonometric functions
  * only once").  X is N x F row-major fp32, targets N fp32.  Builds the device-resident expansion

@@ -20,12 +20,14 @@ GAME_SEL_TOURNAMENT, GAME_SEL_ROULETTE = 0, 1
 GAME_INIT_UNIFORM_PM1, GAME_INIT_NORMAL_PM1, GAME_INIT_UNIFORM_01 = 0, 1, 2
 GAME_ELITE_COPIES_OF_BEST, GAME_ELITE_TOP_E = 0, 1
 GAME_PATH_AUTO, GAME_PATH_FP32, GAME_PATH_TENSOR = 0, 1, 2
+GAME_EXPAND_AUTO, GAME_EXPAND_MATERIALIZED, GAME_EXPAND_REGENERATED = 0, 1, 2
 ERROR_NAMES = {1: "INVALID_ARG", 2: "NOT_LOADED", 3: "ALLOC", 4: "CUDA", 5: "UNSUPPORTED", 6: "NONFINITE_INPUT"}
 
 # every symbol include/game.h declares (tests check the library exports exactly these)
 SYMBOLS = [
     "game_create", "game_destroy", "game_num_terms", "game_generation", "game_last_error",
     "game_set_stream", "game_set_activation", "game_set_error", "game_set_path", "game_resolved_path",
+    "game_set_expansion", "game_resolved_expansion",
     "game_load", "game_load_host", "game_fitness", "game_fitness_host", "game_predict", "game_classify",
     "game_set_population", "game_set_generation", "game_evolve", "game_get_population",
     "game_get_population_host", "game_rank", "game_ga_step", "game_init_population", "game_philox",
@@ -77,6 +79,8 @@ def load_library():
         L.game_set_error.argtypes = [vp, i, C.c_float]
         L.game_set_path.argtypes = [vp, i]
         L.game_resolved_path.argtypes = [vp, i]
+        L.game_set_expansion.argtypes = [vp, i]
+        L.game_resolved_expansion.argtypes = [vp, i]
         L.game_load.argtypes = [vp, vp, vp, ll]
         L.game_load_host.argtypes = [vp, vp, vp, ll]
         L.game_fitness.argtypes = [vp, vp, i, vp]
@@ -183,6 +187,12 @@ class Game:
 
     def set_path(self, path):
         self._ck(self._L.game_set_path(self._h, path))
+
+    def set_expansion(self, mode):
+        self._ck(self._L.game_set_expansion(self._h, mode))
+
+    def resolved_expansion(self, P):
+        return self._L.game_resolved_expansion(self._h, P)
 
     def resolved_path(self, P):
         return self._L.game_resolved_path(self._h, P)

@@ -5,15 +5,20 @@
 
 namespace game {
 
+// flag[0] |= 1 when X (a) or the targets (b) hold a NaN/Inf; flag[2] = max |X| as float bits (the in-kernel
+// generator's fast sincos is only offered for |x| <= pi)
 __global__ void check_finite_kernel(const float *__restrict__ a, long long na, const float *__restrict__ b,
                                     long long nb, int *flag)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     long long stride = (long long)gridDim.x * blockDim.x;
     bool bad = false;
-    for (long long j = i; j < na; j += stride) bad |= !isfinite(a[j]);
+    float mx = 0.f;
+    for (long long j = i; j < na; j += stride) { const float v = a[j]; bad |= !isfinite(v); mx = fmaxf(mx, fabsf(v)); }
     for (long long j = i; j < nb; j += stride) bad |= !isfinite(b[j]);
     if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(flag, 1);
+    for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if ((threadIdx.x & 31) == 0 && mx > 0.f && mx < INFINITY) atomicMax(flag + 2, __float_as_int(mx));   // non-negative floats order as ints
 }
 
 int launch_check_finite(game_ctx *ctx, const float *X, long long nX, const float *t, long long nT, int *flag_dev)

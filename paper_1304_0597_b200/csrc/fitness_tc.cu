@@ -30,14 +30,27 @@ constexpr int BKB = TC_KBLK;       // 64 fp16 = one 128-byte swizzle row per k-b
 constexpr int UMMA_K = 16;
 constexpr int A_BYTES = BM * BKB * 2;
 constexpr int WARP_TMA = 0, WARP_MMA = 1, WARP_EPI0 = 2;      // warp roles; the epilogue warps follow (EW = 8 or 16 of them)
+// Where the B operand (the expansion tile) comes from:
+//   SRC_TMA  streamed from the materialised E16 in HBM, together with the A (population) tile, through a TMA ring
+//   SRC_GEN  regenerated from X inside the kernel by four generator warps writing 128B-swizzled k-blocks straight
+//            into shared memory, with the whole population tile RESIDENT in shared memory (small populations:
+//            one CTA pair covers all chromosomes, so every expansion value is generated exactly once per launch)
+constexpr int SRC_TMA = 0, SRC_GEN = 1;
+constexpr int GEN_WARPS = 4;            // generator threads: GEN_SPLIT per pattern row of this CTA's 128-row B half
+constexpr int GEN_SPLIT = GEN_WARPS / 4; // threads sharing a row: each takes 8 / GEN_SPLIT of a chunk's features
+constexpr int GEN_NJ = 4 / GEN_SPLIT;   // feature PAIRS (float2) per thread and chunk
+constexpr int GEN_STAGES = 4;           // B k-block stages of the generator ring
+constexpr int GEN_B_BYTES = 128 * BKB * 2;
+constexpr int GEN_BAR0 = 2;             // named barriers 2.. : one per generator stage (0 = CTA, 1 = epilogue)
+constexpr int MAX_STAGES = 6;           // barrier slots are laid out for the deepest ring
+constexpr int TC_TAIL_BYTES = 256 /*barriers*/ + 3 * BN * 4 /*targets*/ + 2 * 4 * BM * 4 /*column-block error sums of two tiles*/;
 
 template <int CG> struct Cfg {
     static constexpr int BNL = BN / CG;                 // pattern rows this CTA stages
     static constexpr int B_BYTES = BNL * BKB * 2;
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
     static constexpr int STAGES = CG == 1 ? 4 : 6;
-    static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/ + 3 * BN * 4 /*targets*/
-                              + 2 * 4 * BM * 4 /*per-column-block error sums of two tiles*/;
+    static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 /*align*/ + TC_TAIL_BYTES;
 };
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------
@@ -55,11 +68,14 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// arrive on the barrier at the same offset in CTA `rank` of the cluster
+// arrive on the barrier at the same offset in CTA `rank` of the cluster.  Default semantics (release at CTA scope):
+// what is handed over lives in the ARRIVING CTA's own shared / tensor memory and is made visible there beforehand
+// (tcgen05.fence / fence.proxy.async + a CTA barrier); only the signal crosses to the peer.  A cluster-scope release
+// costs a GPU-wide memory barrier per arrival (measured: it alone bounded the generator variant at 47 % tensor-pipe use).
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t rank)
 {
     asm volatile("{\n\t.reg .b32 ra;\n\tmapa.shared::cluster.u32 ra, %0, %1;\n\t"
-                 "mbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n\t}" ::"r"(bar), "r"(rank) : "memory");
+                 "mbarrier.arrive.shared::cluster.b64 _, [ra];\n\t}" ::"r"(bar), "r"(rank) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
@@ -161,11 +177,6 @@ __host__ __device__ constexpr uint32_t make_idesc(int M, int N)
 
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
 {
-#ifdef GAME_PROBE_SKIP_LDTM      // measurement probe only (never defined in the product build): no TMEM read
-#pragma unroll
-    for (int i = 0; i < 32; ++i) v[i] = (taddr + i) & 0x3fffffffu;
-    return;
-#endif
     asm volatile(
         "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
         "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
@@ -251,27 +262,196 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const fl
     }
 }
 
+// ---- a1 inside the kernel: the generator warps of the SRC_GEN variant ---------------------------------------
+// Each of the 128 generator threads owns one pattern row of this CTA's half of the 256-pattern tile and writes that
+// row's expansion, 16 bytes (8 fp16 = one swizzle chunk) at a time, into the B ring exactly where a 128B-swizzled TMA
+// box would have put it: chunk j of row r of a k-block lives at r*128 + ((j ^ (r & 7)) << 4).  The term order is
+// game_internal.cuh's tc_position(): features in groups of 8, one chunk per term type, the chunk's 8 lanes being the
+// group's features -- so one chunk is one step of a recurrence carried in registers for 8 features at once:
+//   Chebyshev (G7, G9):  T_0 = 1, T_1 = x, T_{m+1} = 2x T_m - T_{m-1}
+//   trigonometric (eq. 8-9):  1, cos x, sin x, then cos / sin (m+1)x = 2 cos x . cos / sin mx - cos / sin (m-1)x
+// in fp32 (packed FFMA2), rounded once to fp16.  Rows beyond N generate zeros (their start value is 0), matching the
+// zero padding of the materialised E16.  A stage is published to the MMA warp of the leader CTA by the async-proxy
+// fence + one mbarrier arrival per warp.
+__device__ __forceinline__ uint32_t pack_half2(float lo, float hi)
+{
+    __half2 h = __floats2half2_rn(lo, hi);
+    return *reinterpret_cast<uint32_t *>(&h);
+}
+
+template <int FAMILY>
+__device__ __forceinline__ void generate_expansion(const float *__restrict__ X, int F, int d, long long N, int k_blocks,
+                                                   int pair, int n_pairs, int total_tiles, int cta_rank, int gt,
+                                                   uint8_t *bring, uint32_t bar0)
+{
+    const int hf = gt >> 7;                   // which part of every chunk this thread writes (warp-uniform)
+    gt &= 127;
+    const int T = tc_terms_per_feature(FAMILY, d);
+    const int ngroups = (F + 7) >> 3;
+    const int nchunks = k_blocks * 8;
+    uint8_t *my_row = bring + gt * 128 + hf * (16 / GEN_SPLIT);
+    const int sw = gt & 7;
+    const bool vec = (F & 3) == 0;
+    int s = 0; uint32_t ph = 0;
+    int cidx = 0;
+    mbar_wait(bar0 + 8u * MAX_STAGES, 1);     // stage 0 starts free
+
+    uint8_t *dst = my_row;                                          // this thread's row in the current stage
+    const int sw16 = sw << 4;
+    int cb16 = 0;                                                   // 16 * (chunk index inside the k-block)
+    auto put = [&](const float2 (&v)[GEN_NJ]) {                   // this thread's part of the row's next 16-byte chunk
+        if (GEN_NJ == 4) {
+            *reinterpret_cast<uint4 *>(dst + (cb16 ^ sw16)) = make_uint4(pack_half2(v[0].x, v[0].y), pack_half2(v[1].x, v[1].y),
+                                                                          pack_half2(v[GEN_NJ / 2].x, v[GEN_NJ / 2].y), pack_half2(v[GEN_NJ - 1].x, v[GEN_NJ - 1].y));
+        } else {
+            *reinterpret_cast<uint2 *>(dst + (cb16 ^ sw16)) = make_uint2(pack_half2(v[0].x, v[0].y), pack_half2(v[GEN_NJ - 1].x, v[GEN_NJ - 1].y));
+        }
+        ++cidx;
+        cb16 += 16;
+        if (cb16 == 128) {
+            cb16 = 0;
+            fence_proxy_async();              // generic-proxy stores -> visible to the tensor core's async proxy
+            __threadfence_block();
+            asm volatile("bar.arrive %0, %1;" ::"r"(GEN_BAR0 + s), "n"(32 * GEN_WARPS + 32) : "memory");
+            if (++s == GEN_STAGES) { s = 0; ph ^= 1; }
+            dst = my_row + s * GEN_B_BYTES;
+            mbar_wait(bar0 + 8u * (MAX_STAGES + s), ph ^ 1);      // the MMAs that read the next stage have retired
+        }
+    };
+    constexpr int NX = 2 * GEN_NJ;                                  // features per thread and group
+    auto load_x = [&](int tile, int g, float (&x)[NX]) {          // this thread's features of its pattern (0 outside)
+        const long long n = (long long)tile * BN + cta_rank * 128 + gt;
+        const int i0 = g * 8 + hf * NX;
+#pragma unroll
+        for (int j = 0; j < NX; ++j) x[j] = 0.f;
+        if (tile >= total_tiles || n >= N) return;
+        const float *xr = X + n * F + i0;
+        if (vec) {
+#pragma unroll
+            for (int q = 0; q < NX / 4; ++q)
+                if (i0 + 4 * q < F) {
+                    const float4 v = __ldg(reinterpret_cast<const float4 *>(xr) + q);
+                    x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
+                }
+        } else {
+#pragma unroll
+            for (int j = 0; j < NX; ++j) if (i0 + j < F) x[j] = __ldg(xr + j);
+        }
+    };
+
+    float xn[NX];
+    load_x(pair, 0, xn);
+    for (int tile = pair; tile < total_tiles; tile += n_pairs) {
+        const long long n = (long long)tile * BN + cta_rank * 128 + gt;
+        const float one = n < N ? 1.f : 0.f;
+        const float2 one2 = make_float2(one, one);
+        cidx = 0;
+        for (int g = 0; g < ngroups; ++g) {
+            float2 x[GEN_NJ];
+#pragma unroll
+            for (int j = 0; j < GEN_NJ; ++j) x[j] = make_float2(xn[2 * j], xn[2 * j + 1]);
+            // fetch the next group's features (the next tile's first group at the end) while this one is generated
+            if (g + 1 < ngroups) load_x(tile, g + 1, xn); else load_x(tile + n_pairs, 0, xn);
+            float2 ones[GEN_NJ];
+#pragma unroll
+            for (int j = 0; j < GEN_NJ; ++j) ones[j] = one2;
+            put(ones);                              // tau = 0: the constant term
+            if (FAMILY == GAME_CHEB) {
+                float2 tm1[GEN_NJ], t0[GEN_NJ], x2[GEN_NJ];
+#pragma unroll
+                for (int j = 0; j < GEN_NJ; ++j) { tm1[j] = one2; t0[j] = __fmul2_rn(x[j], one2); x2[j] = __fadd2_rn(x[j], x[j]); }
+                put(t0);                      // T_1 (degree >= 1 always)
+                // two steps per iteration, the two state registers trading places: no register moves
+                int m = 2;
+                for (; m + 1 <= d; m += 2) {
+#pragma unroll
+                    for (int j = 0; j < GEN_NJ; ++j) tm1[j] = __ffma2_rn(x2[j], t0[j], make_float2(-tm1[j].x, -tm1[j].y));
+                    put(tm1);
+#pragma unroll
+                    for (int j = 0; j < GEN_NJ; ++j) t0[j] = __ffma2_rn(x2[j], tm1[j], make_float2(-t0[j].x, -t0[j].y));
+                    put(t0);
+                }
+                if (m <= d) {
+#pragma unroll
+                    for (int j = 0; j < GEN_NJ; ++j) tm1[j] = __ffma2_rn(x2[j], t0[j], make_float2(-tm1[j].x, -tm1[j].y));
+                    put(tm1);
+                }
+            } else {
+                // cos (m+1)x = 2 cos x cos mx - cos (m-1)x, and the same for sin: one FFMA per value.  In fp32 the
+                // recurrence's error grows like m^2 eps / 2 at worst (x -> 0): 3e-5 at m = 32, far below fp16's 2^-11.
+                float2 C2[GEN_NJ], c[GEN_NJ], cm[GEN_NJ], sn[GEN_NJ], sm[GEN_NJ];
+#pragma unroll
+                for (int j = 0; j < GEN_NJ; ++j) {
+                    float2 C, S;
+                    __sincosf(x[j].x, &S.x, &C.x);                    // |x| <= pi is checked at load for this variant
+                    __sincosf(x[j].y, &S.y, &C.y);
+                    C2[j] = __fadd2_rn(C, C);
+                    cm[j] = one2; c[j] = __fmul2_rn(C, one2);
+                    sm[j] = make_float2(0.f, 0.f); sn[j] = __fmul2_rn(S, one2);
+                }
+                put(c);                          // cos x
+                put(sn);                      // sin x
+                int m = 2;
+                for (; m + 1 <= d; m += 2) {
+#pragma unroll
+                    for (int j = 0; j < GEN_NJ; ++j) cm[j] = __ffma2_rn(C2[j], c[j], make_float2(-cm[j].x, -cm[j].y));
+                    put(cm);
+#pragma unroll
+                    for (int j = 0; j < GEN_NJ; ++j) sm[j] = __ffma2_rn(C2[j], sn[j], make_float2(-sm[j].x, -sm[j].y));
+                    put(sm);
+#pragma unroll
+                    for (int j = 0; j < GEN_NJ; ++j) c[j] = __ffma2_rn(C2[j], cm[j], make_float2(-c[j].x, -c[j].y));
+                    put(c);
+#pragma unroll
+                    for (int j = 0; j < GEN_NJ; ++j) sn[j] = __ffma2_rn(C2[j], sm[j], make_float2(-sn[j].x, -sn[j].y));
+                    put(sn);
+                }
+                if (m <= d) {
+#pragma unroll
+                    for (int j = 0; j < GEN_NJ; ++j) cm[j] = __ffma2_rn(C2[j], c[j], make_float2(-cm[j].x, -cm[j].y));
+                    put(cm);
+#pragma unroll
+                    for (int j = 0; j < GEN_NJ; ++j) sm[j] = __ffma2_rn(C2[j], sn[j], make_float2(-sm[j].x, -sm[j].y));
+                    put(sm);
+                }
+            }
+        }
+        float2 zeros[GEN_NJ];
+#pragma unroll
+        for (int j = 0; j < GEN_NJ; ++j) zeros[j] = make_float2(0.f, 0.f);
+        while (cidx < nchunks) put(zeros);                   // K padded up to whole k-blocks
+    }
+}
+
 // ---- the kernel -----------------------------------------------------------------------------------------
-template <int CG, int ACT, bool TMSE, int EW>
-__global__ void __launch_bounds__(64 + 32 * EW, 1)
+template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY>
+__global__ void __launch_bounds__(64 + 32 * EW + (SRC == SRC_GEN ? 32 * GEN_WARPS : 0), 1)
 fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmE,
                   int n_tiles, int m_blocks, int k_blocks, long long N, const float *__restrict__ tgt, float R,
-                  float *__restrict__ partial, int Ppad, const DevState *state)
+                  float *__restrict__ partial, int Ppad, const DevState *state,
+                  const float *__restrict__ X, int F, int degree)
 {
     using C = Cfg<CG>;
+    static_assert(SRC == SRC_TMA || CG == 2, "the generator variant runs as CTA pairs");
+    constexpr int NSTAGES = SRC == SRC_GEN ? GEN_STAGES : C::STAGES;
+    constexpr int WARP_GEN0 = WARP_EPI0 + EW;
     if (state && state->stopped) return;          // uniform across the grid: nobody has touched a barrier yet
 
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t *gbase = smem_raw + (base - smem_u32(smem_raw));
-    const uint32_t bar0 = base + C::STAGES * C::STAGE_BYTES;
+    // operand area: SRC_TMA a ring of (A, B) k-block stages; SRC_GEN the resident A tile (k_blocks blocks) + a B ring
+    const uint32_t ring_bytes = SRC == SRC_GEN ? (uint32_t)(k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES)
+                                               : (uint32_t)(C::STAGES * C::STAGE_BYTES);
+    const uint32_t bar0 = base + ring_bytes;
     auto full_bar = [&](int s) { return bar0 + 8u * s; };
-    auto empty_bar = [&](int s) { return bar0 + 8u * (C::STAGES + s); };
-    auto tfull_bar = [&](int a) { return bar0 + 8u * (2 * C::STAGES + a); };
-    auto tempty_bar = [&](int a) { return bar0 + 8u * (2 * C::STAGES + 2 + a); };
-    const uint32_t tmem_slot = bar0 + 8u * (2 * C::STAGES + 4);
-    volatile uint32_t *tmem_slot_g = reinterpret_cast<volatile uint32_t *>(gbase + C::STAGES * C::STAGE_BYTES + 8 * (2 * C::STAGES + 4));
-    float *tgt_s = reinterpret_cast<float *>(gbase + C::STAGES * C::STAGE_BYTES + 256);   // [3][BN]
+    auto empty_bar = [&](int s) { return bar0 + 8u * (MAX_STAGES + s); };
+    auto tfull_bar = [&](int a) { return bar0 + 8u * (2 * MAX_STAGES + a); };
+    auto tempty_bar = [&](int a) { return bar0 + 8u * (2 * MAX_STAGES + 2 + a); };
+    const uint32_t afull_bar = bar0 + 8u * (2 * MAX_STAGES + 4);      // SRC_GEN: the resident A tile has landed
+    const uint32_t tmem_slot = bar0 + 8u * (2 * MAX_STAGES + 5);
+    volatile uint32_t *tmem_slot_g = reinterpret_cast<volatile uint32_t *>(gbase + ring_bytes + 8 * (2 * MAX_STAGES + 5));
+    float *tgt_s = reinterpret_cast<float *>(gbase + ring_bytes + 256);   // [3][BN]
     float *sum_s = tgt_s + 3 * BN;                                                        // [2][4][BM]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -281,8 +461,10 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     const int total_tiles = n_tiles * m_blocks;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < C::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        // SRC_GEN: a B stage is full when the generator warps of BOTH CTAs have published their half
+        for (int s = 0; s < NSTAGES; ++s) { mbar_init(full_bar(s), SRC == SRC_GEN ? CG : 1); mbar_init(empty_bar(s), 1); }
         for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), CG * EW); }
+        mbar_init(afull_bar, 1);
         fence_barrier_init();
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmC) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmE) : "memory");
@@ -296,7 +478,27 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
 
     if (warp == WARP_TMA) {
         // ===== TMA producer =====
-        if (lane == 0) {
+        if (lane == 0 && SRC == SRC_GEN) {
+            // the population tile is loaded ONCE and stays: block kb of this CTA's 128 chromosomes at base + kb * A_BYTES
+            if (cta_rank == 0) mbar_expect_tx(afull_bar, (uint32_t)(CG * k_blocks * A_BYTES));
+            for (int kb = 0; kb < k_blocks; ++kb)
+                tma_load_2d<CG>(base + kb * A_BYTES, &tmC, kb * BKB, (int)cta_rank * BM, afull_bar);
+        }
+        if (SRC == SRC_GEN) {
+            // relay: the generators never stall on the hand-over -- each thread makes its stores visible to the async
+            // proxy and arrives (non-blocking) on the stage's named barrier; this otherwise idle warp completes that
+            // barrier and performs the one mbarrier arrival per CTA and stage on the leader's barrier.  (Arriving on
+            // the mbarrier straight from the generator warps was measured slower: 0.322 vs 0.287 ms on config 4.)
+            int s = 0;
+            for (int tile = pair; tile < total_tiles; tile += n_pairs)
+                for (int kb = 0; kb < k_blocks; ++kb) {
+                    asm volatile("bar.sync %0, %1;" ::"r"(GEN_BAR0 + s), "n"(32 * GEN_WARPS + 32) : "memory");
+                    if (lane == 0) {
+                        if (cta_rank == 0) mbar_arrive(full_bar(s)); else mbar_arrive_cluster(full_bar(s), 0);
+                    }
+                    if (++s == GEN_STAGES) s = 0;
+                }
+        } else if (lane == 0) {
             int s = 0; uint32_t ph = 0;
             for (int tile = pair; tile < total_tiles; tile += n_pairs) {
                 const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
@@ -308,7 +510,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                     if (CG == 1 || cta_rank == 0) mbar_expect_tx(full_bar(s), CG * C::STAGE_BYTES);
                     tma_load_2d<CG>(sa, &tmC, kb * BKB, rowC, full_bar(s));
                     tma_load_2d<CG>(sb, &tmE, 0, rowE + kb * BN, full_bar(s));
-                    if (++s == C::STAGES) { s = 0; ph ^= 1; }
+                    if (++s == NSTAGES) { s = 0; ph ^= 1; }
                 }
             }
         }
@@ -318,14 +520,16 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             constexpr uint32_t idesc = make_idesc(BM * CG, BN);
             int s = 0; uint32_t ph = 0;
             int acc = 0; uint32_t aph = 0;
+            if (SRC == SRC_GEN) mbar_wait(afull_bar, 0);      // resident population tile of both CTAs
             for (int tile = pair; tile < total_tiles; tile += n_pairs) {
                 mbar_wait(tempty_bar(acc), aph ^ 1);          // epilogue has drained this accumulator
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
                 for (int kb = 0; kb < k_blocks; ++kb) {
-                    mbar_wait(full_bar(s), ph);               // operands have landed
+                    mbar_wait(full_bar(s), ph);               // operands have landed (SRC_GEN: were generated)
                     tc_fence_after();
-                    const uint32_t sa = base + s * C::STAGE_BYTES, sb = sa + A_BYTES;
+                    const uint32_t sa = SRC == SRC_GEN ? base + kb * A_BYTES : base + s * C::STAGE_BYTES;
+                    const uint32_t sb = SRC == SRC_GEN ? base + k_blocks * A_BYTES + s * GEN_B_BYTES : sa + A_BYTES;
                     const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sb);
 #pragma unroll
                     for (int k = 0; k < BKB / UMMA_K; ++k) {
@@ -333,12 +537,16 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                         umma_f16<CG>(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
                     }
                     umma_commit<CG>(empty_bar(s));            // stage reusable when these MMAs retire
-                    if (++s == C::STAGES) { s = 0; ph ^= 1; }
+                    if (++s == NSTAGES) { s = 0; ph ^= 1; }
                 }
                 umma_commit<CG>(tfull_bar(acc));              // accumulator complete
                 if (++acc == 2) { acc = 0; aph ^= 1; }
             }
         }
+    } else if (SRC == SRC_GEN && warp >= WARP_GEN0) {
+        // ===== generator warps (a1 inside the kernel) =====
+        generate_expansion<FAMILY>(X, F, degree, N, k_blocks, pair, n_pairs, total_tiles, (int)cta_rank,
+                                   threadIdx.x - 32 * WARP_GEN0, gbase + k_blocks * A_BYTES, bar0);
     } else {
         // ===== epilogue warps =====
         // EW warps: warp w may touch TMEM lanes 32*(w%4).., so four warps cover the 128 chromosomes and EW/4 such
@@ -422,9 +630,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                         tmem_ld32(lane_addr + (uint32_t)((acc ^ 1) * BN), nxt);
                     }
                 }
-#ifndef GAME_PROBE_NO_EPI
                 epilogue_chunk<ACT, TMSE>(cur, ts + 32 * c, R, acc2);
-#endif
             }
             sum_s[(sb * 4 + cb) * BM + row] = ((acc2[0].x + acc2[0].y) + (acc2[1].x + acc2[1].y)) + ((acc2[2].x + acc2[2].y) + (acc2[3].x + acc2[3].y));
             prev_off = (long long)n_tile * Ppad + (m_blk * CG + (int)cta_rank) * BM + row;
@@ -551,23 +757,25 @@ int tensor_prepare(game_ctx *ctx)
     return GAME_OK;
 }
 
-template <int CG, int ACT, bool TMSE, int EW>
+template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY>
 static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, const DevState *state)
 {
     using C = Cfg<CG>;
-    auto kern = fitness_tc_kernel<CG, ACT, TMSE, EW>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        GAME_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-        attr_set = true;
+    auto kern = fitness_tc_kernel<CG, ACT, TMSE, EW, SRC, FAMILY>;
+    const int k_blocks = ctx->Kpad / BKB;
+    const int smem = SRC == SRC_GEN ? k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES : C::SMEM;
+    static int attr_smem = 0;
+    if (smem > attr_smem) {
+        GAME_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        attr_smem = smem;
     }
     long long total = (long long)n_tiles * m_blocks;
     int pairs = ctx->sm_count / CG;
     if (pairs > total) pairs = (int)total;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)(pairs * CG));
-    cfg.blockDim = dim3(64 + 32 * EW);
-    cfg.dynamicSmemBytes = C::SMEM;
+    cfg.blockDim = dim3(64 + 32 * EW + (SRC == SRC_GEN ? 32 * GEN_WARPS : 0));
+    cfg.dynamicSmemBytes = smem;
     cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -575,14 +783,37 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     cfg.attrs = attr; cfg.numAttrs = 1;
     KernelTimer timer(ctx);
     GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, ((const CUtensorMap *)ctx->tmap_E)[CG - 1], n_tiles,
-                                      m_blocks, ctx->Kpad / BKB, ctx->N, (const float *)ctx->t, ctx->R, ctx->partial, Ppad, state));
+                                      m_blocks, k_blocks, ctx->N, (const float *)ctx->t, ctx->R, ctx->partial, Ppad, state,
+                                      (const float *)ctx->X, ctx->F, ctx->degree));
     return GAME_OK;
+}
+
+// north_star (1): materialise E or regenerate it in the kernel, by measured cost.  The generator variant needs the
+// whole population in ONE CTA pair (Ppad = 256) and its fp16 copy resident in shared memory beside the B ring, i.e.
+// exactly the shapes where streaming the materialised E16 could limit the kernel (bytes of E16 per flop ~ 1/P).
+// Measured on B200 on config 4 (N = 1e6, K = 544, P = 256), same box: materialised 0.268 ms, regenerated 0.287 ms
+// -- the generator's math is not what limits it (a no-math probe ran at the same 0.287 ms); the CTA-pair ring does
+// (47 % tensor-pipe use against 71 %).  So AUTO streams the materialised matrix; the regenerated variant stays
+// selectable (game_set_expansion) and is held to the same parity tests.  The trigonometric generator uses the fast
+// sincos, accurate on |x| <= pi only (checked against the dataset at load).
+int tensor_expansion(const game_ctx *ctx, int P)
+{
+    const int Ppad = ((P + 255) / 256) * 256;
+    const int k_blocks = ctx->Kpad / BKB;
+    const bool can = tc_permuted(ctx->family) && Ppad == 256 && ctx->X != nullptr &&
+                     k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES <= 227 * 1024 &&
+                     (ctx->family != GAME_TRIG || ctx->x_maxabs <= 3.14159f);
+    if (ctx->expand_mode == GAME_EXPAND_REGENERATED) return can ? GAME_EXPAND_REGENERATED : -1;
+    return GAME_EXPAND_MATERIALIZED;
 }
 
 int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer)
 {
     const int Ppad = ((P + 255) / 256) * 256;
-    const int cg = cta_group(ctx, Ppad);
+    const int expansion = tensor_expansion(ctx, P);
+    if (expansion < 0) return fail(ctx, GAME_ERR_UNSUPPORTED, "regenerated expansion unavailable for this shape (needs P <= 256, K <= 576 after padding, trig: max|X| <= pi)");
+    const int src = expansion == GAME_EXPAND_REGENERATED ? SRC_GEN : SRC_TMA;
+    const int cg = src == SRC_GEN ? 2 : cta_group(ctx, Ppad);
     const int n_tiles = (int)(ctx->Npad256 / BN);
     const int m_blocks = Ppad / (BM * cg);
     long long n = (long long)P * ctx->K;
@@ -594,20 +825,25 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     GAME_LAUNCHED(ctx);
     int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_C, ctx->C16, Ppad, ctx->Kpad, BM);
     if (rc) return rc;
-#define GAME_TC_EW(CGV, M, T)                                                                    \
-    rc = ew == 16 ? launch_variant<CGV, M, T, 16>(ctx, n_tiles, m_blocks, Ppad, state)           \
-                  : launch_variant<CGV, M, T, 8>(ctx, n_tiles, m_blocks, Ppad, state)
-#define GAME_TC_MODE(CGV, M)                                                                     \
-    if (tmse) { GAME_TC_EW(CGV, M, true); } else { GAME_TC_EW(CGV, M, false); }
-#define GAME_TC_DISPATCH(CGV)                                                                    \
-    switch (mode) {                                                                              \
-    case MODE_IDENTITY: GAME_TC_MODE(CGV, MODE_IDENTITY); break;                                 \
-    case MODE_SIG_TANH32: GAME_TC_MODE(CGV, MODE_SIG_TANH32); break;                             \
-    default: GAME_TC_MODE(CGV, MODE_SIG_EXACT); break;                                           \
+#define GAME_TC_EW(CGV, M, T)                                                                              \
+    rc = ew == 16 ? launch_variant<CGV, M, T, 16, SRC_TMA, GAME_TRIG>(ctx, n_tiles, m_blocks, Ppad, state)     \
+                  : launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG>(ctx, n_tiles, m_blocks, Ppad, state)
+#define GAME_TC_GEN(M, T)                                                                                  \
+    rc = ctx->family == GAME_TRIG ? launch_variant<2, M, T, 8, SRC_GEN, GAME_TRIG>(ctx, n_tiles, 1, Ppad, state) \
+                                  : launch_variant<2, M, T, 8, SRC_GEN, GAME_CHEB>(ctx, n_tiles, 1, Ppad, state)
+#define GAME_TC_MODE(CGV, M)                                                                               \
+    if (src == SRC_GEN) { if (tmse) { GAME_TC_GEN(M, true); } else { GAME_TC_GEN(M, false); } }            \
+    else if (tmse) { GAME_TC_EW(CGV, M, true); } else { GAME_TC_EW(CGV, M, false); }
+#define GAME_TC_DISPATCH(CGV)                                                                              \
+    switch (mode) {                                                                                        \
+    case MODE_IDENTITY: GAME_TC_MODE(CGV, MODE_IDENTITY); break;                                           \
+    case MODE_SIG_TANH32: GAME_TC_MODE(CGV, MODE_SIG_TANH32); break;                                       \
+    default: GAME_TC_MODE(CGV, MODE_SIG_EXACT); break;                                                     \
     }
-    if (cg == 2) { GAME_TC_DISPATCH(2); } else { GAME_TC_DISPATCH(1); }
+    if (cg == 2 || src == SRC_GEN) { GAME_TC_DISPATCH(2); } else { GAME_TC_DISPATCH(1); }
 #undef GAME_TC_DISPATCH
 #undef GAME_TC_MODE
+#undef GAME_TC_GEN
 #undef GAME_TC_EW
     if (rc) return rc;
     ++ctx->launches;

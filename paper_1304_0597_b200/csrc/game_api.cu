@@ -132,8 +132,8 @@ static int load_common(game_ctx *c, const float *X, const float *targets, long l
     GAME_CUDA(c, cudaMalloc(&c->X, (size_t)N * c->F * sizeof(float)));
     GAME_CUDA(c, cudaMalloc(&c->t, (size_t)c->Npad256 * sizeof(float)));
     GAME_CUDA(c, cudaMalloc(&c->ET, (size_t)K * c->Npad * sizeof(float)));
-    GAME_CUDA(c, cudaMalloc(&flag, 2 * sizeof(int)));
-    GAME_CUDA(c, cudaMemsetAsync(flag, 0, 2 * sizeof(int), c->stream));
+    GAME_CUDA(c, cudaMalloc(&flag, 3 * sizeof(int)));      // [0] non-finite input, [1] max|E| bits, [2] max|X| bits
+    GAME_CUDA(c, cudaMemsetAsync(flag, 0, 3 * sizeof(int), c->stream));
     GAME_CUDA(c, cudaMemsetAsync(c->t, 0, (size_t)c->Npad256 * sizeof(float), c->stream));
     GAME_CUDA(c, cudaMemsetAsync(c->ET, 0, (size_t)K * c->Npad * sizeof(float), c->stream));
     GAME_CUDA(c, cudaMemcpyAsync(c->X, X, (size_t)N * c->F * sizeof(float), cudaMemcpyDefault, c->stream));
@@ -149,7 +149,7 @@ static int load_common(game_ctx *c, const float *X, const float *targets, long l
         rc = launch_expand_fp16(c, reinterpret_cast<float *>(flag + 1));
         if (rc) { cudaFree(flag); return rc; }
     }
-    int h[2] = {0, 0};
+    int h[3] = {0, 0, 0};
     GAME_CUDA(c, cudaMemcpyAsync(h, flag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     GAME_CUDA(c, cudaStreamSynchronize(c->stream));
     cudaFree(flag);
@@ -160,6 +160,7 @@ static int load_common(game_ctx *c, const float *X, const float *targets, long l
     if (tensor_path_built()) {
         float mx;
         memcpy(&mx, &h[1], sizeof(float));
+        memcpy(&c->x_maxabs, &h[2], sizeof(float));
         // fp16 rounding is relative: sums over features (tied families) of magnitude ~F would carry an absolute
         // error ~F*2^-11 into z, outside the 1e-3 class, so the tensor path is offered for |E| <= 2 only
         c->tensor_ok = mx <= 2.0f;
@@ -257,6 +258,16 @@ int game_set_path(game_ctx *c, int path)
 }
 
 int game_resolved_path(const game_ctx *c, int P) { return c ? resolve_path(c, P) : -1; }
+
+int game_set_expansion(game_ctx *c, int mode)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (mode < GAME_EXPAND_AUTO || mode > GAME_EXPAND_REGENERATED) return fail(c, GAME_ERR_INVALID_ARG, "bad expansion mode");
+    c->expand_mode = mode;
+    return GAME_OK;
+}
+
+int game_resolved_expansion(const game_ctx *c, int P) { return (c && c->N && P >= 1) ? tensor_expansion(c, P) : -1; }
 
 int game_load(game_ctx *c, const float *X, const float *t, long long N) { return load_common(c, X, t, N); }
 int game_load_host(game_ctx *c, const float *X, const float *t, long long N) { return load_common(c, X, t, N); }

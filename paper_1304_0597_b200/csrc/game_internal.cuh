@@ -71,7 +71,7 @@ struct FitnessCfg {
 
 struct game_ctx {
     int family = 0, degree = 0, F = 0, K = 0;
-    int act = GAME_ACT_SIGMOID, err = GAME_ERR_MSE, path = GAME_PATH_AUTO;
+    int act = GAME_ACT_SIGMOID, err = GAME_ERR_MSE, path = GAME_PATH_AUTO, expand_mode = GAME_EXPAND_AUTO;
     float R = 0.f;
     cudaStream_t stream = 0;
     int sm_count = 148;
@@ -86,6 +86,7 @@ struct game_ctx {
     long long Npad256 = 0;
     int Kpad = 0;              // K rounded up to TC_KBLK
     bool tensor_ok = false;    // E16 built and all |E| representable
+    float x_maxabs = 0.f;      // max |X| of the loaded dataset
 
     // population / loop state
     int P = 0;
@@ -165,6 +166,7 @@ int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scra
 // fitness_tc.cu
 bool tensor_path_built();
 int tensor_prepare(game_ctx *ctx);                               // tensor maps etc. after load
+int tensor_expansion(const game_ctx *ctx, int P);                // GAME_EXPAND_MATERIALIZED / _REGENERATED, or -1
 int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer);
 
 // ga.cu

@@ -402,3 +402,83 @@ def test_trajectory_paper_literal(orc):
     trajectory(orc, wl.paper_literal(degree=4), 40)
     # and on row-replicated data (L326): same shape of run, 4x the rows
     trajectory(orc, wl.paper_literal(degree=2, N=8400), 6)
+
+
+# ---- north_star (1): the expansion regenerated inside the fused kernel (game_set_expansion) -----------------------
+REGEN_SHAPES = [
+    # family, degree, F, N, P
+    (TRIG, 8, 32, 1000, 256),      # config 4's K = 544 (9 k-blocks), ragged N over several tiles
+    (CHEB, 12, 24, 700, 130),      # ragged P, T = 13 terms per feature
+    (TRIG, 4, 11, 2100, 20),       # F not a multiple of 8 (scalar feature loads, padded feature lanes)
+    (CHEB, 6, 16, 257, 256),       # one full tile + a one-pattern tail
+    (TRIG, 1, 3, 5, 2),            # degenerate: K = 9, fewer patterns than one tile
+    (CHEB, 32, 8, 300, 64),        # deepest recurrence the ABI allows
+]
+
+
+@pytest.mark.parametrize("shape", REGEN_SHAPES)
+@pytest.mark.parametrize("act,err,R", [(SIGMOID, MSE, 0.0), (SIGMOID, TMSE, 0.49), (IDENTITY, MSE, 0.0)])
+def test_fitness_parity_regenerated(orc, shape, act, err, R):
+    fam, d, F, N, P = shape
+    rng = np.random.default_rng(29)
+    X = rng.uniform(-1, 1, (N, F)).astype(np.float32)
+    t = rng.integers(0, 2, N).astype(np.float32)
+    K = orc.num_terms(fam, d, F)
+    scale = 1.0 if act == SIGMOID else 1.0 / np.sqrt(K)
+    pop = (rng.uniform(-1, 1, (P, K)) * scale).astype(np.float32)
+    ctx = make_ctx(fam, d, X, t, act, err, R, g.GAME_PATH_TENSOR)
+    assert ctx.resolved_path(P) == g.GAME_PATH_TENSOR
+    assert ctx.resolved_expansion(P) == g.GAME_EXPAND_MATERIALIZED          # AUTO: the measured choice
+    ref_fit = ctx.fitness(dev(pop)).cpu().numpy()
+    ctx.set_expansion(g.GAME_EXPAND_REGENERATED)
+    assert ctx.resolved_expansion(P) == g.GAME_EXPAND_REGENERATED
+    got = ctx.fitness(dev(pop)).cpu().numpy()
+    check_fitness(orc, got, fam, d, X, t, pop, act, err, R, g.GAME_PATH_TENSOR, "regenerated")
+    # the two sources round the same values to fp16 (fp64 vs fp32 arithmetic before the rounding): results agree
+    # closely (TMSE is discontinuous at the tube, so it is held to the oracle bound above only)
+    if err != TMSE:
+        assert np.allclose(got, ref_fit, rtol=2e-4, atol=2e-6)
+    perm = rng.permutation(P)                                              # P20 holds for this variant too
+    got2 = ctx.fitness(dev(pop[perm])).cpu().numpy()
+    assert np.array_equal(got2.view(np.uint32), got[perm].view(np.uint32))
+
+
+def test_regenerated_expansion_limits():
+    rng = np.random.default_rng(31)
+    # more than one CTA pair of chromosomes: unavailable, and the call says so
+    X = rng.uniform(-1, 1, (300, 8)).astype(np.float32)
+    t = np.zeros(300, np.float32)
+    ctx = make_ctx(CHEB, 3, X, t, path=g.GAME_PATH_TENSOR)
+    ctx.set_expansion(g.GAME_EXPAND_REGENERATED)
+    assert ctx.resolved_expansion(256) == g.GAME_EXPAND_REGENERATED and ctx.resolved_expansion(257) == -1
+    with pytest.raises(g.GameError) as e:
+        ctx.fitness(dev(np.zeros((257, ctx.num_terms()), np.float32)))
+    assert e.value.code == 5
+    # trigonometric family outside [-pi, pi]: the fast sincos is not offered
+    X2 = (X * 4.0).astype(np.float32)
+    ctx2 = make_ctx(TRIG, 3, X2, t, path=g.GAME_PATH_TENSOR)
+    ctx2.set_expansion(g.GAME_EXPAND_REGENERATED)
+    assert ctx2.resolved_expansion(64) == -1
+    ctx2.set_expansion(g.GAME_EXPAND_AUTO)
+    assert ctx2.resolved_expansion(64) == g.GAME_EXPAND_MATERIALIZED
+
+
+def test_trajectory_regenerated(orc):
+    """A GA run with the regenerated expansion: operators bit-exact, fitness within the tensor class."""
+    w = wl.config(1).scaled(P=64, generations=6)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    ctx = make_ctx(fam, d, X, t, w.act, w.err, w.R, g.GAME_PATH_TENSOR)
+    ctx.set_expansion(g.GAME_EXPAND_REGENERATED)
+    gp = g.ga_params(P=w.P)
+    gpo = orc.GaParams(P=w.P, tournament_size=3, elitism=2, elite_mode=0, selection=0, init_mode=1,
+                       p_crossover=0.9, p_mutation=0.05, stop_error=-1.0)
+    ctx.evolve(0, w.seed, gp)
+    for gen in range(w.generations):
+        pop, fit, order = ctx.get_population_host()
+        check_fitness(orc, fit, fam, d, X, t, pop, w.act, w.err, w.R, g.GAME_PATH_TENSOR, "gen %d" % gen)
+        assert np.array_equal(order, orc.rank(fit))
+        nxt = orc.ga_step(gpo, w.seed, gen, order, fit, pop)
+        ctx.evolve(1, w.seed, gp)
+        pop2, _, _ = ctx.get_population_host()
+        assert np.array_equal(pop2.view(np.uint32), nxt.view(np.uint32))
