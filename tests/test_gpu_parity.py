@@ -256,15 +256,15 @@ def test_error_paths():
 
 
 # ---- whole GA runs, generation by generation, GPU population injected into the oracle (c.4) --------
-def trajectory(orc, w, generations, full_check_every=1, subset=None):
+def trajectory(orc, w, generations, full_check_every=1, subset=None, selection=0, elite_mode=0):
     fam, d = w.family, w.degree
     X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
     ctx = make_ctx(fam, d, X, t, w.act, w.err, w.R)
     path = ctx.resolved_path(w.P)
     gp_g = g.ga_params(P=w.P, tournament_size=w.tournament_size, elitism=w.elitism, init_mode=w.init_mode,
-                       p_crossover=w.p_crossover, p_mutation=w.p_mutation)
-    gp_o = orc.GaParams(P=w.P, tournament_size=w.tournament_size, elitism=w.elitism, elite_mode=0, selection=0,
-                        init_mode=w.init_mode, p_crossover=w.p_crossover, p_mutation=w.p_mutation, stop_error=-1.0)
+                       p_crossover=w.p_crossover, p_mutation=w.p_mutation, selection=selection, elite_mode=elite_mode)
+    gp_o = orc.GaParams(P=w.P, tournament_size=w.tournament_size, elitism=w.elitism, elite_mode=elite_mode,
+                        selection=selection, init_mode=w.init_mode, p_crossover=w.p_crossover, p_mutation=w.p_mutation, stop_error=-1.0)
     res = ctx.evolve(0, w.seed, gp_g)                         # init + fitness + rank
     pop, fit, order = ctx.get_population_host()
     assert np.array_equal(pop.view(np.uint32), orc.init_population(w.init_mode, w.seed, w.P, w.K).view(np.uint32))
@@ -307,6 +307,15 @@ def test_trajectory_paper_parameters(orc):
     w = wl.config(1)
     from dataclasses import replace
     trajectory(orc, replace(w, P=23, tournament_size=4, p_mutation=0.2), 20)
+
+
+@pytest.mark.parametrize("cfg,init_mode,selection,elite_mode", [(3, 0, 1, 0), (3, 2, 1, 1), (2, 0, 1, 1), (2, 2, 0, 1)])
+def test_trajectory_roulette_and_init_modes_at_scale(orc, cfg, init_mode, selection, elite_mode):
+    # roulette selection (R4), init modes U[-1,1) / U[0,1) and top-e elitism on the larger
+    # configs at full P; fitness on a chromosome subset where the oracle would need minutes for all of them
+    from dataclasses import replace
+    w = replace(wl.config(cfg), init_mode=init_mode)
+    trajectory(orc, w, 3, subset=48 if cfg == 3 else None, selection=selection, elite_mode=elite_mode)
 
 
 def test_resume_and_single_call_agree(orc):
