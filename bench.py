@@ -201,8 +201,12 @@ def run_ours(args, w):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peaks = read_peaks()
 
-    # replicas: every rank runs the same-shaped problem with its own seed (weak scaling, no data-path collective)
-    wr = replicas.replica_workload(w, rank)
+    # default: replicas -- every rank runs the same-shaped problem with its own seed (weak scaling, no data-path
+    # collective).  --shard: ONE problem, its patterns split over the ranks, one all-reduce of P doubles per generation
+    # (strong scaling; paper_1304_0597_b200/sharded.py).
+    from paper_1304_0597_b200 import sharded
+    wr = w if args.shard else replicas.replica_workload(w, rank)
+    lo, hi = sharded.shard_rows(w.N, world, rank) if args.shard else (0, w.N)
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
         # planted targets need a forward pass of the planted chromosome: the library's own game_predict
@@ -221,7 +225,7 @@ def run_ours(args, w):
         ctx.set_error(wr.err, wr.R)
         if args.path != "auto":
             ctx.set_path({"fp32": g.GAME_PATH_FP32, "tensor": g.GAME_PATH_TENSOR}[args.path])
-        Xp, tp = torch.from_numpy(X).pin_memory(), torch.from_numpy(t).pin_memory()
+        Xp, tp = torch.from_numpy(X[lo:hi]).pin_memory(), torch.from_numpy(t[lo:hi]).pin_memory()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         ctx.load_host(Xp.numpy(), tp.numpy())
@@ -238,7 +242,21 @@ def run_ours(args, w):
                 dist.barrier()
             torch.cuda.synchronize()
 
-        ctx.evolve(max(args.warmup, 3), wr.seed, gp)            # W untimed warm-up steps (also creates the population)
+        if args.shard:
+            sg = sharded.ShardedGame(ctx, w.N, world)
+
+            class _Res:
+                pass
+
+            def evolve(k):
+                done, last = sg.evolve(k, wr.seed, gp)
+                r = _Res()
+                r.generations_run, r.best_error = done, last.best_error
+                return r
+        else:
+            def evolve(k):
+                return ctx.evolve(k, wr.seed, gp)
+        evolve(max(args.warmup, 3))                             # W untimed warm-up steps (also creates the population)
         # The dominant kernel is bracketed by CUDA events inside the timed region -- except on the launch-latency
         # bound configs (1-2), where per-launch events would perturb the captured-graph loop being timed: there
         # the kernel is timed in a second, identical pass right after.
@@ -250,7 +268,7 @@ def run_ours(args, w):
         barrier()
         launches0 = ctx.launch_count()
         e0.record(stream)
-        res = ctx.evolve(args.steps, wr.seed, gp)               # exactly K steps (+ the final re-evaluation)
+        res = evolve(args.steps)                                # exactly K steps (+ the final re-evaluation)
         e1.record(stream)
         barrier()
         sampler.stop_flag = True
@@ -261,7 +279,7 @@ def run_ours(args, w):
         if separate_pass:
             ctx.set_kernel_timing(True)
             e0.record(stream)
-            ctx.evolve(min(args.steps, 200), wr.seed, gp)
+            evolve(min(args.steps, 200))
             e1.record(stream)
             stream.synchronize()
             kern_pass_ms = e0.elapsed_time(e1)
@@ -270,7 +288,8 @@ def run_ours(args, w):
         sampler.join()
         assert res.generations_run == args.steps
 
-        value, ms_max = replicas.job_throughput(float(w.N) * w.P * (args.steps + 1), world, ms, "cuda")
+        share = 1.0 / world if args.shard else 1.0             # sharded: the ranks split ONE job's evaluations
+        value, ms_max = replicas.job_throughput(float(w.N) * w.P * (args.steps + 1) * share, world, ms, "cuda")
 
         # e2e: the same metric through the C ABI with HOST buffers: population in, fitness out, every step
         pop_host, _, _ = ctx.get_population_host()
@@ -285,7 +304,7 @@ def run_ours(args, w):
             ctx.fitness_host(pop_pin.numpy(), fit_pin.numpy())
         e1.record(stream)
         barrier()
-        e2e_value, _ = replicas.job_throughput(float(w.N) * w.P * e2e_steps, world, e0.elapsed_time(e1), "cuda")
+        e2e_value, _ = replicas.job_throughput(float(hi - lo) * w.P * e2e_steps, world, e0.elapsed_time(e1), "cuda")
         e2e = {"value": e2e_value, "unit": UNIT,
                "h2d_bytes_per_step": int(wr.P * wr.K * 4), "d2h_bytes_per_step": int(wr.P * 4),
                "what": "game_fitness_host: population from pinned host memory in, fitness back out, per step; "
@@ -294,7 +313,7 @@ def run_ours(args, w):
     if rank != 0:
         return
     # roofline of the dominant kernel (fused contraction + epilogue)
-    flops = 2.0 * w.N * w.K * w.P
+    flops = 2.0 * (hi - lo) * w.K * w.P           # what ONE launch of this rank's kernel computes
     avg_s = kern_ms * 1e-3 / max(kern_n, 1)
     if path == g.GAME_PATH_TENSOR:
         # two candidate bounds for the fused kernel: the tensor pipe (2NKP flops) and, for shallow contractions, the
@@ -302,17 +321,17 @@ def run_ours(args, w):
         # 15.9).  The one with the larger floor time binds and is the one reported.
         peak = peaks["bf16_tflops_sustained"]      # fp16 in / fp32 accumulate: same rate as bf16; timed inside a long step
         mufu_peak = 148 * 16 * peaks["sm_max_mhz"] * 1e6
-        t_tensor, t_mufu = flops / (peak * 1e12), float(w.N) * w.P / mufu_peak
+        t_tensor, t_mufu = flops / (peak * 1e12), float(hi - lo) * w.P / mufu_peak
         tensor = {"bound": "tensor", "achieved": flops / avg_s / 1e12, "peak": peak, "unit": "TFLOP/s",
                   "peak_source": "MEASURED_PEAKS.json bf16_tflops_sustained (%s), fp16 = bf16 rate" % peaks["source"]}
         if t_mufu > t_tensor:
-            roof = {"bound": "alu", "achieved": float(w.N) * w.P / avg_s / 1e9, "peak": mufu_peak / 1e9, "unit": "Gop/s",
+            roof = {"bound": "alu", "achieved": float(hi - lo) * w.P / avg_s / 1e9, "peak": mufu_peak / 1e9, "unit": "Gop/s",
                     "peak_source": "special-function unit: 148 SM x 16 tanh lanes/clk x sm_max_mhz (derived; binds because "
                                    "N*P/peak_mufu = %.0f us > 2NKP/peak_tensor = %.0f us)" % (t_mufu * 1e6, t_tensor * 1e6),
                     "tensor_frac": tensor["achieved"] / tensor["peak"], "tensor_tflops": tensor["achieved"]}
         else:
             roof = tensor
-            roof["mufu_frac"] = (float(w.N) * w.P / avg_s) / mufu_peak
+            roof["mufu_frac"] = (float(hi - lo) * w.P / avg_s) / mufu_peak
     else:
         peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
         roof = {"bound": "alu", "achieved": flops / avg_s / 1e12, "peak": peak, "unit": "TFLOP/s",
@@ -332,9 +351,9 @@ def run_ours(args, w):
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms_max / args.steps, "generations_per_sec": args.steps / (ms_max * 1e-3),
-           "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "higher_is_better": True, "scaling": "strong" if args.shard else "weak", "vs_baseline": None,
            "dtype": "f16 operands, f32 accumulate" if path == g.GAME_PATH_TENSOR else "f32",
-           "data": "synthetic", "config": workload_dict(w, path_name), "clocks": sampler.summary(), "e2e": e2e,
+           "data": "synthetic", "config": dict(workload_dict(w, path_name), **({"parallelism": "patterns sharded over %d ranks, all-reduce of P doubles per generation" % world} if args.shard else {})), "clocks": sampler.summary(), "e2e": e2e,
            "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
            "best_error": float(res.best_error), "load_ms": load_ms}
     print(json.dumps(out))
@@ -349,6 +368,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--path", default="auto", choices=["auto", "fp32", "tensor"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shard", action="store_true", help="N>1: split the patterns of ONE problem over the ranks (all-reduce of P doubles per generation) instead of running replicas")
     args = ap.parse_args()
     from paper_1304_0597_b200 import workloads as wl
     w = wl.config(args.config)

@@ -117,6 +117,21 @@ int game_load_host(game_ctx *ctx, const float *X, const float *targets, long lon
 int game_fitness(game_ctx *ctx, const float *pop, int P, float *out);
 int game_fitness_host(game_ctx *ctx, const float *pop, int P, float *out);
 
+
+/* Pattern-sharded evaluation (the paper's future work (iii), L421): when the patterns are split over
+ * several contexts -- one per GPU -- each evaluates its shard and the per-chromosome error totals are added across
+ * shards (one all-reduce of P doubles per generation) before eq. 4's mean is taken.
+ * game_fitness_sums: a1-a5 without the mean: sums[p] = sum over THIS context's patterns of e (eq. 3 / eq. 10), fp64,
+ *   in a fixed order.  pop DEV P x K (or NULL: the context's own population, P ignored), sums DEV P doubles.
+ *   Asynchronous on the context's stream.
+ * game_advance: the rest of one generation from the (summed) totals: fit = sums / N_total (root for RMSE), rank (a6),
+ *   stop test (a7) and, if apply_operators != 0 and the stop test did not fire, a8-a11 on the context's population
+ *   (generation counter + 1).  Every shard calls it with the same totals, seed and parameters and so holds the same
+ *   population afterwards, bit for bit (the random numbers are counter-based).  With one shard and N_total = N it
+ *   reproduces game_evolve(1) exactly.  sums DEV P doubles; res HOST; synchronises the stream. */
+int game_fitness_sums(game_ctx *ctx, const float *pop, int P, double *sums);
+int game_advance(game_ctx *ctx, const double *sums, long long N_total, unsigned long long seed, const game_ga_params *params,
+                 int apply_operators, game_result *res);
 /* Forward pass of ONE chromosome (the paper's test / run use cases, L127-L129): z_out[n] = Out(pat_n),
  * y_out[n] = act(z).  genes: K fp32, z_out / y_out: N fp32, either may be NULL.  DEV pointers. fp32. */
 int game_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out);

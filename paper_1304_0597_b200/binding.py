@@ -27,7 +27,7 @@ ERROR_NAMES = {1: "INVALID_ARG", 2: "NOT_LOADED", 3: "ALLOC", 4: "CUDA", 5: "UNS
 SYMBOLS = [
     "game_create", "game_destroy", "game_num_terms", "game_generation", "game_last_error",
     "game_set_stream", "game_set_activation", "game_set_error", "game_set_path", "game_resolved_path",
-    "game_set_expansion", "game_resolved_expansion",
+    "game_set_expansion", "game_resolved_expansion", "game_fitness_sums", "game_advance",
     "game_load", "game_load_host", "game_fitness", "game_fitness_host", "game_predict", "game_classify",
     "game_set_population", "game_set_generation", "game_evolve", "game_get_population",
     "game_get_population_host", "game_rank", "game_ga_step", "game_init_population", "game_philox",
@@ -79,6 +79,8 @@ def load_library():
         L.game_set_error.argtypes = [vp, i, C.c_float]
         L.game_set_path.argtypes = [vp, i]
         L.game_resolved_path.argtypes = [vp, i]
+        L.game_fitness_sums.argtypes = [vp, vp, i, vp]
+        L.game_advance.argtypes = [vp, vp, ll, u64, C.POINTER(game_ga_params), i, C.POINTER(game_result)]
         L.game_set_expansion.argtypes = [vp, i]
         L.game_resolved_expansion.argtypes = [vp, i]
         L.game_load.argtypes = [vp, vp, vp, ll]
@@ -187,6 +189,23 @@ class Game:
 
     def set_path(self, path):
         self._ck(self._L.game_set_path(self._h, path))
+
+    def fitness_sums(self, pop=None, P=0, out=None):
+        """Per-chromosome fp64 error totals over this context's patterns (pop None: the context's own population of P)."""
+        t = self._torch
+        if pop is not None:
+            P = pop.shape[0]
+            assert pop.shape == (P, self.K)
+        if out is None:
+            out = t.empty(P, dtype=t.float64, device="cuda")
+        self._ck(self._L.game_fitness_sums(self._h, _dev(pop, t.float32), P, _dev(out, t.float64)))
+        return out
+
+    def advance(self, sums, N_total, seed, params, apply_operators=True):
+        res = game_result()
+        self._ck(self._L.game_advance(self._h, _dev(sums, self._torch.float64), N_total, seed, C.byref(params),
+                                      1 if apply_operators else 0, C.byref(res)))
+        return res
 
     def set_expansion(self, mode):
         self._ck(self._L.game_set_expansion(self._h, mode))

@@ -194,8 +194,10 @@ int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scra
 }
 
 // fit[p] = (sum over chunks, ascending, in fp64) / N; RMSE takes the root (eq. 4-5).
+// With `sums` set the fp64 total itself is written instead (game_fitness_sums: the pattern-sharded exchange adds the
+// totals of all shards before the mean is taken).
 __global__ void finalize_kernel(const float *__restrict__ partial, int n_chunks, int Ppad, int P, long long N,
-                                int err, float *__restrict__ out, const DevState *state)
+                                int err, float *__restrict__ out, double *__restrict__ sums, const DevState *state)
 {
     if (state && state->stopped) return;
     __shared__ double red[32][33];
@@ -209,6 +211,7 @@ __global__ void finalize_kernel(const float *__restrict__ partial, int n_chunks,
     if (r == 0 && p < P) {
         double tot = 0.0;
         for (int q = 0; q < 32; ++q) tot += red[q][c];
+        if (sums) { sums[p] = tot; return; }
         double f = tot / (double)N;
         if (err == GAME_ERR_RMSE) f = sqrt(f);
         out[p] = (float)f;
@@ -240,13 +243,14 @@ __global__ void finalize_split_kernel(const float *__restrict__ partial, int n_c
 }
 
 __global__ void finalize_merge_kernel(const double *__restrict__ fin2, int Ppad, int P, long long N, int err,
-                                      float *__restrict__ out, const DevState *state)
+                                      float *__restrict__ out, double *__restrict__ sums, const DevState *state)
 {
     if (state && state->stopped) return;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P) return;
     double tot = 0.0;
     for (int y = 0; y < FIN_SPLIT; ++y) tot += fin2[(long long)y * Ppad + p];
+    if (sums) { sums[p] = tot; return; }
     double f = tot / (double)N;
     if (err == GAME_ERR_RMSE) f = sqrt(f);
     out[p] = (float)f;
@@ -364,19 +368,36 @@ size_t fitness_partial_floats(const game_ctx *ctx, int P)
     return (size_t)(ctx->n_slabs + 2) * Ppad;     // worst case: one row per slab (tensor path pads N to 256)
 }
 
-int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, const DevState *state)
+// fit[p] = sums[p] / N_total (root for RMSE): the tail of a5 after the shards' totals have been added
+__global__ void fit_from_sums_kernel(const double *__restrict__ sums, int P, long long N_total, int err, float *__restrict__ out)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    double f = sums[p] / (double)N_total;
+    if (err == GAME_ERR_RMSE) f = sqrt(f);
+    out[p] = (float)f;
+}
+
+int launch_fit_from_sums(game_ctx *ctx, const double *sums, int P, long long N_total, float *out)
+{
+    fit_from_sums_kernel<<<(P + 255) / 256, 256, 0, ctx->stream>>>(sums, P, N_total, ctx->err, out);
+    GAME_LAUNCHED(ctx);
+    return GAME_OK;
+}
+
+int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, const DevState *state, double *sums)
 {
     dim3 block(32, 32);
     if (n_chunks >= 1024 && (P + 31) / 32 < 2 * ctx->sm_count) {
         dim3 grid((P + 31) / 32, FIN_SPLIT);
         finalize_split_kernel<<<grid, block, 0, ctx->stream>>>(ctx->partial, n_chunks, Ppad, P, ctx->fin2, state);
         GAME_LAUNCHED(ctx);
-        finalize_merge_kernel<<<(P + 255) / 256, 256, 0, ctx->stream>>>(ctx->fin2, Ppad, P, ctx->N, ctx->err, out, state);
+        finalize_merge_kernel<<<(P + 255) / 256, 256, 0, ctx->stream>>>(ctx->fin2, Ppad, P, ctx->N, ctx->err, out, sums, state);
         GAME_LAUNCHED(ctx);
         return GAME_OK;
     }
     finalize_kernel<<<(P + 31) / 32, block, 0, ctx->stream>>>(ctx->partial, n_chunks, Ppad, P, ctx->N, ctx->err, out,
-                                                               state);
+                                                               sums, state);
     GAME_LAUNCHED(ctx);
     return GAME_OK;
 }

@@ -299,6 +299,54 @@ int game_fitness_host(game_ctx *c, const float *pop, int P, float *out)
     return GAME_OK;
 }
 
+int game_fitness_sums(game_ctx *c, const float *pop, int P, double *sums)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!c->N) return fail(c, GAME_ERR_NOT_LOADED, "game_fitness_sums before game_load");
+    if (!pop) {                                   // the context's own population
+        if (!c->have_pop) return fail(c, GAME_ERR_NOT_LOADED, "game_fitness_sums: no population yet");
+        pop = c->pop; P = c->P;
+    }
+    if (!sums || P < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_fitness_sums: sums NULL or P < 1");
+    PartialInfo pi{};
+    int rc = run_fitness(c, pop, P, nullptr, nullptr, &pi);
+    if (rc) return rc;
+    return launch_finalize(c, pi.n_chunks, pi.Ppad, P, nullptr, nullptr, sums);
+}
+
+int game_advance(game_ctx *c, const double *sums, long long N_total, unsigned long long seed, const game_ga_params *gp,
+                 int apply_operators, game_result *res)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    int rc = validate_params(c, gp);
+    if (rc) return rc;
+    if (!c->have_pop || c->P != gp->P) return fail(c, GAME_ERR_NOT_LOADED, "game_advance: no population of params->P chromosomes installed");
+    if (!sums || N_total < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_advance: sums NULL or N_total < 1");
+    const int P = gp->P;
+    GAME_CUDA(c, cudaMemsetAsync(c->state, 0, sizeof(DevState), c->stream));
+    rc = launch_fit_from_sums(c, sums, P, N_total, c->fit);                                         // a5 tail
+    if (!rc) rc = launch_rank(c, c->fit, P, c->rank, c->order, c->state, gp->stop_error, true);    // a6, a7
+    if (rc) return rc;
+    if (apply_operators) {                                                                          // a8-a11
+        rc = launch_ga_step(c, gp, seed, (unsigned int)c->generation, c->order, c->fit, c->pop, c->pop_next, c->state, c->rw,
+                            c->rprefix);
+        if (rc) return rc;
+        float *tmp = c->pop; c->pop = c->pop_next; c->pop_next = tmp;
+    }
+    DevState h{};
+    GAME_CUDA(c, cudaMemcpyAsync(&h, c->state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->generation += h.gens_run;
+    c->have_fit = !apply_operators || h.gens_run == 0;      // fit/order describe the CURRENT population only if it did not move
+    if (res) {
+        res->generations_run = h.gens_run;
+        res->stopped_on_error = (h.stopped || h.stop_request) ? 1 : 0;
+        res->best_error = h.best_error;
+        res->best_index = h.best_index;
+    }
+    return GAME_OK;
+}
+
 int game_predict(game_ctx *c, const float *genes, float *z_out, float *y_out)
 {
     if (!c) return GAME_ERR_INVALID_ARG;

@@ -158,7 +158,8 @@ int launch_classify(game_ctx *ctx, const float *genes, float cut, long long *cou
 // fitness_fp32.cu
 size_t fitness_partial_floats(const game_ctx *ctx, int P);
 int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer);
-int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, const DevState *state);
+int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, const DevState *state, double *sums = nullptr);
+int launch_fit_from_sums(game_ctx *ctx, const double *sums, int P, long long N_total, float *out);
 // a5 tail + a6 + a7 in one go: final reduction of the slab sums, rank, stop test (single CTA when small)
 int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scratch, int *order, DevState *state,
                 float stop_error);

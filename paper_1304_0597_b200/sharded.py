@@ -1,0 +1,75 @@
+"""Pattern-sharded GA run over several GPUs, one process per GPU (the paper's future work (iii), L421).
+
+Rank r holds rows ``shard_rows(N, world, r)`` of X and the targets.  One generation is
+
+    sums_r = game_fitness_sums(population)          # a1-a5 on the local patterns, fp64 totals, no mean
+    sums   = all_reduce(sums_r, SUM)                # THE exchange step: P doubles (80 B ... 64 KB)
+    game_advance(sums, N_total, seed, params)       # mean, rank, stop test, GA operators -- replicated
+
+The all-reduce leaves the same bits on every rank and the operators draw counter-based random numbers, so every
+rank holds the same population afterwards without any further traffic.  This module is host logic only (which rows,
+which calls, the reduction); every step of the method runs in the library's kernels.  The evaluate / advance steps
+are passed in as callables so the same loop is exercised on CPU with ``gloo`` in the tests (tests/ may put the
+oracle behind them; the product path always puts a ``Game`` context there, see ``ShardedGame``).
+"""
+
+
+def shard_rows(N, world, rank):
+    """Contiguous, balanced row range [lo, hi) of rank `rank`: the first N % world ranks take one extra row."""
+    if not (0 <= rank < world) or N < 0:
+        raise ValueError("bad shard request")
+    base, extra = divmod(N, world)
+    lo = rank * base + min(rank, extra)
+    return lo, lo + base + (1 if rank < extra else 0)
+
+
+def all_reduce_sum(t, world):
+    """SUM-reduce a tensor of per-chromosome totals over the ranks, in place (no-op for one rank)."""
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return t
+
+
+def run_generations(evaluate, advance, world, generations, final_evaluation=True):
+    """The sharded loop.  evaluate() -> local fp64 totals (tensor of P); advance(totals, apply) -> result with
+    .generations_run / .stopped_on_error.  Returns (generations applied, last result)."""
+    done, res = 0, None
+    for _ in range(generations):
+        res = advance(all_reduce_sum(evaluate(), world), True)
+        done += res.generations_run
+        if res.stopped_on_error:
+            return done, res
+    if final_evaluation:          # the returned fitness belongs to the returned population (DESIGN G18)
+        res = advance(all_reduce_sum(evaluate(), world), False)
+    return done, res
+
+
+class ShardedGame:
+    """A ``Game`` context per rank holding that rank's rows; `evolve` runs the loop above over the process group."""
+
+    def __init__(self, game, N_total, world):
+        self.game, self.N_total, self.world = game, int(N_total), int(world)
+
+    @classmethod
+    def load(cls, family, degree, X, targets, world, rank, stream=None, configure=None):
+        """X, targets: the FULL host arrays (numpy); this rank uploads only its rows."""
+        import torch
+        from .binding import Game
+        lo, hi = shard_rows(X.shape[0], world, rank)
+        if hi <= lo:
+            raise ValueError("rank %d of %d would hold no pattern (N = %d)" % (rank, world, X.shape[0]))
+        g = Game(family, degree, X.shape[1], stream=stream)
+        if configure is not None:
+            configure(g)
+        g.load(torch.from_numpy(X[lo:hi]).cuda(), torch.from_numpy(targets[lo:hi]).cuda())
+        return cls(g, X.shape[0], world)
+
+    def evolve(self, generations, seed, params):
+        g = self.game
+        if g.generation() == 0 and not getattr(self, "_started", False):
+            g.evolve(0, seed, params)            # a12: every rank draws the same initial population (counter-based)
+        self._started = True
+        return run_generations(lambda: g.fitness_sums(None, params.P),
+                               lambda sums, apply: g.advance(sums, self.N_total, seed, params, apply),
+                               self.world, generations)

@@ -491,3 +491,67 @@ def test_trajectory_regenerated(orc):
         ctx.evolve(1, w.seed, gp)
         pop2, _, _ = ctx.get_population_host()
         assert np.array_equal(pop2.view(np.uint32), nxt.view(np.uint32))
+
+
+# ---- pattern-sharded evaluation (game_fitness_sums + game_advance) ------------------------------------
+@pytest.mark.parametrize("cfg_P", [(1, 20), (2, 300), (3, 512)])
+def test_sharded_one_rank_equals_evolve(orc, cfg_P):
+    """One shard holding every pattern: the sharded loop reproduces game_evolve bit for bit."""
+    from paper_1304_0597_b200 import sharded
+    cfg, P = cfg_P
+    w = wl.config(cfg).scaled(N=min(wl.config(cfg).N, 20000), P=P, generations=5)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    gp = g.ga_params(P=w.P)
+    ref = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    ref.evolve(w.generations, w.seed, gp)
+    pop_r, fit_r, ord_r = ref.get_population_host()
+
+    def configure(c):
+        c.set_activation(w.act)
+        c.set_error(w.err, w.R)
+    sg = sharded.ShardedGame.load(fam, d, X, t, 1, 0, configure=configure)
+    done, res = sg.evolve(w.generations, w.seed, gp)
+    assert done == w.generations and sg.game.generation() == w.generations
+    pop_s, fit_s, ord_s = sg.game.get_population_host()
+    assert np.array_equal(pop_s.view(np.uint32), pop_r.view(np.uint32))
+    assert np.array_equal(fit_s.view(np.uint32), fit_r.view(np.uint32)) and np.array_equal(ord_s, ord_r)
+    assert res.best_index == ord_r[0] and res.best_error == fit_r[ord_r[0]]
+
+
+@pytest.mark.parametrize("path", [g.GAME_PATH_FP32, g.GAME_PATH_TENSOR])
+@pytest.mark.parametrize("err,R", [(MSE, 0.0), (TMSE, 0.49), (RMSE, 0.0)])
+def test_sharded_three_shards_one_gpu(orc, path, err, R):
+    """Three uneven shards of the patterns, evaluated one after the other on this GPU (nothing waits on anything):
+    the summed totals give the full-data fitness within the path's tolerance, and all shards end every generation
+    with the same population, bit for bit -- which is also what the oracle's operators produce from that fitness."""
+    from paper_1304_0597_b200 import sharded
+    rng = np.random.default_rng(41)
+    fam, d, F, N, P, world = CHEB, 5, 16, 40000, 256, 3
+    X = rng.uniform(-1, 1, (N, F)).astype(np.float32)
+    t = rng.integers(0, 2, N).astype(np.float32)
+    seed = 77
+    gp = g.ga_params(P=P)
+    gpo = orc.GaParams(P=P, tournament_size=3, elitism=2, elite_mode=0, selection=0, init_mode=1, p_crossover=0.9,
+                       p_mutation=0.05, stop_error=-1.0)
+
+    def configure(c):
+        c.set_error(err, R)
+        c.set_path(path)
+    shards = [sharded.ShardedGame.load(fam, d, X, t, world, r, configure=configure) for r in range(world)]
+    for s in shards:
+        s.game.evolve(0, seed, gp)                      # identical initial populations (counter-based)
+    for gen in range(3):
+        sums = sum(s.game.fitness_sums(None, P) for s in shards)          # what the all-reduce would deliver
+        pop0 = shards[0].game.get_population_host(want_fit=False)[0]
+        fit = (sums.cpu().numpy() / N)
+        if err == RMSE:
+            fit = np.sqrt(fit)
+        check_fitness(orc, fit, fam, d, X, t, pop0, SIGMOID, err, R, path, "gen %d" % gen)
+        results = [s.game.advance(sums, N, seed, gp, True) for s in shards]
+        assert all(r.generations_run == 1 and r.best_index == results[0].best_index for r in results)
+        fit32 = fit.astype(np.float32)
+        nxt = orc.ga_step(gpo, seed, gen, orc.rank(fit32), fit32, pop0)
+        for s in shards:
+            p = s.game.get_population_host(want_fit=False)[0]
+            assert np.array_equal(p.view(np.uint32), nxt.view(np.uint32))
