@@ -44,7 +44,7 @@ enum { GAME_INIT_UNIFORM_PM1 = 0, GAME_INIT_NORMAL_PM1 = 1, GAME_INIT_UNIFORM_01
 enum { GAME_ELITE_COPIES_OF_BEST = 0, GAME_ELITE_TOP_E = 1 };      /* L148; DESIGN G17 */
 /* Fitness kernel choice.  FP32: FFMA contraction, |rel err| <= 1e-5 class.  TENSOR: tcgen05 fp16-input /
  * fp32-accumulate MMA (same 11-bit significand as TF32), 1e-3 class.  AUTO picks by problem shape. */
-enum { GAME_PATH_AUTO = 0, GAME_PATH_FP32 = 1, GAME_PATH_TENSOR = 2 };
+enum { GAME_PATH_AUTO = 0, GAME_PATH_FP32 = 1, GAME_PATH_TENSOR = 2, GAME_PATH_TENSOR_SPLIT = 3 };
 enum { GAME_EXPAND_AUTO = 0, GAME_EXPAND_MATERIALIZED = 1, GAME_EXPAND_REGENERATED = 2 };
 
 /* GA parameters (L275-L291).  Probabilities are per parent pair (crossover, DESIGN G15) and per gene

@@ -19,7 +19,7 @@ GAME_ERR_MSE, GAME_ERR_TMSE, GAME_ERR_RMSE = 0, 1, 2
 GAME_SEL_TOURNAMENT, GAME_SEL_ROULETTE = 0, 1
 GAME_INIT_UNIFORM_PM1, GAME_INIT_NORMAL_PM1, GAME_INIT_UNIFORM_01 = 0, 1, 2
 GAME_ELITE_COPIES_OF_BEST, GAME_ELITE_TOP_E = 0, 1
-GAME_PATH_AUTO, GAME_PATH_FP32, GAME_PATH_TENSOR = 0, 1, 2
+GAME_PATH_AUTO, GAME_PATH_FP32, GAME_PATH_TENSOR, GAME_PATH_TENSOR_SPLIT = 0, 1, 2, 3
 GAME_EXPAND_AUTO, GAME_EXPAND_MATERIALIZED, GAME_EXPAND_REGENERATED = 0, 1, 2
 ERROR_NAMES = {1: "INVALID_ARG", 2: "NOT_LOADED", 3: "ALLOC", 4: "CUDA", 5: "UNSUPPORTED", 6: "NONFINITE_INPUT"}
 

@@ -34,9 +34,12 @@ int launch_check_finite(game_ctx *ctx, const float *X, long long nX, const float
 
 // One thread per (feature i, pattern n); n is the fastest thread index so the term-major stores
 // ET[k][n] are coalesced.  Term index k = i*B + m, block order [1, cos 1..d, sin 1..d] / [T_0..T_d].
+// split != 0 (TENSOR_SPLIT path): E is written as three fp16 k-ranges [hi | hi | lo] of ld/3 positions each, hi = fp16(E),
+// lo = fp16(E - hi), so that against genes laid out [hi | lo | hi] one fp16 contraction over 3K terms yields
+// E_hi C_hi + E_hi C_lo + E_lo C_hi = E C to ~2^-22 relative.
 template <typename OutT, bool PATTERN_MAJOR>
 __global__ void expand_kernel(const float *__restrict__ X, long long N, int F, int family, int d,
-                              OutT *__restrict__ E, long long ld, float *maxabs)
+                              OutT *__restrict__ E, long long ld, float *maxabs, int split = 0)
 {
     long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     int i = blockIdx.y;
@@ -52,7 +55,14 @@ __global__ void expand_kernel(const float *__restrict__ X, long long N, int F, i
                 // TENSOR path: permuted term order (tc_position), tile-blocked [n/256][k/64][256][64] so that every
                 // TMA box is one contiguous 32 KB run
                 const long long k = tc_position(family, d, i, m);
-                E[(((n >> 8) * (ld >> 6) + (k >> 6)) << 14) + ((n & 255) << 6) + (k & 63)] = (OutT)f;
+                auto at = [&](long long kk) -> OutT & { return E[(((n >> 8) * (ld >> 6) + (kk >> 6)) << 14) + ((n & 255) << 6) + (kk & 63)]; };
+                if (!split) {
+                    at(k) = (OutT)f;
+                } else {
+                    const long long third = ld / 3;
+                    const OutT hi = (OutT)f;
+                    at(k) = hi; at(third + k) = hi; at(2 * third + k) = (OutT)(f - (float)hi);
+                }
             } else {
                 E[(long long)(k0 + m) * ld + n] = (OutT)f;
             }
@@ -137,6 +147,15 @@ int launch_expand_fp32(game_ctx *ctx)
     dim3 grid((unsigned)((ctx->N + 255) / 256), (unsigned)ctx->F);
     expand_kernel<float, false><<<grid, 256, 0, ctx->stream>>>(ctx->X, ctx->N, ctx->F, ctx->family, ctx->degree,
                                                                 ctx->ET, ctx->Npad, nullptr);
+    GAME_LAUNCHED(ctx);
+    return GAME_OK;
+}
+
+int launch_expand_split(game_ctx *ctx)
+{
+    dim3 grid((unsigned)((ctx->N + 255) / 256), (unsigned)ctx->F);
+    expand_kernel<__half, true><<<grid, 256, 0, ctx->stream>>>(ctx->X, ctx->N, ctx->F, ctx->family, ctx->degree,
+                                                                ctx->E16s, 3LL * ctx->Kpad, nullptr, 1);
     GAME_LAUNCHED(ctx);
     return GAME_OK;
 }

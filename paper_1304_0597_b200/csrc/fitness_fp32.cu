@@ -29,6 +29,8 @@ fitness_fp32_kernel(const float *__restrict__ ET, long long Npad, long long N, i
                     int n_slabs, int slabs_per_cta, FitnessCfg cfg, float *__restrict__ partial, int Ppad,
                     const DevState *state)
 {
+    pdl_wait();
+    pdl_trigger();
     if (state && state->stopped) return;
     __shared__ __align__(16) float As[BK][BN];        // E chunk: [k][n]
     __shared__ __align__(16) float Bs[BK][BP + 4];    // C chunk: [k][p], padded against store conflicts
@@ -142,6 +144,8 @@ __global__ void __launch_bounds__(256, 1)
 post_small_kernel(const float *__restrict__ partial, int n_chunks, int Ppad, int P, long long N, int err,
                   float *__restrict__ fit, int *__restrict__ order, DevState *state, float stop_error)
 {
+    pdl_wait();
+    pdl_trigger();
     if (state->stopped) return;            // single CTA: the flag this kernel may set is stop_request, read by later launches
     __shared__ unsigned long long keys[256];
     __shared__ float part[POST_SMALL_FLOATS];
@@ -183,9 +187,9 @@ int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scra
                 float stop_error)
 {
     if (P <= 256 && (long long)pi.n_chunks * P <= POST_SMALL_FLOATS) {
-        post_small_kernel<<<1, 256, 0, ctx->stream>>>(ctx->partial, pi.n_chunks, pi.Ppad, P, ctx->N, ctx->err, fit, order,
-                                                           state, stop_error);
-        GAME_LAUNCHED(ctx);
+        GAME_CUDA(ctx, launch_pdl(post_small_kernel, dim3(1), dim3(256), 0, ctx->stream, ctx->partial, pi.n_chunks, pi.Ppad, P, ctx->N,
+                                  ctx->err, fit, order, state, stop_error));
+        ++ctx->launches;
         return GAME_OK;
     }
     int rc = launch_finalize(ctx, pi.n_chunks, pi.Ppad, P, fit, state);
@@ -199,6 +203,8 @@ int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scra
 __global__ void finalize_kernel(const float *__restrict__ partial, int n_chunks, int Ppad, int P, long long N,
                                 int err, float *__restrict__ out, double *__restrict__ sums, const DevState *state)
 {
+    pdl_wait();
+    pdl_trigger();
     if (state && state->stopped) return;
     __shared__ double red[32][33];
     int c = threadIdx.x, r = threadIdx.y;
@@ -224,6 +230,8 @@ __global__ void finalize_kernel(const float *__restrict__ partial, int n_chunks,
 __global__ void finalize_split_kernel(const float *__restrict__ partial, int n_chunks, int Ppad, int P,
                                       double *__restrict__ fin2, const DevState *state)
 {
+    pdl_wait();
+    pdl_trigger();
     if (state && state->stopped) return;
     __shared__ double red[32][33];
     const int c = threadIdx.x, r = threadIdx.y;
@@ -245,6 +253,8 @@ __global__ void finalize_split_kernel(const float *__restrict__ partial, int n_c
 __global__ void finalize_merge_kernel(const double *__restrict__ fin2, int Ppad, int P, long long N, int err,
                                       float *__restrict__ out, double *__restrict__ sums, const DevState *state)
 {
+    pdl_wait();
+    pdl_trigger();
     if (state && state->stopped) return;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P) return;
@@ -272,6 +282,8 @@ fitness_small_kernel(const float *__restrict__ ET, long long Npad, long long N, 
                      int P, const float *__restrict__ tgt, int n_slabs, int spc, int kcap, FitnessCfg cfg,
                      float *__restrict__ partial, int Ppad, const DevState *state)
 {
+    pdl_wait();
+    pdl_trigger();
     if (state && state->stopped) return;
     extern __shared__ __align__(16) float small_smem[];
     float (*Es)[SLAB] = reinterpret_cast<float (*)[SLAB]>(small_smem);                       // [k][n], as in ET
@@ -390,15 +402,16 @@ int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, co
     dim3 block(32, 32);
     if (n_chunks >= 1024 && (P + 31) / 32 < 2 * ctx->sm_count) {
         dim3 grid((P + 31) / 32, FIN_SPLIT);
-        finalize_split_kernel<<<grid, block, 0, ctx->stream>>>(ctx->partial, n_chunks, Ppad, P, ctx->fin2, state);
-        GAME_LAUNCHED(ctx);
-        finalize_merge_kernel<<<(P + 255) / 256, 256, 0, ctx->stream>>>(ctx->fin2, Ppad, P, ctx->N, ctx->err, out, sums, state);
-        GAME_LAUNCHED(ctx);
+        GAME_CUDA(ctx, launch_pdl(finalize_split_kernel, grid, block, 0, ctx->stream, ctx->partial, n_chunks, Ppad, P, ctx->fin2, state));
+        ++ctx->launches;
+        GAME_CUDA(ctx, launch_pdl(finalize_merge_kernel, dim3((P + 255) / 256), dim3(256), 0, ctx->stream, ctx->fin2, Ppad, P, ctx->N,
+                                  ctx->err, out, sums, state));
+        ++ctx->launches;
         return GAME_OK;
     }
-    finalize_kernel<<<(P + 31) / 32, block, 0, ctx->stream>>>(ctx->partial, n_chunks, Ppad, P, ctx->N, ctx->err, out,
-                                                               sums, state);
-    GAME_LAUNCHED(ctx);
+    GAME_CUDA(ctx, launch_pdl(finalize_kernel, dim3((P + 31) / 32), block, 0, ctx->stream, ctx->partial, n_chunks, Ppad, P, ctx->N,
+                              ctx->err, out, sums, state));
+    ++ctx->launches;
     return GAME_OK;
 }
 
@@ -422,10 +435,10 @@ int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, cons
         }
         {
             KernelTimer timer(ctx);
-            fitness_small_kernel<<<grid, 128, smem, ctx->stream>>>(ctx->ET, ctx->Npad, ctx->N, ctx->K, pop, P, ctx->t,
-                                                                   ctx->n_slabs, spc, kcap, cfg, ctx->partial, Ppad, state);
+            GAME_CUDA(ctx, launch_pdl(fitness_small_kernel, grid, dim3(128), (size_t)smem, ctx->stream, ctx->ET, ctx->Npad, ctx->N, ctx->K,
+                                      pop, P, ctx->t, ctx->n_slabs, spc, kcap, cfg, ctx->partial, Ppad, state));
         }
-        GAME_LAUNCHED(ctx);
+        ++ctx->launches;
         if (defer) { defer->n_chunks = n_chunks; defer->Ppad = Ppad; return GAME_OK; }
         return launch_finalize(ctx, n_chunks, Ppad, P, out, state);
     }
@@ -434,10 +447,10 @@ int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, cons
     dim3 grid((unsigned)n_chunks, (unsigned)((P + BP - 1) / BP));
     {
         KernelTimer timer(ctx);
-        fitness_fp32_kernel<<<grid, NT, 0, ctx->stream>>>(ctx->ET, ctx->Npad, ctx->N, ctx->K, pop, P, ctx->t,
-                                                          ctx->n_slabs, spc, cfg, ctx->partial, Ppad, state);
+        GAME_CUDA(ctx, launch_pdl(fitness_fp32_kernel, grid, dim3(NT), 0, ctx->stream, ctx->ET, ctx->Npad, ctx->N, ctx->K, pop, P, ctx->t,
+                                  ctx->n_slabs, spc, cfg, ctx->partial, Ppad, state));
     }
-    GAME_LAUNCHED(ctx);
+    ++ctx->launches;
     if (defer) { defer->n_chunks = n_chunks; defer->Ppad = Ppad; return GAME_OK; }
     return launch_finalize(ctx, n_chunks, Ppad, P, out, state);
 }

@@ -435,8 +435,6 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     static_assert(SRC == SRC_TMA || CG == 2, "the generator variant runs as CTA pairs");
     constexpr int NSTAGES = SRC == SRC_GEN ? GEN_STAGES : C::STAGES;
     constexpr int WARP_GEN0 = WARP_EPI0 + EW;
-    if (state && state->stopped) return;          // uniform across the grid: nobody has touched a barrier yet
-
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t *gbase = smem_raw + (base - smem_u32(smem_raw));
@@ -476,7 +474,13 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_g;
 
-    if (warp == WARP_TMA) {
+    // Everything above touched only this CTA's own shared / tensor memory, so under programmatic dependent launch it
+    // overlaps the tail of the previous kernel; from here on the kernel reads what its predecessors wrote.
+    pdl_wait();
+    const bool stopped = state && state->stopped;      // uniform across the grid: the loop has stopped, nothing to do
+
+    if (stopped) {
+    } else if (warp == WARP_TMA) {
         // ===== TMA producer =====
         if (lane == 0 && SRC == SRC_GEN) {
             // the population tile is loaded ONCE and stays: block kb of this CTA's 128 chromosomes at base + kb * A_BYTES
@@ -645,6 +649,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     }
 
     // teardown: everyone done with TMEM before it is released
+    pdl_trigger();
     tc_fence_before();
     if (CG == 2) { asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory"); }
     else __syncthreads();
@@ -653,9 +658,12 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
 
 // pop fp32 [P][K] -> C16 fp16 [Ppad][Kpad] (round to nearest even, clamped to the finite fp16 range), times `scale`
 // (1 or 0.5: exact, see the epilogue modes)
+// split != 0 (TENSOR_SPLIT path): rows of 3 Kpad positions [hi | lo | hi], hi = fp16(c), lo = fp16(c - hi); see expand_kernel
 __global__ void pop_to_f16_kernel(const float *__restrict__ pop, int P, int K, int Kpad, int family, int d, float scale,
-                                  __half *__restrict__ C16, const DevState *state)
+                                  __half *__restrict__ C16, const DevState *state, int split)
 {
+    pdl_wait();
+    pdl_trigger();
     if (state && state->stopped) return;
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= (long long)P * K) return;
@@ -666,7 +674,13 @@ __global__ void pop_to_f16_kernel(const float *__restrict__ pop, int P, int K, i
         const int B = tc_terms_per_feature(family, d);
         pos = tc_position(family, d, k / B, k % B);
     }
-    C16[(long long)p * Kpad + pos] = __float2half_rn(v);
+    if (!split) {
+        C16[(long long)p * Kpad + pos] = __float2half_rn(v);
+    } else {
+        __half *row = C16 + (long long)p * 3 * Kpad;
+        const __half hi = __float2half_rn(v);
+        row[pos] = hi; row[Kpad + pos] = __float2half_rn(v - __half2float(hi)); row[2 * Kpad + pos] = hi;
+    }
 }
 
 // ---- host side ------------------------------------------------------------------------------------------
@@ -708,15 +722,16 @@ bool tensor_path_built() { return true; }
 // measured on B200 they win for deep contractions over wide populations (config 5: 1500 vs 1442 TFLOP/s)
 // and lose where the pair leaves too few chromosome blocks (config 4) or K is shallow (config 3).
 // GAME_TC_CTA_GROUP=1|2 overrides, for measurement.
-static int cta_group(const game_ctx *ctx, int Ppad)
+static int cta_group(const game_ctx *ctx, int Ppad, int Kp)
 {
+    (void)ctx;
     static int forced = -1;
     if (forced < 0) {
         const char *e = getenv("GAME_TC_CTA_GROUP");
         forced = e ? (e[0] == '2' ? 2 : 1) : 0;
     }
     if (forced) return forced;
-    return (ctx->Kpad >= 512 && Ppad >= 1024) ? 2 : 1;
+    return (Kp >= 512 && Ppad >= 1024) ? 2 : 1;
 }
 
 // Epilogue warps per CTA: 8.  16 (four per scheduler, 96 registers each) were measured on B200 and lose everywhere
@@ -757,12 +772,31 @@ int tensor_prepare(game_ctx *ctx)
     return GAME_OK;
 }
 
+// TENSOR_SPLIT path: the [hi | hi | lo] expansion and its tensor maps, built on the first call that needs them
+int tensor_prepare_split(game_ctx *ctx)
+{
+    if (ctx->E16s) return GAME_OK;
+    const size_t n16 = (size_t)ctx->Npad256 * 3 * ctx->Kpad;
+    GAME_CUDA(ctx, cudaMalloc(&ctx->E16s, n16 * sizeof(__half)));
+    GAME_CUDA(ctx, cudaMemsetAsync(ctx->E16s, 0, n16 * sizeof(__half), ctx->stream));
+    int rc = launch_expand_split(ctx);
+    if (rc) return rc;
+    if (!ctx->tmap_Es) ctx->tmap_Es = aligned_alloc(64, 2 * sizeof(CUtensorMap));
+    if (!ctx->tmap_Es) return fail(ctx, GAME_ERR_ALLOC, "tensor map allocation failed");
+    for (int cg = 1; cg <= 2; ++cg) {
+        rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_Es + (cg - 1), ctx->E16s, ctx->Npad256 * (3 * ctx->Kpad / BKB), BKB, BN / cg);
+        if (rc) return rc;
+    }
+    return GAME_OK;
+}
+
 template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY>
-static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, const DevState *state)
+static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, const DevState *state, bool split = false)
 {
     using C = Cfg<CG>;
     auto kern = fitness_tc_kernel<CG, ACT, TMSE, EW, SRC, FAMILY>;
-    const int k_blocks = ctx->Kpad / BKB;
+    const int k_blocks = (split ? 3 : 1) * ctx->Kpad / BKB;
+    const CUtensorMap *maps_E = (const CUtensorMap *)(split ? ctx->tmap_Es : ctx->tmap_E);
     const int smem = SRC == SRC_GEN ? k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES : C::SMEM;
     static int attr_smem = 0;
     if (smem > attr_smem) {
@@ -777,12 +811,14 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     cfg.blockDim = dim3(64 + 32 * EW + (SRC == SRC_GEN ? 32 * GEN_WARPS : 0));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = ctx->stream;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl_enabled() ? 2 : 1;
     KernelTimer timer(ctx);
-    GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, ((const CUtensorMap *)ctx->tmap_E)[CG - 1], n_tiles,
+    GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, maps_E[CG - 1], n_tiles,
                                       m_blocks, k_blocks, ctx->N, (const float *)ctx->t, ctx->R, ctx->partial, Ppad, state,
                                       (const float *)ctx->X, ctx->F, ctx->degree));
     return GAME_OK;
@@ -807,27 +843,33 @@ int tensor_expansion(const game_ctx *ctx, int P)
     return GAME_EXPAND_MATERIALIZED;
 }
 
-int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer)
+int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer, bool split)
 {
     const int Ppad = ((P + 255) / 256) * 256;
-    const int expansion = tensor_expansion(ctx, P);
+    if (split) {
+        int rcs = tensor_prepare_split(ctx);
+        if (rcs) return rcs;
+    }
+    const int Kp = (split ? 3 : 1) * ctx->Kpad;              // contraction depth the kernel sees
+    const int expansion = split ? GAME_EXPAND_MATERIALIZED : tensor_expansion(ctx, P);
     if (expansion < 0) return fail(ctx, GAME_ERR_UNSUPPORTED, "regenerated expansion unavailable for this shape (needs P <= 256, K <= 576 after padding, trig: max|X| <= pi)");
     const int src = expansion == GAME_EXPAND_REGENERATED ? SRC_GEN : SRC_TMA;
-    const int cg = src == SRC_GEN ? 2 : cta_group(ctx, Ppad);
+    const int cg = src == SRC_GEN ? 2 : cta_group(ctx, Ppad, Kp);
     const int n_tiles = (int)(ctx->Npad256 / BN);
     const int m_blocks = Ppad / (BM * cg);
     long long n = (long long)P * ctx->K;
     const bool tmse = ctx->err == GAME_ERR_TMSE;
-    const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : sigmoid_mode();
+    // the split path is the 1e-5 tolerance class: its logistic is the ex2 + rcp form (2^-22), not tanh.approx (2^-11)
+    const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : (split ? MODE_SIG_EXACT : sigmoid_mode());
     const int ew = epilogue_warps(ctx);
-    pop_to_f16_kernel<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(pop, P, ctx->K, ctx->Kpad, ctx->family, ctx->degree,
-                                                                            mode == MODE_SIG_TANH32 ? 0.5f : 1.0f, ctx->C16, state);
-    GAME_LAUNCHED(ctx);
-    int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_C, ctx->C16, Ppad, ctx->Kpad, BM);
+    GAME_CUDA(ctx, launch_pdl(pop_to_f16_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, ctx->stream, pop, P, ctx->K, ctx->Kpad,
+                              ctx->family, ctx->degree, mode == MODE_SIG_TANH32 ? 0.5f : 1.0f, split ? ctx->C16s : ctx->C16, state, split ? 1 : 0));
+    ++ctx->launches;
+    int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_C, split ? ctx->C16s : ctx->C16, Ppad, Kp, BM);
     if (rc) return rc;
 #define GAME_TC_EW(CGV, M, T)                                                                              \
-    rc = ew == 16 ? launch_variant<CGV, M, T, 16, SRC_TMA, GAME_TRIG>(ctx, n_tiles, m_blocks, Ppad, state)     \
-                  : launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG>(ctx, n_tiles, m_blocks, Ppad, state)
+    rc = ew == 16 ? launch_variant<CGV, M, T, 16, SRC_TMA, GAME_TRIG>(ctx, n_tiles, m_blocks, Ppad, state, split)     \
+                  : launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG>(ctx, n_tiles, m_blocks, Ppad, state, split)
 #define GAME_TC_GEN(M, T)                                                                                  \
     rc = ctx->family == GAME_TRIG ? launch_variant<2, M, T, 8, SRC_GEN, GAME_TRIG>(ctx, n_tiles, 1, Ppad, state) \
                                   : launch_variant<2, M, T, 8, SRC_GEN, GAME_CHEB>(ctx, n_tiles, 1, Ppad, state)

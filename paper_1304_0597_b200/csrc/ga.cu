@@ -85,6 +85,8 @@ constexpr int RANK_T = 128, RANK_Q = 256;   // chromosomes per CTA x keys per CT
 
 __global__ void rank_count_kernel(const float *__restrict__ fit, int P, int *__restrict__ rank, const DevState *state)
 {
+    pdl_wait();
+    pdl_trigger();
     if (state && state->stopped) return;
     __shared__ unsigned long long keys[RANK_Q];
     int p = blockIdx.x * RANK_T + threadIdx.x;
@@ -107,6 +109,8 @@ __global__ void rank_count_kernel(const float *__restrict__ fit, int P, int *__r
 __global__ void rank_scatter_kernel(const float *__restrict__ fit, int P, int *__restrict__ rank,
                                     int *__restrict__ order, DevState *state, float stop_error, int update_state)
 {
+    pdl_wait();
+    pdl_trigger();
     if (state && state->stopped) return;
     int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P) return;
@@ -126,11 +130,11 @@ int launch_rank(game_ctx *ctx, const float *fit, int P, int *rank_scratch, int *
                 float stop_error, bool update_state)
 {
     dim3 grid((P + RANK_T - 1) / RANK_T, (P + RANK_Q - 1) / RANK_Q);
-    rank_count_kernel<<<grid, RANK_T, 0, ctx->stream>>>(fit, P, rank_scratch, state);
-    GAME_LAUNCHED(ctx);
-    rank_scatter_kernel<<<(P + 255) / 256, 256, 0, ctx->stream>>>(fit, P, rank_scratch, order, state, stop_error,
-                                                                  update_state ? 1 : 0);
-    GAME_LAUNCHED(ctx);
+    GAME_CUDA(ctx, launch_pdl(rank_count_kernel, grid, dim3(RANK_T), 0, ctx->stream, fit, P, rank_scratch, state));
+    ++ctx->launches;
+    GAME_CUDA(ctx, launch_pdl(rank_scatter_kernel, dim3((P + 255) / 256), dim3(256), 0, ctx->stream, fit, P, rank_scratch, order, state,
+                              stop_error, update_state ? 1 : 0));
+    ++ctx->launches;
     return GAME_OK;
 }
 
@@ -139,6 +143,8 @@ __global__ void roulette_kernel(const float *__restrict__ fit, const int *__rest
                                 unsigned int *__restrict__ wts, unsigned long long *__restrict__ prefix,
                                 const DevState *state)
 {
+    pdl_wait();
+    pdl_trigger();
     if (state && state->stopped) return;
     __shared__ float smax[32], smin[32];
     __shared__ int scnt[32];
@@ -223,6 +229,8 @@ __global__ void ga_step_kernel(StepArgs a, const int *__restrict__ order, const 
                                DevState *state, int *dbg)
 {
     const int K = a.K;
+    pdl_wait();
+    pdl_trigger();
     if (state) a.gen += (uint32_t)(state->evals_done - 1);     // written by the rank step of THIS generation, stable here
     const bool stopped = state && (state->stopped | state->stop_request);
     if (stopped && threadIdx.x == 0) state->stopped = 1;      // promote (every CTA writes the same value)
@@ -279,12 +287,13 @@ int launch_ga_step(game_ctx *ctx, const game_ga_params *gp, unsigned long long s
     a.pc = host_thr(gp->p_crossover); a.pm = host_thr(gp->p_mutation);
     a.seed = seed; a.gen = gen_base;
     if (gp->selection == GAME_SEL_ROULETTE) {
-        roulette_kernel<<<1, 1024, 0, ctx->stream>>>(fit, order, gp->P, rw, rprefix, state);
-        GAME_LAUNCHED(ctx);
+        GAME_CUDA(ctx, launch_pdl(roulette_kernel, dim3(1), dim3(1024), 0, ctx->stream, fit, order, gp->P, rw, rprefix, state));
+        ++ctx->launches;
     }
     int threads = ctx->K >= 512 ? 256 : ctx->K >= 128 ? 128 : 64;
-    ga_step_kernel<<<a.e + a.npairs, threads, 0, ctx->stream>>>(a, order, pop, next, rprefix, state, nullptr);
-    GAME_LAUNCHED(ctx);
+    GAME_CUDA(ctx, launch_pdl(ga_step_kernel, dim3(a.e + a.npairs), dim3(threads), 0, ctx->stream, a, order, pop, next, rprefix, state,
+                              (int *)nullptr));
+    ++ctx->launches;
     return GAME_OK;
 }
 

@@ -1,6 +1,7 @@
 // The C ABI of libgame_b200 (include/game.h): context management, argument validation and the
 // host-side sequencing of the kernels.  No arithmetic of the method happens on the host.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -12,6 +13,16 @@ int fail(game_ctx *ctx, int code, const char *what)
 {
     if (ctx) ctx->msg = what;
     return code;
+}
+
+bool pdl_enabled()
+{
+    static int on = -1;
+    if (on < 0) {
+        const char *e = getenv("GAME_PDL");
+        on = (e && e[0] == '0') ? 0 : 1;
+    }
+    return on != 0;
 }
 
 int cuda_fail(game_ctx *ctx, cudaError_t e, const char *where)
@@ -31,7 +42,7 @@ static void dfree(T *&p)
 
 static void free_dataset(game_ctx *c)
 {
-    dfree(c->X); dfree(c->t); dfree(c->ET); dfree(c->E16);
+    dfree(c->X); dfree(c->t); dfree(c->ET); dfree(c->E16); dfree(c->E16s);
     c->N = 0; c->tensor_ok = false;
 }
 
@@ -80,6 +91,12 @@ static int ensure_scratch(game_ctx *c, int P)
         GAME_CUDA(c, cudaMemsetAsync(c->C16, 0, need16 * sizeof(__half), c->stream));
         c->c16_cap = need16;
     }
+    if (c->tensor_ok && c->path != GAME_PATH_FP32 && c->path != GAME_PATH_TENSOR && 3 * need16 > c->c16s_cap) {   // AUTO or SPLIT may need it
+        dfree(c->C16s);
+        GAME_CUDA(c, cudaMalloc(&c->C16s, 3 * need16 * sizeof(__half)));
+        GAME_CUDA(c, cudaMemsetAsync(c->C16s, 0, 3 * need16 * sizeof(__half), c->stream));
+        c->c16s_cap = 3 * need16;
+    }
     return GAME_OK;
 }
 
@@ -88,7 +105,14 @@ static int resolve_path(const game_ctx *c, int P)
     bool can_tensor = tensor_path_built() && c->tensor_ok;
     if (c->path == GAME_PATH_FP32) return GAME_PATH_FP32;
     if (c->path == GAME_PATH_TENSOR) return can_tensor ? GAME_PATH_TENSOR : -1;
-    return (can_tensor && P >= 256 && c->N >= 16384) ? GAME_PATH_TENSOR : GAME_PATH_FP32;
+    const bool can_split = can_tensor && tc_permuted(c->family);
+    if (c->path == GAME_PATH_TENSOR_SPLIT) return can_split ? GAME_PATH_TENSOR_SPLIT : -1;
+    // AUTO: wide populations go to the tensor cores -- large datasets in the 1e-3 class (one fp16 pass), small ones
+    // (where the whole contraction is a few microseconds either way) in the 1e-5 class via the split-fp16 path, which
+    // beats the FFMA kernel there (config 2: DESIGN.md section 7); everything else stays on the FFMA kernels
+    if (can_tensor && P >= 256 && c->N >= 16384) return GAME_PATH_TENSOR;
+    if (can_split && P >= 256) return GAME_PATH_TENSOR_SPLIT;
+    return GAME_PATH_FP32;
 }
 
 static int run_fitness(game_ctx *c, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer = nullptr)
@@ -97,8 +121,9 @@ static int run_fitness(game_ctx *c, const float *pop, int P, float *out, const D
     if (rc) return rc;
     int path = resolve_path(c, P);
     if (path < 0) return fail(c, GAME_ERR_UNSUPPORTED, "tensor path unavailable for this dataset (not built, or |E| exceeds fp16 range)");
-    return path == GAME_PATH_TENSOR ? launch_fitness_tensor(c, pop, P, out, state, defer)
-                                    : launch_fitness_fp32(c, pop, P, out, state, defer);
+    if (path == GAME_PATH_TENSOR) return launch_fitness_tensor(c, pop, P, out, state, defer, false);
+    if (path == GAME_PATH_TENSOR_SPLIT) return launch_fitness_tensor(c, pop, P, out, state, defer, true);
+    return launch_fitness_fp32(c, pop, P, out, state, defer);
 }
 
 static int validate_params(game_ctx *c, const game_ga_params *g)
@@ -212,8 +237,8 @@ void game_destroy(game_ctx *c)
     cudaStreamSynchronize(c->stream);
     free_dataset(c);
     free_population(c);
-    dfree(c->partial); dfree(c->fin2); dfree(c->C16); dfree(c->stage_pop); dfree(c->stage_fit); dfree(c->state);
-    free(c->tmap_E); free(c->tmap_C);
+    dfree(c->partial); dfree(c->fin2); dfree(c->C16); dfree(c->C16s); dfree(c->stage_pop); dfree(c->stage_fit); dfree(c->state);
+    free(c->tmap_E); free(c->tmap_C); free(c->tmap_Es);
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     delete c;
 }
@@ -252,7 +277,7 @@ int game_set_error(game_ctx *c, int err, float R)
 int game_set_path(game_ctx *c, int path)
 {
     if (!c) return GAME_ERR_INVALID_ARG;
-    if (path < GAME_PATH_AUTO || path > GAME_PATH_TENSOR) return fail(c, GAME_ERR_INVALID_ARG, "bad path");
+    if (path < GAME_PATH_AUTO || path > GAME_PATH_TENSOR_SPLIT) return fail(c, GAME_ERR_INVALID_ARG, "bad path");
     c->path = path;
     return GAME_OK;
 }

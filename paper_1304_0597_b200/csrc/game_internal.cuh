@@ -62,6 +62,14 @@ __host__ __device__ inline int tc_position(int family, int d, int i, int m)
     return ((i >> 3) * T + tau) * 8 + (i & 7);
 }
 
+// ---- programmatic dependent launch (PDL) -----------------------------------------------------------------------
+// The kernels of one generation form a chain of small dependent launches; with the programmatic-stream-serialization
+// attribute the next kernel's CTAs are scheduled while the previous kernel drains, and wait (griddepcontrol.wait) only
+// where they first touch what the predecessor wrote.  pdl_wait() returns once every prerequisite grid has COMPLETED and
+// its writes are visible, so it is always safe; pdl_trigger() lets the dependents be scheduled early.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 struct FitnessCfg {
     int act, err;
     float R;
@@ -83,6 +91,7 @@ struct game_ctx {
     float *t = nullptr;        // Npad, zero padded
     float *ET = nullptr;       // K x Npad fp32, term-major (FP32 path), zero padded
     __half *E16 = nullptr;     // Npad256 x Kpad fp16, pattern-major (TENSOR path), zero padded
+    __half *E16s = nullptr;    // Npad256 x 3 Kpad fp16: [hi | hi | lo] halves of E (TENSOR_SPLIT path), built on first use
     long long Npad256 = 0;
     int Kpad = 0;              // K rounded up to TC_KBLK
     bool tensor_ok = false;    // E16 built and all |E| representable
@@ -107,9 +116,12 @@ struct game_ctx {
     size_t fin2_cap = 0;
     __half *C16 = nullptr;     // Ppad128 x Kpad fp16 population copy (TENSOR path)
     size_t c16_cap = 0;
+    __half *C16s = nullptr;    // Ppad x 3 Kpad fp16 [hi | lo | hi] population copy (TENSOR_SPLIT path); padding stays zero
+    size_t c16s_cap = 0;
     float *stage_pop = nullptr, *stage_fit = nullptr;   // device staging for *_host calls
     size_t stage_cap = 0;
     void *tmap_E = nullptr, *tmap_C = nullptr;          // host copies of CUtensorMap (TENSOR path)
+    void *tmap_Es = nullptr;                            // the same for E16s
 
     long long launches = 0;
     bool timing = false;
@@ -148,10 +160,26 @@ struct KernelTimer {
     ~KernelTimer() { if (c->timing) cudaEventRecord(c->ev.back(), c->stream); }
 };
 
+bool pdl_enabled();      // GAME_PDL=0 turns the attribute off (measurement knob)
+
+// kernel<<<grid, block, smem, stream>>>(args...) with the PDL attribute
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args &&...args)
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl_enabled() ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 // expand.cu
 int launch_check_finite(game_ctx *ctx, const float *X, long long nX, const float *t, long long nT, int *flag_dev);
 int launch_expand_fp32(game_ctx *ctx);      // X -> ET
 int launch_expand_fp16(game_ctx *ctx, float *maxabs_dev);   // X -> E16
+int launch_expand_split(game_ctx *ctx);                     // X -> E16s
 int launch_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out);
 int launch_classify(game_ctx *ctx, const float *genes, float cut, long long *counts, double *fom, unsigned int *ticket);
 
@@ -168,7 +196,9 @@ int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scra
 bool tensor_path_built();
 int tensor_prepare(game_ctx *ctx);                               // tensor maps etc. after load
 int tensor_expansion(const game_ctx *ctx, int P);                // GAME_EXPAND_MATERIALIZED / _REGENERATED, or -1
-int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer);
+int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer,
+                          bool split = false);
+int tensor_prepare_split(game_ctx *ctx);                         // E16s + its tensor maps, on first use
 
 // ga.cu
 int launch_init_population(game_ctx *ctx, int mode, unsigned long long seed, int P, float *pop);

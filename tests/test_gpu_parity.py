@@ -1,7 +1,7 @@
 """GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element.
 
 Tolerances: fitness |gpu - ref| <= rtol*|ref| + atol with rtol=1e-5, atol=1e-7 on
-the FP32 path and rtol=1e-3, atol=1e-5 on the TENSOR path; TMSE is discontinuous at |r| = R, so its
+the FP32 and TENSOR_SPLIT paths and rtol=1e-3, atol=1e-5 on the TENSOR path; TMSE is discontinuous at |r| = R, so its
 bound is widened by near_p*(R+delta)^2/N where near_p counts the patterns within delta of the tube
 (delta = 1e-5 / 5e-3).  GA decisions (rank, parents, cut points, mutation masks and values, initial
 genes, Philox words) are bit-exact.
@@ -21,7 +21,8 @@ from paper_1304_0597_b200 import workloads as wl  # noqa: E402
 TRIG, CHEB = 0, 1
 SIGMOID, IDENTITY = 0, 1
 MSE, TMSE, RMSE = 0, 1, 2
-TOL = {g.GAME_PATH_FP32: (1e-5, 1e-7, 1e-5), g.GAME_PATH_TENSOR: (1e-3, 1e-5, 5e-3)}
+TOL = {g.GAME_PATH_FP32: (1e-5, 1e-7, 1e-5), g.GAME_PATH_TENSOR: (1e-3, 1e-5, 5e-3),
+       g.GAME_PATH_TENSOR_SPLIT: (1e-5, 1e-7, 1e-5)}       # split-fp16 on the tensor cores: the FP32 path's class
 
 
 def dev(a):
@@ -56,9 +57,10 @@ def make_ctx(fam, d, X, t, act=SIGMOID, err=MSE, R=0.0, path=g.GAME_PATH_AUTO):
 
 def paths_available(ctx, P):
     out = [g.GAME_PATH_FP32]
-    ctx.set_path(g.GAME_PATH_TENSOR)
-    if ctx.resolved_path(P) == g.GAME_PATH_TENSOR:
-        out.append(g.GAME_PATH_TENSOR)
+    for path in (g.GAME_PATH_TENSOR, g.GAME_PATH_TENSOR_SPLIT):
+        ctx.set_path(path)
+        if ctx.resolved_path(P) == path:
+            out.append(path)
     ctx.set_path(g.GAME_PATH_AUTO)
     return out
 
