@@ -83,8 +83,19 @@ const char *game_last_error(const game_ctx *ctx);   /* HOST string owned by the 
 int game_set_stream(game_ctx *ctx, void *cuda_stream);
 int game_set_activation(game_ctx *ctx, int act);                 /* default GAME_ACT_SIGMOID */
 int game_set_error(game_ctx *ctx, int err_type, float tmse_R);   /* default MSE; R in (0,1) for TMSE (L116) */
-int game_set_path(game_ctx *ctx, int path);                      /* default GAME_PATH_AUTO */
-/* Which path the next fitness call will take for population size P: GAME_PATH_FP32 or GAME_PATH_TENSOR. */
+/* Which kernels evaluate a2-a5, i.e. the arithmetic and the tolerance class of the returned fitness (north_star (2)):
+ *   GAME_PATH_FP32          fp32 FFMA contraction, fp32 epilogue: |fit - exact| <= 1e-5 |exact| + 1e-7;
+ *   GAME_PATH_TENSOR        tcgen05 tensor cores, fp16 operands (TF32's 11-bit significand), fp32 accumulate:
+ *                           1e-3 |exact| + 1e-5;  needs max|E| <= 2 (else GAME_ERR_UNSUPPORTED);
+ *   GAME_PATH_TENSOR_SPLIT  tensor cores on split operands: E and the genes are each an fp16 hi + lo pair and the three
+ *                           products hi.hi + hi.lo + lo.hi run as one fp16 contraction over 3K terms, fp32 accumulate,
+ *                           ex2 + rcp logistic: the FP32 path's class (1e-5 |exact| + 1e-7; measured 3e-7 .. 9e-7).
+ *                           Per-feature families with max|E| <= 2;
+ *   GAME_PATH_AUTO          (default) P >= 256 and N >= 16384: TENSOR;  P >= 256 otherwise: TENSOR_SPLIT;  else FP32
+ *                           (each falling back to FP32 where its condition on E fails). */
+int game_set_path(game_ctx *ctx, int path);
+/* Which path the next fitness call will take for population size P (one of the three above), or -1 if the requested
+ * one is unavailable for the loaded dataset. */
 int game_resolved_path(const game_ctx *ctx, int P);
 /* a1, TENSOR path only: where the fused fitness kernel takes the expansion from (north_star (1)).
  *   GAME_EXPAND_MATERIALIZED  streams the fp16 expansion matrix built once by game_load (L254's hoisting);

@@ -192,6 +192,8 @@ int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scra
         ++ctx->launches;
         return GAME_OK;
     }
+    // (a fused multi-CTA finalize + rank kernel for mid-size populations was measured on config 2: 22.7 vs 19.7 us per
+    // generation -- inside the captured graph three small kernels cost less than one with serial phases)
     int rc = launch_finalize(ctx, pi.n_chunks, pi.Ppad, P, fit, state);
     if (rc) return rc;
     return launch_rank(ctx, fit, P, rank_scratch, order, state, stop_error, true);

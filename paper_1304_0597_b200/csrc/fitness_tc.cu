@@ -656,31 +656,15 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     if (warp == WARP_MMA) { __syncwarp(); tc_fence_after(); tmem_dealloc<CG>(tmem_base, 512); }
 }
 
-// pop fp32 [P][K] -> C16 fp16 [Ppad][Kpad] (round to nearest even, clamped to the finite fp16 range), times `scale`
-// (1 or 0.5: exact, see the epilogue modes)
-// split != 0 (TENSOR_SPLIT path): rows of 3 Kpad positions [hi | lo | hi], hi = fp16(c), lo = fp16(c - hi); see expand_kernel
-__global__ void pop_to_f16_kernel(const float *__restrict__ pop, int P, int K, int Kpad, int family, int d, float scale,
-                                  __half *__restrict__ C16, const DevState *state, int split)
+// pop fp32 [P][K] -> the fp16 copy described by `sink` (c16_store)
+__global__ void pop_to_f16_kernel(const float *__restrict__ pop, int P, int K, C16Sink sink, const DevState *state)
 {
     pdl_wait();
     pdl_trigger();
     if (state && state->stopped) return;
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= (long long)P * K) return;
-    int p = (int)(i / K), k = (int)(i % K);
-    float v = fminf(fmaxf(pop[i], -65504.f), 65504.f) * scale;
-    int pos = k;
-    if (tc_permuted(family)) {              // ABI order k = i*B + m  ->  the tensor path's term order
-        const int B = tc_terms_per_feature(family, d);
-        pos = tc_position(family, d, k / B, k % B);
-    }
-    if (!split) {
-        C16[(long long)p * Kpad + pos] = __float2half_rn(v);
-    } else {
-        __half *row = C16 + (long long)p * 3 * Kpad;
-        const __half hi = __float2half_rn(v);
-        row[pos] = hi; row[Kpad + pos] = __float2half_rn(v - __half2float(hi)); row[2 * Kpad + pos] = hi;
-    }
+    c16_store(sink, (int)(i / K), (int)(i % K), pop[i]);
 }
 
 // ---- host side ------------------------------------------------------------------------------------------
@@ -757,6 +741,16 @@ static int sigmoid_mode()
         m = (e && e[0] == '0') ? MODE_SIG_EXACT : MODE_SIG_TANH32;
     }
     return m;
+}
+
+C16Sink tensor_sink(const game_ctx *ctx, bool split)
+{
+    const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : (split ? MODE_SIG_EXACT : sigmoid_mode());
+    C16Sink s;
+    s.ptr = split ? ctx->C16s : ctx->C16;
+    s.Kpad = ctx->Kpad; s.family = ctx->family; s.d = ctx->degree; s.split = split ? 1 : 0;
+    s.scale = mode == MODE_SIG_TANH32 ? 0.5f : 1.0f;
+    return s;
 }
 
 int tensor_prepare(game_ctx *ctx)
@@ -862,9 +856,12 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     // the split path is the 1e-5 tolerance class: its logistic is the ex2 + rcp form (2^-22), not tanh.approx (2^-11)
     const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : (split ? MODE_SIG_EXACT : sigmoid_mode());
     const int ew = epilogue_warps(ctx);
-    GAME_CUDA(ctx, launch_pdl(pop_to_f16_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, ctx->stream, pop, P, ctx->K, ctx->Kpad,
-                              ctx->family, ctx->degree, mode == MODE_SIG_TANH32 ? 0.5f : 1.0f, split ? ctx->C16s : ctx->C16, state, split ? 1 : 0));
-    ++ctx->launches;
+    const C16Sink sink = tensor_sink(ctx, split);
+    if (!(ctx->c16_src == pop && ctx->c16_split == sink.split && ctx->c16_scale == sink.scale)) {   // else ga_step_kernel already wrote it
+        GAME_CUDA(ctx, launch_pdl(pop_to_f16_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, ctx->stream, pop, P, ctx->K, sink, state));
+        ++ctx->launches;
+        ctx->c16_src = nullptr;           // an external population: nothing to remember
+    }
     int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_C, split ? ctx->C16s : ctx->C16, Ppad, Kp, BM);
     if (rc) return rc;
 #define GAME_TC_EW(CGV, M, T)                                                                              \

@@ -197,6 +197,7 @@ struct StepArgs {
     Thr pc, pm;
     unsigned long long seed;
     uint32_t gen;
+    C16Sink sink;        // the next fitness call's fp16 copy of `next`, written alongside (ptr == nullptr: none)
 };
 
 __device__ int select_parent(const StepArgs &a, uint32_t slot, const int *__restrict__ order,
@@ -237,15 +238,25 @@ __global__ void ga_step_kernel(StepArgs a, const int *__restrict__ order, const 
     if (blockIdx.x < a.e) {                         // a8 elitism (L148, L291; DESIGN G17)
         int j = blockIdx.x;
         int src = stopped ? j : (a.elite_mode == GAME_ELITE_TOP_E ? order[j] : order[0]);
-        for (int k = threadIdx.x; k < K; k += blockDim.x) next[(long long)j * K + k] = pop[(long long)src * K + k];
+        for (int k = threadIdx.x; k < K; k += blockDim.x) {
+            const float v = pop[(long long)src * K + k];
+            next[(long long)j * K + k] = v;
+            if (a.sink.ptr) c16_store(a.sink, j, k, v);
+        }
         return;
     }
     const int q = blockIdx.x - a.e;
     const int sA = a.e + 2 * q, sB = sA + 1;
     if (stopped) {                                  // loop already stopped: carry the population over unchanged
         for (int k = threadIdx.x; k < K; k += blockDim.x) {
-            next[(long long)sA * K + k] = pop[(long long)sA * K + k];
-            if (sB < a.P) next[(long long)sB * K + k] = pop[(long long)sB * K + k];
+            const float vA = pop[(long long)sA * K + k];
+            next[(long long)sA * K + k] = vA;
+            if (a.sink.ptr) c16_store(a.sink, sA, k, vA);
+            if (sB < a.P) {
+                const float vB = pop[(long long)sB * K + k];
+                next[(long long)sB * K + k] = vB;
+                if (a.sink.ptr) c16_store(a.sink, sB, k, vB);
+            }
         }
         return;
     }
@@ -269,19 +280,22 @@ __global__ void ga_step_kernel(StepArgs a, const int *__restrict__ order, const 
         W4 w = draw(a.seed, (uint32_t)k, (uint32_t)sA, a.gen, TAG_MUTATE);       // a11 (R6)
         if (hit(w.x, a.pm)) cA = upm1(w.y);
         next[(long long)sA * K + k] = cA;
+        if (a.sink.ptr) c16_store(a.sink, sA, k, cA);
         if (sB < a.P) {
             W4 v = draw(a.seed, (uint32_t)k, (uint32_t)sB, a.gen, TAG_MUTATE);
             if (hit(v.x, a.pm)) cB = upm1(v.y);
             next[(long long)sB * K + k] = cB;
+            if (a.sink.ptr) c16_store(a.sink, sB, k, cB);
         }
     }
 }
 
 int launch_ga_step(game_ctx *ctx, const game_ga_params *gp, unsigned long long seed, unsigned int gen_base,
                    const int *order, const float *fit, const float *pop, float *next, DevState *state,
-                   unsigned int *rw, unsigned long long *rprefix)
+                   unsigned int *rw, unsigned long long *rprefix, const C16Sink *sink)
 {
     StepArgs a;
+    if (sink) a.sink = *sink; else a.sink.ptr = nullptr;
     a.P = gp->P; a.K = ctx->K; a.e = gp->elitism; a.elite_mode = gp->elite_mode; a.selection = gp->selection;
     a.tsize = gp->tournament_size; a.npairs = (gp->P - gp->elitism + 1) / 2;
     a.pc = host_thr(gp->p_crossover); a.pm = host_thr(gp->p_mutation);

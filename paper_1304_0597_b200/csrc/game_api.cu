@@ -89,13 +89,13 @@ static int ensure_scratch(game_ctx *c, int P)
         dfree(c->C16);
         GAME_CUDA(c, cudaMalloc(&c->C16, need16 * sizeof(__half)));
         GAME_CUDA(c, cudaMemsetAsync(c->C16, 0, need16 * sizeof(__half), c->stream));
-        c->c16_cap = need16;
+        c->c16_cap = need16; c->c16_src = nullptr;
     }
     if (c->tensor_ok && c->path != GAME_PATH_FP32 && c->path != GAME_PATH_TENSOR && 3 * need16 > c->c16s_cap) {   // AUTO or SPLIT may need it
         dfree(c->C16s);
         GAME_CUDA(c, cudaMalloc(&c->C16s, 3 * need16 * sizeof(__half)));
         GAME_CUDA(c, cudaMemsetAsync(c->C16s, 0, 3 * need16 * sizeof(__half), c->stream));
-        c->c16s_cap = 3 * need16;
+        c->c16s_cap = 3 * need16; c->c16_src = nullptr;
     }
     return GAME_OK;
 }
@@ -148,6 +148,7 @@ static int load_common(game_ctx *c, const float *X, const float *targets, long l
     if (!X || !targets || N < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_load: X, targets must be non-NULL and N >= 1");
     free_dataset(c);
     dfree(c->partial); c->partial_cap = 0;
+    c->c16_src = nullptr;
     const int K = c->K;
     c->N = N;
     c->n_slabs = (int)((N + SLAB - 1) / SLAB);
@@ -357,6 +358,7 @@ int game_advance(game_ctx *c, const double *sums, long long N_total, unsigned lo
                             c->rprefix);
         if (rc) return rc;
         float *tmp = c->pop; c->pop = c->pop_next; c->pop_next = tmp;
+        c->c16_src = nullptr;
     }
     DevState h{};
     GAME_CUDA(c, cudaMemcpyAsync(&h, c->state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
@@ -395,7 +397,7 @@ int game_set_population(game_ctx *c, const float *pop, int P)
     int rc = ensure_population(c, P);
     if (rc) return rc;
     GAME_CUDA(c, cudaMemcpyAsync(c->pop, pop, (size_t)P * c->K * sizeof(float), cudaMemcpyDefault, c->stream));
-    c->P = P; c->have_pop = true; c->have_fit = false;
+    c->P = P; c->have_pop = true; c->have_fit = false; c->c16_src = nullptr;
     return GAME_OK;
 }
 
@@ -420,7 +422,7 @@ int game_evolve(game_ctx *c, int generations, unsigned long long seed, const gam
         if (rc) return rc;
         rc = launch_init_population(c, gp->init_mode, seed, P, c->pop);     // a12
         if (rc) return rc;
-        c->P = P; c->have_pop = true;
+        c->P = P; c->have_pop = true; c->c16_src = nullptr;
     }
     GAME_CUDA(c, cudaMemsetAsync(c->state, 0, sizeof(DevState), c->stream));
     DevState h{};
@@ -435,9 +437,15 @@ int game_evolve(game_ctx *c, int generations, unsigned long long seed, const gam
     auto generation = [&]() -> int {
         int r = evaluate();
         if (r) return r;
-        r = launch_ga_step(c, gp, seed, gen_base, c->order, c->fit, c->pop, c->pop_next, c->state, c->rw, c->rprefix);   // a8-a11
+        // a8-a11; on the tensor paths the operators also write the fp16 copy the next evaluation contracts against
+        const int path = resolve_path(c, P);
+        C16Sink sink = tensor_sink(c, path == GAME_PATH_TENSOR_SPLIT);
+        const bool with_sink = (path == GAME_PATH_TENSOR || path == GAME_PATH_TENSOR_SPLIT) && sink.ptr != nullptr;
+        r = launch_ga_step(c, gp, seed, gen_base, c->order, c->fit, c->pop, c->pop_next, c->state, c->rw, c->rprefix,
+                           with_sink ? &sink : nullptr);
         if (r) return r;
         float *tmp = c->pop; c->pop = c->pop_next; c->pop_next = tmp;
+        c->c16_src = with_sink ? c->pop : nullptr; c->c16_split = sink.split; c->c16_scale = sink.scale;
         return GAME_OK;
     };
     auto stopped_now = [&](bool &stop) -> int {                      // poll the device-side stop flag

@@ -70,6 +70,32 @@ __host__ __device__ inline int tc_position(int family, int d, int i, int m)
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
+// Where (and how) the tensor paths keep their fp16 copy of a population: written by pop_to_f16_kernel, or directly by
+// ga_step_kernel while it builds the next generation (one launch and one pass over the genes less per generation).
+struct C16Sink {
+    __half *ptr;         // nullptr: no copy wanted
+    int Kpad, family, d, split;
+    float scale;         // 1, or 0.5 for the tanh logistic (exact)
+};
+// gene k (ABI order) of chromosome p -> its fp16 position(s): round to nearest even, clamped to the finite fp16 range;
+// split: rows of 3 Kpad positions [hi | lo | hi], hi = fp16(c), lo = fp16(c - hi) (see expand_kernel)
+__device__ __forceinline__ void c16_store(const C16Sink &s, int p, int k, float gene)
+{
+    const float v = fminf(fmaxf(gene, -65504.f), 65504.f) * s.scale;
+    int pos = k;
+    if (tc_permuted(s.family)) {              // ABI order k = i*B + m  ->  the tensor path's term order
+        const int B = tc_terms_per_feature(s.family, s.d);
+        pos = tc_position(s.family, s.d, k / B, k % B);
+    }
+    if (!s.split) {
+        s.ptr[(long long)p * s.Kpad + pos] = __float2half_rn(v);
+    } else {
+        __half *row = s.ptr + (long long)p * 3 * s.Kpad;
+        const __half hi = __float2half_rn(v);
+        row[pos] = hi; row[s.Kpad + pos] = __float2half_rn(v - __half2float(hi)); row[2 * s.Kpad + pos] = hi;
+    }
+}
+
 struct FitnessCfg {
     int act, err;
     float R;
@@ -118,6 +144,9 @@ struct game_ctx {
     size_t c16_cap = 0;
     __half *C16s = nullptr;    // Ppad x 3 Kpad fp16 [hi | lo | hi] population copy (TENSOR_SPLIT path); padding stays zero
     size_t c16s_cap = 0;
+    const float *c16_src = nullptr;   // the fp32 population the fp16 copy currently mirrors (nullptr: none), and how
+    int c16_split = 0;
+    float c16_scale = 0.f;
     float *stage_pop = nullptr, *stage_fit = nullptr;   // device staging for *_host calls
     size_t stage_cap = 0;
     void *tmap_E = nullptr, *tmap_C = nullptr;          // host copies of CUtensorMap (TENSOR path)
@@ -207,7 +236,9 @@ int launch_rank(game_ctx *ctx, const float *fit, int P, int *rank_scratch, int *
 // generation index = gen_base (+ state->evals_done - 1 when state is given: the loop's device-side counter)
 int launch_ga_step(game_ctx *ctx, const game_ga_params *gp, unsigned long long seed, unsigned int gen_base,
                    const int *order, const float *fit, const float *pop, float *next, DevState *state,
-                   unsigned int *rw, unsigned long long *rprefix);
+                   unsigned int *rw, unsigned long long *rprefix, const C16Sink *sink = nullptr);
+// the sink a TENSOR / TENSOR_SPLIT fitness call on this context would read (ptr == nullptr when buffers are missing)
+C16Sink tensor_sink(const game_ctx *ctx, bool split);
 int launch_philox(game_ctx *ctx, unsigned long long seed, const unsigned int *ctr, int n, unsigned int *out);
 
 }  // namespace game
