@@ -73,3 +73,40 @@ class ShardedGame:
         return run_generations(lambda: g.fitness_sums(None, params.P),
                                lambda sums, apply: g.advance(sums, self.N_total, seed, params, apply),
                                self.world, generations)
+
+
+class ChunkedGame:
+    """Out-of-core evaluation ("massive datasets ... GPU memory management", L417): the same
+    decomposition in TIME instead of space.  The dataset stays in (pinned) host memory; every generation its row
+    chunks pass through ONE context one after the other -- game_load(chunk) (upload + expansion), game_fitness_sums --
+    and the fp64 totals add up on the device before game_advance takes the mean over all N.  The population lives in
+    the context and survives the loads.  Costs one upload and one expansion of the dataset per generation: for datasets
+    that do not fit beside their expansion, not a fast path for those that do."""
+
+    def __init__(self, game, X_host, t_host, rows_per_chunk):
+        if rows_per_chunk < 1:
+            raise ValueError("rows_per_chunk must be >= 1")
+        self.game, self.X, self.t, self.rows = game, X_host, t_host, int(rows_per_chunk)
+        self.N_total = X_host.shape[0]
+        self._started = False
+
+    def chunks(self):
+        return [(lo, min(lo + self.rows, self.N_total)) for lo in range(0, self.N_total, self.rows)]
+
+    def totals(self, P):
+        import torch
+        sums = torch.zeros(P, dtype=torch.float64, device="cuda")
+        for lo, hi in self.chunks():
+            self.game.load_host(self.X[lo:hi], self.t[lo:hi])
+            sums += self.game.fitness_sums(None, P)
+        return sums
+
+    def evolve(self, generations, seed, params):
+        g = self.game
+        if not self._started:
+            lo, hi = self.chunks()[0]
+            g.load_host(self.X[lo:hi], self.t[lo:hi])
+            g.evolve(0, seed, params)            # a12: the initial population
+            self._started = True
+        return run_generations(lambda: self.totals(params.P),
+                               lambda sums, apply: g.advance(sums, self.N_total, seed, params, apply), 1, generations)

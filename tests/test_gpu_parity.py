@@ -557,3 +557,34 @@ def test_sharded_three_shards_one_gpu(orc, path, err, R):
         for s in shards:
             p = s.game.get_population_host(want_fit=False)[0]
             assert np.array_equal(p.view(np.uint32), nxt.view(np.uint32))
+
+
+def test_out_of_core_chunks(orc):
+    """the dataset streamed through one context in row chunks every generation (ragged last chunk):
+    fitness within the path's tolerance of the full-data oracle, operators bit-exact from the GPU's ranks."""
+    from paper_1304_0597_b200 import sharded
+    rng = np.random.default_rng(43)
+    fam, d, F, N, P = TRIG, 3, 8, 10000, 64
+    X = rng.uniform(-1, 1, (N, F)).astype(np.float32)
+    t = rng.integers(0, 2, N).astype(np.float32)
+    seed = 9
+    gp = g.ga_params(P=P)
+    gpo = orc.GaParams(P=P, tournament_size=3, elitism=2, elite_mode=0, selection=0, init_mode=1, p_crossover=0.9,
+                       p_mutation=0.05, stop_error=-1.0)
+    ctx = g.Game(fam, d, F)
+    ctx.set_error(TMSE, 0.49)
+    cg = sharded.ChunkedGame(ctx, X, t, 3000)
+    assert cg.chunks() == [(0, 3000), (3000, 6000), (6000, 9000), (9000, 10000)]
+    cg.evolve(0, seed, gp)
+    for gen in range(3):
+        pop = ctx.get_population_host(want_fit=False)[0]
+        sums = cg.totals(P)
+        path = ctx.resolved_path(P)
+        fit = sums.cpu().numpy() / N
+        check_fitness(orc, fit, fam, d, X, t, pop, SIGMOID, TMSE, 0.49, path, "gen %d" % gen)
+        done, res = cg.evolve(1, seed, gp)
+        assert done == 1 and ctx.generation() == gen + 1
+        # evolve(1) recomputed the same totals (deterministic), so the operators started from `fit`
+        fit32 = fit.astype(np.float32)
+        nxt = orc.ga_step(gpo, seed, gen, orc.rank(fit32), fit32, pop)
+        assert np.array_equal(ctx.get_population_host(want_fit=False)[0].view(np.uint32), nxt.view(np.uint32))
