@@ -91,8 +91,8 @@ int game_set_error(game_ctx *ctx, int err_type, float tmse_R);   /* default MSE;
  *                           products hi.hi + hi.lo + lo.hi run as one fp16 contraction over 3K terms, fp32 accumulate,
  *                           ex2 + rcp logistic: the FP32 path's class (1e-5 |exact| + 1e-7; measured 3e-7 .. 9e-7).
  *                           Per-feature families with max|E| <= 2;
- *   GAME_PATH_AUTO          (default) P >= 256 and N >= 16384: TENSOR;  P >= 256 otherwise: TENSOR_SPLIT;  else FP32
- *                           (each falling back to FP32 where its condition on E fails). */
+ *   GAME_PATH_AUTO          (default) N >= 16384: TENSOR;  smaller datasets: TENSOR_SPLIT;  FP32 where the tensor paths'
+ *                           conditions fail (tied families, max|E| > 2). */
 int game_set_path(game_ctx *ctx, int path);
 /* Which path the next fitness call will take for population size P (one of the three above), or -1 if the requested
  * one is unavailable for the loaded dataset. */
