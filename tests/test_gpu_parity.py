@@ -370,13 +370,16 @@ def test_stop_criterion(orc):
 
 
 # ---- BASELINE.json's full sizes, in the launch configuration bench.py times: sampled outputs ---------
-@pytest.mark.parametrize("cfg,nsample", [(3, 24), (4, 8), (5, 8)])
-def test_full_size_sampled(orc, cfg, nsample):
+@pytest.mark.parametrize("cfg,nsample,want_path", [(3, 24, g.GAME_PATH_AUTO), (4, 8, g.GAME_PATH_AUTO), (5, 8, g.GAME_PATH_AUTO),
+                                                  (3, 24, g.GAME_PATH_TENSOR_SPLIT), (5, 8, g.GAME_PATH_TENSOR_SPLIT),
+                                                  (1, 15, g.GAME_PATH_AUTO), (2, 24, g.GAME_PATH_AUTO)])
+def test_full_size_sampled(orc, cfg, nsample, want_path):
     w = wl.config(cfg)
     fam, d = w.family, w.degree
     X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
-    ctx = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    ctx = make_ctx(fam, d, X, t, w.act, w.err, w.R, want_path)
     path = ctx.resolved_path(w.P)
+    assert path == (want_path if want_path != g.GAME_PATH_AUTO else (g.GAME_PATH_TENSOR if w.N >= 16384 else g.GAME_PATH_TENSOR_SPLIT))
     gp = g.ga_params(P=w.P)
     ctx.evolve(2, w.seed, gp)                                 # init + two real generations at full size
     pop, fit, order = ctx.get_population_host()
