@@ -191,7 +191,9 @@ static int load_common(game_ctx *c, const float *X, const float *targets, long l
         memcpy(&c->x_maxabs, &h[2], sizeof(float));
         // fp16 rounding is relative: sums over features (tied families) of magnitude ~F would carry an absolute
         // error ~F*2^-11 into z, outside the 1e-3 class, so the tensor path is offered for |E| <= 2 only
-        c->tensor_ok = mx <= 2.0f;
+        // ... and the tile-blocked expansion is addressed with 32-bit TMA row coordinates (the split form has 3x the rows)
+        const bool rows_ok = (double)c->Npad256 * (3.0 * c->Kpad / TC_KBLK) < 2147483647.0;
+        c->tensor_ok = mx <= 2.0f && rows_ok;
         if (c->tensor_ok) {
             rc = tensor_prepare(c);
             if (rc) return rc;
