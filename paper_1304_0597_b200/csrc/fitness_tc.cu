@@ -45,7 +45,7 @@ constexpr int GEN_STAGES = 4;           // B k-block stages of the generator rin
 constexpr int GEN_B_BYTES = 128 * BKB * 2;
 constexpr int GEN_BAR0 = 2;             // named barriers 2.. : one per generator stage (0 = CTA, 1 = epilogue)
 constexpr int MAX_STAGES = 6;           // barrier slots are laid out for the deepest ring
-constexpr int TC_TAIL_BYTES = 256 /*barriers*/ + 3 * BN * 4 /*targets*/ + 2 * 4 * BM * 4 /*column-block error sums of two tiles*/;
+constexpr int TC_TAIL_BYTES = 256 /*barriers*/ + 3 * BN * 4 /*targets: [3][BN], or [team][2][BN]*/ + 2 * 4 * BM * 4 /*column-block error sums of two tiles*/;
 
 template <int CG> struct Cfg {
     static constexpr int BNL = BN / CG;                 // pattern rows this CTA stages
@@ -426,7 +426,7 @@ __device__ __forceinline__ void generate_expansion(const float *__restrict__ X, 
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------
-template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY>
+template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY, bool TEAMS>
 __global__ void __launch_bounds__(64 + 32 * EW + (SRC == SRC_GEN ? 32 * GEN_WARPS : 0), 1)
 fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmE,
                   int n_tiles, int m_blocks, int k_blocks, long long N, const float *__restrict__ tgt, float R,
@@ -452,8 +452,8 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     const uint32_t afull_bar = bar0 + 8u * (2 * MAX_STAGES + 4);      // SRC_GEN: the resident A tile has landed
     const uint32_t tmem_slot = bar0 + 8u * (2 * MAX_STAGES + 5);
     volatile uint32_t *tmem_slot_g = reinterpret_cast<volatile uint32_t *>(gbase + ring_bytes + 8 * (2 * MAX_STAGES + 5));
-    float *tgt_s = reinterpret_cast<float *>(gbase + ring_bytes + 256);   // [3][BN]
-    float *sum_s = tgt_s + 3 * BN;                                                        // [2][4][BM]
+    float *tgt_s = reinterpret_cast<float *>(gbase + ring_bytes + 256);   // [3][BN] (TEAMS: [2 teams][2][BN], reaching into sum_s)
+    float *sum_s = tgt_s + 3 * BN;                                        // [2][4][BM]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint32_t cta_rank = 0;
@@ -464,7 +464,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     if (threadIdx.x == 0) {
         // SRC_GEN: a B stage is full when the generator warps of BOTH CTAs have published their half
         for (int s = 0; s < NSTAGES; ++s) { mbar_init(full_bar(s), SRC == SRC_GEN ? CG : 1); mbar_init(empty_bar(s), 1); }
-        for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), CG * EW); }
+        for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), CG * (TEAMS ? 4 : EW) /* the epilogue warps (per CTA) that drain one accumulator */); }
         mbar_init(afull_bar, 1);
         fence_barrier_init();
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmC) : "memory");
@@ -568,99 +568,171 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
         generate_expansion<FAMILY>(X, F, degree, N, k_blocks, pair, n_pairs, total_tiles, (int)cta_rank,
                                    threadIdx.x - 32 * WARP_GEN0, gbase + k_blocks * A_BYTES, bar0);
     } else {
-        // ===== epilogue warps =====
-        // EW warps: warp w may touch TMEM lanes 32*(w%4).., so four warps cover the 128 chromosomes and EW/4 such
-        // groups split the tile's 256 pattern columns.  16 warps (4 per scheduler) keep the MUFU pipe fed where the
-        // epilogue is the bound (shallow K); 8 leave more registers per thread.
-        constexpr int NCB = EW / 4;                 // column blocks per tile
-        constexpr int CBW = BN / NCB;               // columns per block: 128 or 64
-        constexpr int NCH = CBW / 32;               // 32-column chunks per tile and warp: 4 or 2 (even)
-        const int ew = warp - WARP_EPI0;
-        const int quarter = warp & 3;               // TMEM lane quarter this warp may touch
-        const int cb = ew >> 2;                     // which column block of the 256-column tile
-        const int et = threadIdx.x - 32 * WARP_EPI0;
-        // One continuous stream of 32-column chunks: the TMEM load of the next chunk -- the next TILE's first chunk
-        // included -- is in flight while the current one is evaluated.  Targets are staged one tile ahead in a ring
-        // of three buffers: the buffer written during tile i was last read in tile i-2, and the one barrier per tile
-        // separates the two.  Patterns beyond N carry the target that makes their residual exactly zero (their
-        // expansion rows are zero, so z = 0): no masked code path.  The column blocks' sums of a tile meet in shared
-        // memory and are added in fixed order by block 0's warps one tile later: one partial row per 256 patterns.
-        constexpr float tbias = ACT == MODE_SIG_TANH32 ? 0.5f : 0.f;           // staged target = t - tbias
-        constexpr float tneutral = ACT == MODE_SIG_EXACT ? 0.5f : 0.f;         // staged target of a padding pattern
-        // raw target of this thread's pattern in `tile` (tneutral + tbias for a padding pattern); the bias comes
-        // off when the value is staged one tile later, so nothing waits on the load where it is issued
-        auto fetch_target = [&](int tile) -> float {
-            const long long n = (long long)(tile / m_blocks) * BN + et;
-            return (et < BN && n < N) ? tgt[n] : tneutral + tbias;
-        };
-        auto epi_barrier = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(32 * EW) : "memory"); };
-        const int row = quarter * 32 + lane;        // chromosome row inside the 128-row block
-        long long prev_off = -1;                    // where the previous tile's sum goes in `partial`
-        auto flush = [&](int buf) {                 // block 0's warps: add the tile's column-block sums, ascending
-            if (cb == 0 && prev_off >= 0) {
-                const float *ss = sum_s + buf * 4 * BM + row;
-                float s = ss[0];
-#pragma unroll
-                for (int j = 1; j < NCB; ++j) s += ss[j * BM];
-                partial[prev_off] = s;
-            }
-        };
-        const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(cb * CBW);
-        int acc = 0; uint32_t aph = 0; int tb = 0, sb = 0;
-        uint32_t va[32], vb[32];
-        float t_next = 0.f;
-        if (pair < total_tiles) {
-            if (et < BN) tgt_s[et] = fetch_target(pair) - tbias;
-            if (pair + n_pairs < total_tiles) t_next = fetch_target(pair + n_pairs);
-            epi_barrier();
-            mbar_wait(tfull_bar(0), 0);
-            tc_fence_after();
-            tmem_ld32(lane_addr, va);
-        }
-        for (int tile = pair; tile < total_tiles; tile += n_pairs) {
-            const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
-            const bool has_next = tile + n_pairs < total_tiles;
-            const uint32_t t0 = lane_addr + (uint32_t)(acc * BN);
-            const float *ts = tgt_s + tb * BN + cb * CBW;
-            const int tbn = tb == 2 ? 0 : tb + 1;
-            float2 acc2[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
-#pragma unroll
-            for (int c = 0; c < NCH; ++c) {
-                uint32_t (&cur)[32] = (c & 1) ? vb : va;
-                uint32_t (&nxt)[32] = (c & 1) ? va : vb;
-                tmem_ld_wait(cur);
-                if (c + 1 < NCH) {
-                    tmem_ld32(t0 + 32 * (c + 1), nxt);
-                } else {
-                    // every TMEM read of this tile's accumulator has completed: hand it back to the MMA warp
-                    // BEFORE waiting for the next one
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) {
-                        if (CG == 1) mbar_arrive(tempty_bar(acc));
-                        else mbar_arrive_cluster(tempty_bar(acc), 0);
+        if (TEAMS) {
+            // ===== epilogue warps: two independent teams of four =====
+            // Warp w may touch TMEM lanes 32*(w%4).., so four warps cover a tile's 128 chromosomes.  Team g (warps 4g..4g+3)
+            // owns accumulator g and takes every other tile of this CTA's sequence: a thread walks ALL 256 pattern columns of
+            // its chromosome, so the error sum of a tile is finished in registers (no cross-warp combine) and `partial` gets
+            // one row per 256 patterns.  The two warps that share a scheduler belong to different teams and therefore to
+            // different tiles at different stages: while one team waits for its accumulator's next MMA the other keeps the
+            // special-function unit busy, which two warps marching through the same tile in lockstep could not.
+            // Inside a tile the TMEM load of the next 32-column chunk is in flight while the current one is evaluated.
+            // Targets are staged per team through two buffers (the team's one barrier per tile separates writer and
+            // readers); the next tile's target is fetched a tile ahead.  Patterns beyond N carry the target that makes their
+            // residual exactly zero (their expansion rows are zero, so z = 0): no masked code path.
+            static_assert(EW == 8, "two teams of four warps");
+            constexpr int NCH = BN / 32;                // 32-column chunks per tile: 8
+            const int ew = warp - WARP_EPI0;
+            const int team = ew >> 2;
+            const int quarter = warp & 3;               // TMEM lane quarter this warp may touch
+            const int tt = (ew & 3) * 32 + lane;        // thread index inside the team, 0..127
+            constexpr float tbias = ACT == MODE_SIG_TANH32 ? 0.5f : 0.f;           // staged target = t - tbias
+            constexpr float tneutral = ACT == MODE_SIG_EXACT ? 0.5f : 0.f;         // staged target of a padding pattern
+            // raw targets of this thread's two patterns in `tile` (tneutral + tbias for a padding pattern); the bias comes
+            // off when the values are staged one tile later, so nothing waits on the loads where they are issued
+            auto fetch_targets = [&](int tile, float &t0v, float &t1v) {
+                const long long n = (long long)(tile / m_blocks) * BN + tt;
+                t0v = n < N ? tgt[n] : tneutral + tbias;
+                t1v = n + 128 < N ? tgt[n + 128] : tneutral + tbias;
+            };
+            auto team_barrier = [&]() { asm volatile("bar.sync %0, 128;" ::"r"(1 + team) : "memory"); };
+            const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(team * BN);
+            const uint32_t tfull_b = tfull_bar(team), tempty_b = tempty_bar(team);
+            const int row = quarter * 32 + lane;        // chromosome row inside the 128-row block
+            const int step = 2 * n_pairs;
+            uint32_t aph = 0; int tb = 0;
+            uint32_t va[32], vb[32];
+            float tn0 = 0.f, tn1 = 0.f;
+            if (pair + team * n_pairs < total_tiles) fetch_targets(pair + team * n_pairs, tn0, tn1);
+            for (int tile = pair + team * n_pairs; tile < total_tiles; tile += step) {
+                const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
+                float *ts = tgt_s + (team * 2 + tb) * BN;
+                ts[tt] = tn0 - tbias;
+                ts[tt + 128] = tn1 - tbias;
+                if (tile + step < total_tiles) fetch_targets(tile + step, tn0, tn1);
+                team_barrier();
+                mbar_wait(tfull_b, aph);
+                tc_fence_after();
+                tmem_ld32(lane_addr, va);
+                float2 acc2[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+    #pragma unroll
+                for (int c = 0; c < NCH; ++c) {
+                    uint32_t (&cur)[32] = (c & 1) ? vb : va;
+                    uint32_t (&nxt)[32] = (c & 1) ? va : vb;
+                    tmem_ld_wait(cur);
+                    if (c + 1 < NCH) {
+                        tmem_ld32(lane_addr + 32 * (c + 1), nxt);
+                    } else {
+                        // every TMEM read of this accumulator has completed: hand it back to the MMA warp right away
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) {
+                            if (CG == 1) mbar_arrive(tempty_b);
+                            else mbar_arrive_cluster(tempty_b, 0);
+                        }
                     }
-                    if (has_next && et < BN) tgt_s[tbn * BN + et] = t_next - tbias;
-                    if (tile + 2 * n_pairs < total_tiles) t_next = fetch_target(tile + 2 * n_pairs);
-                    epi_barrier();
-                    flush(sb ^ 1);
-                    if (has_next) {                   // uniform over the CTA's epilogue warps
-                        mbar_wait(tfull_bar(acc ^ 1), acc ? aph ^ 1 : aph);
-                        tc_fence_after();
-                        tmem_ld32(lane_addr + (uint32_t)((acc ^ 1) * BN), nxt);
-                    }
+                    epilogue_chunk<ACT, TMSE>(cur, ts + 32 * c, R, acc2);
                 }
-                epilogue_chunk<ACT, TMSE>(cur, ts + 32 * c, R, acc2);
+                partial[(long long)n_tile * Ppad + (m_blk * CG + (int)cta_rank) * BM + row] =
+                    ((acc2[0].x + acc2[0].y) + (acc2[1].x + acc2[1].y)) + ((acc2[2].x + acc2[2].y) + (acc2[3].x + acc2[3].y));
+                tb ^= 1;
+                aph ^= 1;
             }
-            sum_s[(sb * 4 + cb) * BM + row] = ((acc2[0].x + acc2[0].y) + (acc2[1].x + acc2[1].y)) + ((acc2[2].x + acc2[2].y) + (acc2[3].x + acc2[3].y));
-            prev_off = (long long)n_tile * Ppad + (m_blk * CG + (int)cta_rank) * BM + row;
-            tb = tbn;
-            sb ^= 1;
-            if (++acc == 2) { acc = 0; aph ^= 1; }
-        }
-        if (pair < total_tiles) {
-            epi_barrier();
-            flush(sb ^ 1);
+        } else {
+            // ===== epilogue warps =====
+            // EW warps: warp w may touch TMEM lanes 32*(w%4).., so four warps cover the 128 chromosomes and EW/4 such
+            // groups split the tile's 256 pattern columns.  16 warps (4 per scheduler) keep the MUFU pipe fed where the
+            // epilogue is the bound (shallow K); 8 leave more registers per thread.
+            constexpr int NCB = EW / 4;                 // column blocks per tile
+            constexpr int CBW = BN / NCB;               // columns per block: 128 or 64
+            constexpr int NCH = CBW / 32;               // 32-column chunks per tile and warp: 4 or 2 (even)
+            const int ew = warp - WARP_EPI0;
+            const int quarter = warp & 3;               // TMEM lane quarter this warp may touch
+            const int cb = ew >> 2;                     // which column block of the 256-column tile
+            const int et = threadIdx.x - 32 * WARP_EPI0;
+            // One continuous stream of 32-column chunks: the TMEM load of the next chunk -- the next TILE's first chunk
+            // included -- is in flight while the current one is evaluated.  Targets are staged one tile ahead in a ring
+            // of three buffers: the buffer written during tile i was last read in tile i-2, and the one barrier per tile
+            // separates the two.  Patterns beyond N carry the target that makes their residual exactly zero (their
+            // expansion rows are zero, so z = 0): no masked code path.  The column blocks' sums of a tile meet in shared
+            // memory and are added in fixed order by block 0's warps one tile later: one partial row per 256 patterns.
+            constexpr float tbias = ACT == MODE_SIG_TANH32 ? 0.5f : 0.f;           // staged target = t - tbias
+            constexpr float tneutral = ACT == MODE_SIG_EXACT ? 0.5f : 0.f;         // staged target of a padding pattern
+            // raw target of this thread's pattern in `tile` (tneutral + tbias for a padding pattern); the bias comes
+            // off when the value is staged one tile later, so nothing waits on the load where it is issued
+            auto fetch_target = [&](int tile) -> float {
+                const long long n = (long long)(tile / m_blocks) * BN + et;
+                return (et < BN && n < N) ? tgt[n] : tneutral + tbias;
+            };
+            auto epi_barrier = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(32 * EW) : "memory"); };
+            const int row = quarter * 32 + lane;        // chromosome row inside the 128-row block
+            long long prev_off = -1;                    // where the previous tile's sum goes in `partial`
+            auto flush = [&](int buf) {                 // block 0's warps: add the tile's column-block sums, ascending
+                if (cb == 0 && prev_off >= 0) {
+                    const float *ss = sum_s + buf * 4 * BM + row;
+                    float s = ss[0];
+    #pragma unroll
+                    for (int j = 1; j < NCB; ++j) s += ss[j * BM];
+                    partial[prev_off] = s;
+                }
+            };
+            const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(cb * CBW);
+            int acc = 0; uint32_t aph = 0; int tb = 0, sb = 0;
+            uint32_t va[32], vb[32];
+            float t_next = 0.f;
+            if (pair < total_tiles) {
+                if (et < BN) tgt_s[et] = fetch_target(pair) - tbias;
+                if (pair + n_pairs < total_tiles) t_next = fetch_target(pair + n_pairs);
+                epi_barrier();
+                mbar_wait(tfull_bar(0), 0);
+                tc_fence_after();
+                tmem_ld32(lane_addr, va);
+            }
+            for (int tile = pair; tile < total_tiles; tile += n_pairs) {
+                const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
+                const bool has_next = tile + n_pairs < total_tiles;
+                const uint32_t t0 = lane_addr + (uint32_t)(acc * BN);
+                const float *ts = tgt_s + tb * BN + cb * CBW;
+                const int tbn = tb == 2 ? 0 : tb + 1;
+                float2 acc2[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+    #pragma unroll
+                for (int c = 0; c < NCH; ++c) {
+                    uint32_t (&cur)[32] = (c & 1) ? vb : va;
+                    uint32_t (&nxt)[32] = (c & 1) ? va : vb;
+                    tmem_ld_wait(cur);
+                    if (c + 1 < NCH) {
+                        tmem_ld32(t0 + 32 * (c + 1), nxt);
+                    } else {
+                        // every TMEM read of this tile's accumulator has completed: hand it back to the MMA warp
+                        // BEFORE waiting for the next one
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) {
+                            if (CG == 1) mbar_arrive(tempty_bar(acc));
+                            else mbar_arrive_cluster(tempty_bar(acc), 0);
+                        }
+                        if (has_next && et < BN) tgt_s[tbn * BN + et] = t_next - tbias;
+                        if (tile + 2 * n_pairs < total_tiles) t_next = fetch_target(tile + 2 * n_pairs);
+                        epi_barrier();
+                        flush(sb ^ 1);
+                        if (has_next) {                   // uniform over the CTA's epilogue warps
+                            mbar_wait(tfull_bar(acc ^ 1), acc ? aph ^ 1 : aph);
+                            tc_fence_after();
+                            tmem_ld32(lane_addr + (uint32_t)((acc ^ 1) * BN), nxt);
+                        }
+                    }
+                    epilogue_chunk<ACT, TMSE>(cur, ts + 32 * c, R, acc2);
+                }
+                sum_s[(sb * 4 + cb) * BM + row] = ((acc2[0].x + acc2[0].y) + (acc2[1].x + acc2[1].y)) + ((acc2[2].x + acc2[2].y) + (acc2[3].x + acc2[3].y));
+                prev_off = (long long)n_tile * Ppad + (m_blk * CG + (int)cta_rank) * BM + row;
+                tb = tbn;
+                sb ^= 1;
+                if (++acc == 2) { acc = 0; aph ^= 1; }
+            }
+            if (pair < total_tiles) {
+                epi_barrier();
+                flush(sb ^ 1);
+            }
         }
     }
 
@@ -734,20 +806,6 @@ static int cta_group(const game_ctx *ctx, int Ppad, int Kp)
     return (Kp >= 512 && Ppad >= 1024) ? 2 : 1;
 }
 
-// Epilogue warps per CTA: 8.  16 (four per scheduler, 96 registers each) were measured on B200 and lose everywhere
-// (config 3: 0.177 vs 0.154 ms; config 5: 2.32 vs 2.23 ms); GAME_TC_EPI_WARPS=16 keeps that variant measurable.
-static int epilogue_warps(const game_ctx *ctx)
-{
-    static int forced = -1;
-    if (forced < 0) {
-        const char *e = getenv("GAME_TC_EPI_WARPS");
-        forced = e ? (atoi(e) == 16 ? 16 : 8) : 0;
-    }
-    if (forced) return forced;
-    (void)ctx;
-    return 8;
-}
-
 // Which logistic form the epilogue uses: mode 2 unless GAME_TC_SIGMOID=0 (measurement knob).
 static int sigmoid_mode()
 {
@@ -800,11 +858,11 @@ int tensor_prepare_split(game_ctx *ctx)
     return GAME_OK;
 }
 
-template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY>
+template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY, bool TEAMS = false>
 static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, const DevState *state, bool split = false)
 {
     using C = Cfg<CG>;
-    auto kern = fitness_tc_kernel<CG, ACT, TMSE, EW, SRC, FAMILY>;
+    auto kern = fitness_tc_kernel<CG, ACT, TMSE, EW, SRC, FAMILY, TEAMS>;
     const int k_blocks = (split ? 3 : 1) * ctx->Kpad / BKB;
     const CUtensorMap *maps_E = (const CUtensorMap *)(split ? ctx->tmap_Es : ctx->tmap_E);
     const int smem = SRC != SRC_TMA ? k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES : C::SMEM;
@@ -873,13 +931,19 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     const bool resident_only = expansion != GAME_EXPAND_REGENERATED && resident_ok && Ppad == 256 && fits && Kp >= 256;
     const int src = expansion == GAME_EXPAND_REGENERATED ? SRC_GEN : (resident_only ? SRC_RES : SRC_TMA);
     const int cg = src != SRC_TMA ? 2 : cta_group(ctx, Ppad, Kp);
+    // Which epilogue: for shallow contractions (the MMAs of a tile take less time than its epilogue) two independent
+    // teams of four warps, one per accumulator, so the warps sharing a scheduler are in different stages of different
+    // tiles (config 3, same box: 0.139 vs 0.150 ms); for deep ones all eight warps on one tile, which hands the
+    // accumulator back sooner (configs 4, 5: the team form loses 1-2 % there).  GAME_TC_TEAMS=0|1 overrides.
+    static int teams_forced = -1;
+    if (teams_forced < 0) { const char *e = getenv("GAME_TC_TEAMS"); teams_forced = e ? (e[0] == '1' ? 1 : 0) : 2; }
+    const bool teams = teams_forced == 2 ? Kp <= 256 : teams_forced == 1;
     const int n_tiles = (int)(ctx->Npad256 / BN);
     const int m_blocks = Ppad / (BM * cg);
     long long n = (long long)P * ctx->K;
     const bool tmse = ctx->err == GAME_ERR_TMSE;
     // the split path is the 1e-5 tolerance class: its logistic is the ex2 + rcp form (2^-22), not tanh.approx (2^-11)
     const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : (split ? MODE_SIG_EXACT : sigmoid_mode());
-    const int ew = epilogue_warps(ctx);
     const C16Sink sink = tensor_sink(ctx, split);
     if (!(ctx->c16_src == pop && ctx->c16_split == sink.split && ctx->c16_scale == sink.scale)) {   // else ga_step_kernel already wrote it
         GAME_CUDA(ctx, launch_pdl(pop_to_f16_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, ctx->stream, pop, P, ctx->K, sink, state));
@@ -889,8 +953,8 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_C, split ? ctx->C16s : ctx->C16, Ppad, Kp, BM);
     if (rc) return rc;
 #define GAME_TC_EW(CGV, M, T)                                                                              \
-    rc = ew == 16 ? launch_variant<CGV, M, T, 16, SRC_TMA, GAME_TRIG>(ctx, n_tiles, m_blocks, Ppad, state, split)     \
-                  : launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG>(ctx, n_tiles, m_blocks, Ppad, state, split)
+    rc = teams ? launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG, true>(ctx, n_tiles, m_blocks, Ppad, state, split)           \
+               : launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG, false>(ctx, n_tiles, m_blocks, Ppad, state, split)
 #define GAME_TC_GEN(M, T)                                                                                  \
     rc = resident_only ? launch_variant<2, M, T, 8, SRC_RES, GAME_TRIG>(ctx, n_tiles, 1, Ppad, state, split) \
        : ctx->family == GAME_TRIG ? launch_variant<2, M, T, 8, SRC_GEN, GAME_TRIG>(ctx, n_tiles, 1, Ppad, state) \
