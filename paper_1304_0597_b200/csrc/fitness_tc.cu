@@ -426,7 +426,9 @@ __device__ __forceinline__ void generate_expansion(const float *__restrict__ X, 
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------
-template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY, bool TEAMS>
+// BNT: patterns per tile, 256 or (SRC_TMA, single CTAs, team epilogue only) 128: problems of less than one wave of
+// 256-pattern tiles finish sooner on twice as many half-size tiles (configs 1-2).
+template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY, bool TEAMS, int BNT = BN>
 __global__ void __launch_bounds__(64 + 32 * EW + (SRC == SRC_GEN ? 32 * GEN_WARPS : 0), 1)
 fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmE,
                   int n_tiles, int m_blocks, int k_blocks, long long N, const float *__restrict__ tgt, float R,
@@ -435,15 +437,19 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
 {
     using C = Cfg<CG>;
     static_assert(SRC == SRC_TMA || CG == 2, "the generator variant runs as CTA pairs");
+    static_assert(BNT == BN || (BNT == 128 && SRC == SRC_TMA && CG == 1 && TEAMS), "half-size tiles: streamed, single CTA, team epilogue");
     constexpr bool RESIDENT_A = SRC != SRC_TMA;
-    constexpr int NSTAGES = RESIDENT_A ? GEN_STAGES : C::STAGES;
+    constexpr int B_BYTES_K = (BNT / CG) * BKB * 2;                        // B k-block bytes this CTA stages
+    constexpr int STAGE_BYTES_K = A_BYTES + B_BYTES_K;
+    constexpr int NSTAGES = RESIDENT_A ? GEN_STAGES : (STAGE_BYTES_K <= 32768 ? 6 : 4);
+    static_assert(BNT != BN || (STAGE_BYTES_K == C::STAGE_BYTES && NSTAGES == (RESIDENT_A ? GEN_STAGES : C::STAGES)), "Cfg<CG> describes the full-size tile");
     constexpr int WARP_GEN0 = WARP_EPI0 + EW;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t *gbase = smem_raw + (base - smem_u32(smem_raw));
     // operand area: SRC_TMA a ring of (A, B) k-block stages; SRC_GEN the resident A tile (k_blocks blocks) + a B ring
     const uint32_t ring_bytes = RESIDENT_A ? (uint32_t)(k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES)
-                                               : (uint32_t)(C::STAGES * C::STAGE_BYTES);
+                                               : (uint32_t)(NSTAGES * STAGE_BYTES_K);
     const uint32_t bar0 = base + ring_bytes;
     auto full_bar = [&](int s) { return bar0 + 8u * s; };
     auto empty_bar = [&](int s) { return bar0 + 8u * (MAX_STAGES + s); };
@@ -523,11 +529,13 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             for (int tile = pair; tile < total_tiles; tile += n_pairs) {
                 const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
                 const int rowC = (m_blk * CG + (int)cta_rank) * BM;
-                const int rowE = n_tile * k_blocks * BN + (int)cta_rank * C::BNL;     // E16 is tile-blocked: [n_tile][kb][256][64]
+                // E16 is tile-blocked [n/256][kb][256][64]: this tile's (and this CTA's) rows inside the 256-row block
+                const int n_first = n_tile * BNT + (int)cta_rank * (BNT / CG);
+                const int rowE = (n_first >> 8) * k_blocks * BN + (n_first & 255);
                 for (int kb = 0; kb < k_blocks; ++kb) {
                     mbar_wait(empty_bar(s), ph ^ 1);
-                    const uint32_t sa = base + s * C::STAGE_BYTES, sb = sa + A_BYTES;
-                    if (CG == 1 || cta_rank == 0) mbar_expect_tx(full_bar(s), CG * C::STAGE_BYTES);
+                    const uint32_t sa = base + s * STAGE_BYTES_K, sb = sa + A_BYTES;
+                    if (CG == 1 || cta_rank == 0) mbar_expect_tx(full_bar(s), CG * STAGE_BYTES_K);
                     tma_load_2d<CG>(sa, &tmC, kb * BKB, rowC, full_bar(s));
                     tma_load_2d<CG>(sb, &tmE, 0, rowE + kb * BN, full_bar(s));
                     if (++s == NSTAGES) { s = 0; ph ^= 1; }
@@ -537,18 +545,18 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     } else if (warp == WARP_MMA) {
         // ===== MMA issuer (one thread; leader CTA only when paired) =====
         if (lane == 0 && cta_rank == 0) {
-            constexpr uint32_t idesc = make_idesc(BM * CG, BN);
+            constexpr uint32_t idesc = make_idesc(BM * CG, BNT);
             int s = 0; uint32_t ph = 0;
             int acc = 0; uint32_t aph = 0;
             if (RESIDENT_A) mbar_wait(afull_bar, 0);          // resident population tile of both CTAs
             for (int tile = pair; tile < total_tiles; tile += n_pairs) {
                 mbar_wait(tempty_bar(acc), aph ^ 1);          // epilogue has drained this accumulator
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
+                const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BNT);
                 for (int kb = 0; kb < k_blocks; ++kb) {
                     mbar_wait(full_bar(s), ph);               // operands have landed (SRC_GEN: were generated)
                     tc_fence_after();
-                    const uint32_t sa = RESIDENT_A ? base + kb * A_BYTES : base + s * C::STAGE_BYTES;
+                    const uint32_t sa = RESIDENT_A ? base + kb * A_BYTES : base + s * STAGE_BYTES_K;
                     const uint32_t sb = RESIDENT_A ? base + k_blocks * A_BYTES + s * GEN_B_BYTES : sa + A_BYTES;
                     const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sb);
 #pragma unroll
@@ -581,7 +589,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             // readers); the next tile's target is fetched a tile ahead.  Patterns beyond N carry the target that makes their
             // residual exactly zero (their expansion rows are zero, so z = 0): no masked code path.
             static_assert(EW == 8, "two teams of four warps");
-            constexpr int NCH = BN / 32;                // 32-column chunks per tile: 8
+            constexpr int NCH = BNT / 32;               // 32-column chunks per tile: 8 (4 for half-size tiles)
             const int ew = warp - WARP_EPI0;
             const int team = ew >> 2;
             const int quarter = warp & 3;               // TMEM lane quarter this warp may touch
@@ -591,12 +599,12 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             // raw targets of this thread's two patterns in `tile` (tneutral + tbias for a padding pattern); the bias comes
             // off when the values are staged one tile later, so nothing waits on the loads where they are issued
             auto fetch_targets = [&](int tile, float &t0v, float &t1v) {
-                const long long n = (long long)(tile / m_blocks) * BN + tt;
+                const long long n = (long long)(tile / m_blocks) * BNT + tt;
                 t0v = n < N ? tgt[n] : tneutral + tbias;
-                t1v = n + 128 < N ? tgt[n + 128] : tneutral + tbias;
+                t1v = (BNT > 128 && n + 128 < N) ? tgt[n + 128] : tneutral + tbias;
             };
             auto team_barrier = [&]() { asm volatile("bar.sync %0, 128;" ::"r"(1 + team) : "memory"); };
-            const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(team * BN);
+            const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(team * BNT);
             const uint32_t tfull_b = tfull_bar(team), tempty_b = tempty_bar(team);
             const int row = quarter * 32 + lane;        // chromosome row inside the 128-row block
             const int step = 2 * n_pairs;
@@ -606,9 +614,9 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             if (pair + team * n_pairs < total_tiles) fetch_targets(pair + team * n_pairs, tn0, tn1);
             for (int tile = pair + team * n_pairs; tile < total_tiles; tile += step) {
                 const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
-                float *ts = tgt_s + (team * 2 + tb) * BN;
+                float *ts = tgt_s + (team * 2 + tb) * BNT;
                 ts[tt] = tn0 - tbias;
-                ts[tt + 128] = tn1 - tbias;
+                if (BNT > 128) ts[tt + 128] = tn1 - tbias;
                 if (tile + step < total_tiles) fetch_targets(tile + step, tn0, tn1);
                 team_barrier();
                 mbar_wait(tfull_b, aph);
@@ -858,14 +866,16 @@ int tensor_prepare_split(game_ctx *ctx)
     return GAME_OK;
 }
 
-template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY, bool TEAMS = false>
+template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY, bool TEAMS = false, int BNT = BN>
 static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, const DevState *state, bool split = false)
 {
     using C = Cfg<CG>;
-    auto kern = fitness_tc_kernel<CG, ACT, TMSE, EW, SRC, FAMILY, TEAMS>;
+    auto kern = fitness_tc_kernel<CG, ACT, TMSE, EW, SRC, FAMILY, TEAMS, BNT>;
     const int k_blocks = (split ? 3 : 1) * ctx->Kpad / BKB;
     const CUtensorMap *maps_E = (const CUtensorMap *)(split ? ctx->tmap_Es : ctx->tmap_E);
-    const int smem = SRC != SRC_TMA ? k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES : C::SMEM;
+    const int smem = SRC != SRC_TMA ? k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES
+                   : BNT == BN    ? C::SMEM
+                                  : 6 * (A_BYTES + BNT * BKB * 2) + 1024 + TC_TAIL_BYTES;
     static int attr_smem = 0;
     if (smem > attr_smem) {
         GAME_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
@@ -886,7 +896,7 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = pdl_enabled() ? 2 : 1;
     KernelTimer timer(ctx);
-    GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, maps_E[CG - 1], n_tiles,
+    GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, maps_E[BNT / CG == 128 ? 1 : 0], n_tiles,
                                       m_blocks, k_blocks, ctx->N, (const float *)ctx->t, ctx->R, ctx->partial, Ppad, state,
                                       (const float *)ctx->X, ctx->F, ctx->degree));
     return GAME_OK;
@@ -928,7 +938,9 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     static int resident_ok = -1;
     if (resident_ok < 0) { const char *e = getenv("GAME_TC_RESIDENT"); resident_ok = (e && e[0] == '0') ? 0 : 1; }
     const bool fits = (Kp / BKB) * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES <= 227 * 1024;
-    const bool resident_only = expansion != GAME_EXPAND_REGENERATED && resident_ok && Ppad == 256 && fits && Kp >= 256;
+    const long long tiles256 = (long long)(ctx->Npad256 / BN) * ((P + BM - 1) / BM);     // 128-chromosome x 256-pattern tiles
+    const bool resident_only = expansion != GAME_EXPAND_REGENERATED && resident_ok && Ppad == 256 && fits && Kp >= 256 &&
+                               tiles256 >= ctx->sm_count;
     const int src = expansion == GAME_EXPAND_REGENERATED ? SRC_GEN : (resident_only ? SRC_RES : SRC_TMA);
     const int cg = src != SRC_TMA ? 2 : cta_group(ctx, Ppad, Kp);
     // Which epilogue: for shallow contractions (the MMAs of a tile take less time than its epilogue) two independent
@@ -938,8 +950,13 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     static int teams_forced = -1;
     if (teams_forced < 0) { const char *e = getenv("GAME_TC_TEAMS"); teams_forced = e ? (e[0] == '1' ? 1 : 0) : 2; }
     const bool teams = teams_forced == 2 ? Kp <= 256 : teams_forced == 1;
-    const int n_tiles = (int)(ctx->Npad256 / BN);
-    const int m_blocks = Ppad / (BM * cg);
+    // Less than one wave of 256-pattern tiles (configs 1-2): twice as many 128-pattern tiles on single CTAs finish sooner.
+    // GAME_TC_HALF_TILES=0|1 overrides, for measurement.
+    static int half_forced = -1;
+    if (half_forced < 0) { const char *e = getenv("GAME_TC_HALF_TILES"); half_forced = e ? (e[0] == '1' ? 1 : 0) : 2; }
+    const bool half_tiles = src == SRC_TMA && (half_forced == 2 ? tiles256 < ctx->sm_count : half_forced == 1);
+    const int n_tiles = (int)(ctx->Npad256 / (half_tiles ? 128 : BN));
+    const int m_blocks = half_tiles ? (P + BM - 1) / BM : Ppad / (BM * cg);
     long long n = (long long)P * ctx->K;
     const bool tmse = ctx->err == GAME_ERR_TMSE;
     // the split path is the 1e-5 tolerance class: its logistic is the ex2 + rcp form (2^-22), not tanh.approx (2^-11)
@@ -953,7 +970,8 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_C, split ? ctx->C16s : ctx->C16, Ppad, Kp, BM);
     if (rc) return rc;
 #define GAME_TC_EW(CGV, M, T)                                                                              \
-    rc = teams ? launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG, true>(ctx, n_tiles, m_blocks, Ppad, state, split)           \
+    rc = half_tiles ? launch_variant<1, M, T, 8, SRC_TMA, GAME_TRIG, true, 128>(ctx, n_tiles, m_blocks, Ppad, state, split)  \
+       : teams ? launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG, true>(ctx, n_tiles, m_blocks, Ppad, state, split)           \
                : launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG, false>(ctx, n_tiles, m_blocks, Ppad, state, split)
 #define GAME_TC_GEN(M, T)                                                                                  \
     rc = resident_only ? launch_variant<2, M, T, 8, SRC_RES, GAME_TRIG>(ctx, n_tiles, 1, Ppad, state, split) \
