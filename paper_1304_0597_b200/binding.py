@@ -60,8 +60,13 @@ def load_library():
     global _lib
     if _lib is None:
         if not os.path.exists(LIB_PATH):
-            raise ImportError("%s not found: run `python -m paper_1304_0597_b200.build` (there is no CPU fallback)"
-                              % LIB_PATH)
+            # a fresh checkout: compile the CUDA library once (nvcc, sm_100a); there is no CPU fallback to fall to
+            try:
+                from . import build
+                build.build_library()
+            except Exception as e:
+                raise ImportError("%s not found and building it failed (%s): run `python -m paper_1304_0597_b200.build`"
+                                  % (LIB_PATH, e))
         L = C.CDLL(LIB_PATH)
         vp, ll, i, u64 = C.c_void_p, C.c_longlong, C.c_int, C.c_uint64
         L.game_create.argtypes = [i, i, i, C.POINTER(vp)]
