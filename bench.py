@@ -2,12 +2,16 @@
 """bench.py -- GAME hot path on B200: chromosome x pattern fitness evaluations / second.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
+                  [--path auto|fp32|tensor|split] [--shard] [--no-cpu-baseline]
 
 A *step* is one generation of the whole hot path (fused fitness of every chromosome
 on every pattern, rank, stop test, elitism, selection, crossover, mutation) on the config's synthetic
 workload.  `game_evolve(K)` runs K such steps plus the final re-evaluation of the returned population
 (DESIGN G18); the timed region is exactly that call, so `value` counts (K+1)*N*P evaluations and
 `ms_per_step` = time / K (the final evaluation is charged to the steps).  Prints ONE JSON line.
+The default workload is config 5, the largest (the one north_star quotes its roofline target on); --config picks the
+others.  At N > 1 every rank runs its own replica (weak scaling); --shard splits ONE problem's patterns over the ranks
+instead (one all-reduce of P doubles per generation, strong scaling).
 
 --impl reference times the fp64 CPU oracle (oracle/, as it stands) on the box's host cores on a bounded
 sample of the same workload -- a deliberately slow baseline, not a target.
