@@ -591,3 +591,25 @@ def test_out_of_core_chunks(orc):
         fit32 = fit.astype(np.float32)
         nxt = orc.ga_step(gpo, seed, gen, orc.rank(fit32), fit32, pop)
         assert np.array_equal(ctx.get_population_host(want_fit=False)[0].view(np.uint32), nxt.view(np.uint32))
+
+
+@pytest.mark.parametrize("fam,d,F,P", [(2, 8, 11, 23), (2, 1, 11, 23), (3, 6, 11, 32), (CHEB, 3, 2, 5), (TRIG, 2, 3, 17)])
+@pytest.mark.parametrize("act,err,R", [(IDENTITY, TMSE, 0.49), (SIGMOID, MSE, 0.0)])
+def test_thin_models_many_patterns(orc, fam, d, F, P, act, err, R):
+    """Thin models on many patterns on the FP32 path (K <= 64 genes, P <= 32: the paper's Table 3 shapes), ragged N.
+    (A dedicated two-patterns-per-thread kernel for these shapes was measured slower than fitness_small_kernel --
+    2484 vs 2734 generations/s at 7e6 rows, degree 8 -- and dropped; the shapes stay covered here.)"""
+    rng = np.random.default_rng(47)
+    N = 70001
+    X = rng.uniform(-1, 1, (N, F)).astype(np.float32)
+    t = rng.integers(0, 2, N).astype(np.float32)
+    K = orc.num_terms(fam, d, F)
+    pop = (rng.uniform(-1, 1, (P, K)) / (np.sqrt(K) if act == IDENTITY else 1.0)).astype(np.float32)
+    if fam in (2, 3):
+        pop = (pop / F).astype(np.float32)               # tied terms are sums over F features
+    ctx = make_ctx(fam, d, X, t, act, err, R, g.GAME_PATH_FP32)
+    got = ctx.fitness(dev(pop)).cpu().numpy()
+    check_fitness(orc, got, fam, d, X, t, pop, act, err, R, g.GAME_PATH_FP32, "thin")
+    perm = rng.permutation(P)                             # P20: independent of the chromosome's position
+    got2 = ctx.fitness(dev(pop[perm])).cpu().numpy()
+    assert np.array_equal(got2.view(np.uint32), got[perm].view(np.uint32))
