@@ -144,7 +144,9 @@ int game_fitness_sums(game_ctx *ctx, const float *pop, int P, double *sums);
 int game_advance(game_ctx *ctx, const double *sums, long long N_total, unsigned long long seed, const game_ga_params *params,
                  int apply_operators, game_result *res);
 /* Forward pass of ONE chromosome (the paper's test / run use cases, L127-L129): z_out[n] = Out(pat_n),
- * y_out[n] = act(z).  genes: K fp32, z_out / y_out: N fp32, either may be NULL.  DEV pointers. fp32. */
+ * y_out[n] = act(z), over the patterns of the LOADED dataset -- to apply a trained chromosome to other data (a test or
+ * run set), game_load that data (into this or a second context of the same family / degree / F) and call this.
+ * genes: K fp32, z_out / y_out: N fp32, either may be NULL.  DEV pointers. fp32. */
 int game_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out);
 
 /* Figures of merit of a trained chromosome on the loaded dataset (L301).  A pattern is classified as class 1
