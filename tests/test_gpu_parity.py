@@ -613,3 +613,32 @@ def test_thin_models_many_patterns(orc, fam, d, F, P, act, err, R):
     perm = rng.permutation(P)                             # P20: independent of the chromosome's position
     got2 = ctx.fitness(dev(pop[perm])).cpu().numpy()
     assert np.array_equal(got2.view(np.uint32), got[perm].view(np.uint32))
+
+
+@pytest.mark.parametrize("cfg,N,P,path", [(1, None, None, g.GAME_PATH_AUTO), (2, None, 300, g.GAME_PATH_AUTO),
+                                          (3, 20000, 512, g.GAME_PATH_AUTO), (4, 30000, 200, g.GAME_PATH_AUTO),
+                                          (1, None, None, g.GAME_PATH_FP32)])
+def test_graph_loop_equals_stepwise(orc, cfg, N, P, path):
+    """game_evolve(G >= 8) on a capturable stream replays a CUDA graph of two generations (with the operators writing the
+    next evaluation's fp16 genes); it must give, bit for bit, what G single-generation calls on the default stream give."""
+    w = wl.config(cfg)
+    w = w.scaled(N=N or w.N, P=P or w.P, generations=21)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    gp = g.ga_params(P=w.P)
+    step = make_ctx(fam, d, X, t, w.act, w.err, w.R, path)
+    for _ in range(w.generations):
+        step.evolve(1, w.seed, gp)
+    ps, fs, os_ = step.get_population_host()
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        ctx = g.Game(fam, d, w.F, stream=stream)
+        ctx.set_activation(w.act)
+        ctx.set_error(w.err, w.R)
+        ctx.set_path(path)
+        ctx.load(dev(X), dev(t))
+        res = ctx.evolve(w.generations, w.seed, gp)
+        pg, fg, og = ctx.get_population_host()
+    assert res.generations_run == w.generations
+    assert np.array_equal(pg.view(np.uint32), ps.view(np.uint32))
+    assert np.array_equal(fg.view(np.uint32), fs.view(np.uint32)) and np.array_equal(og, os_)
