@@ -90,9 +90,9 @@ int game_set_error(game_ctx *ctx, int err_type, float tmse_R);   /* default MSE;
  *   GAME_PATH_TENSOR_SPLIT  tensor cores on split operands: E and the genes are each an fp16 hi + lo pair and the three
  *                           products hi.hi + hi.lo + lo.hi run as one fp16 contraction over 3K terms, fp32 accumulate,
  *                           ex2 + rcp logistic: the FP32 path's class (1e-5 |exact| + 1e-7; measured 3e-7 .. 9e-7).
- *                           Per-feature families with max|E| <= 2;
+ *                           Per-feature families with max|E| <= 1024;
  *   GAME_PATH_AUTO          (default) N >= 16384: TENSOR;  smaller datasets: TENSOR_SPLIT;  FP32 where the tensor paths'
- *                           conditions fail (tied families, max|E| > 2). */
+ *                           conditions fail (tied families, large |E|). */
 int game_set_path(game_ctx *ctx, int path);
 /* Which path the next fitness call will take for population size P (one of the three above), or -1 if the requested
  * one is unavailable for the loaded dataset. */

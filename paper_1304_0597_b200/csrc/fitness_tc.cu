@@ -868,7 +868,8 @@ int tensor_prepare_split(game_ctx *ctx)
     int rc = launch_expand_split(ctx);
     if (rc) return rc;
     if (!ctx->tmap_Es) ctx->tmap_Es = aligned_alloc(64, 2 * sizeof(CUtensorMap));
-    if (!ctx->tmap_Es) return fail(ctx, GAME_ERR_ALLOC, "tensor map allocation failed");
+    if (!ctx->tmap_C) ctx->tmap_C = aligned_alloc(64, sizeof(CUtensorMap));           // (the TENSOR path may be unavailable)
+    if (!ctx->tmap_Es || !ctx->tmap_C) return fail(ctx, GAME_ERR_ALLOC, "tensor map allocation failed");
     for (int cg = 1; cg <= 2; ++cg) {
         rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_Es + (cg - 1), ctx->E16s, ctx->Npad256 * (3 * ctx->Kpad / BKB), BKB, BN / cg);
         if (rc) return rc;

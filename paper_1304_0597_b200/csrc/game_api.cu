@@ -43,7 +43,7 @@ static void dfree(T *&p)
 static void free_dataset(game_ctx *c)
 {
     dfree(c->X); dfree(c->t); dfree(c->ET); dfree(c->E16); dfree(c->E16s);
-    c->N = 0; c->tensor_ok = false;
+    c->N = 0; c->tensor_ok = false; c->split_ok = false;
 }
 
 static void free_population(game_ctx *c)
@@ -91,7 +91,7 @@ static int ensure_scratch(game_ctx *c, int P)
         GAME_CUDA(c, cudaMemsetAsync(c->C16, 0, need16 * sizeof(__half), c->stream));
         c->c16_cap = need16; c->c16_src = nullptr;
     }
-    if (c->tensor_ok && c->path != GAME_PATH_FP32 && c->path != GAME_PATH_TENSOR && 3 * need16 > c->c16s_cap) {   // AUTO or SPLIT may need it
+    if (c->split_ok && c->path != GAME_PATH_FP32 && c->path != GAME_PATH_TENSOR && 3 * need16 > c->c16s_cap) {   // AUTO or SPLIT may need it
         dfree(c->C16s);
         GAME_CUDA(c, cudaMalloc(&c->C16s, 3 * need16 * sizeof(__half)));
         GAME_CUDA(c, cudaMemsetAsync(c->C16s, 0, 3 * need16 * sizeof(__half), c->stream));
@@ -105,7 +105,7 @@ static int resolve_path(const game_ctx *c, int P)
     bool can_tensor = tensor_path_built() && c->tensor_ok;
     if (c->path == GAME_PATH_FP32) return GAME_PATH_FP32;
     if (c->path == GAME_PATH_TENSOR) return can_tensor ? GAME_PATH_TENSOR : -1;
-    const bool can_split = can_tensor && tc_permuted(c->family);
+    const bool can_split = tensor_path_built() && c->split_ok;
     if (c->path == GAME_PATH_TENSOR_SPLIT) return can_split ? GAME_PATH_TENSOR_SPLIT : -1;
     // AUTO: the tensor cores wherever they can be used -- measured on B200 they beat the FFMA kernels at every population
     // size down to P = 8 (N = 2e5, K = 544: 0.05 / 0.14 ms against 0.43 ms; config 1 in the loop: 60.6k against 48.5k
@@ -194,6 +194,9 @@ static int load_common(game_ctx *c, const float *X, const float *targets, long l
         // ... and the tile-blocked expansion is addressed with 32-bit TMA row coordinates (the split form has 3x the rows)
         const bool rows_ok = (double)c->Npad256 * (3.0 * c->Kpad / TC_KBLK) < 2147483647.0;
         c->tensor_ok = mx <= 2.0f && rows_ok;
+        // the split form keeps ~22 bits of every value whatever its magnitude (hi + lo), so it only needs the values well
+        // inside fp16's range and above its subnormals' grain: |E| <= 1024 (e.g. Chebyshev terms of unnormalised features)
+        c->split_ok = mx <= 1024.0f && rows_ok && tc_permuted(c->family);
         if (c->tensor_ok) {
             rc = tensor_prepare(c);
             if (rc) return rc;

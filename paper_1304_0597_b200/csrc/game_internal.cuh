@@ -120,7 +120,8 @@ struct game_ctx {
     __half *E16s = nullptr;    // Npad256 x 3 Kpad fp16: [hi | hi | lo] halves of E (TENSOR_SPLIT path), built on first use
     long long Npad256 = 0;
     int Kpad = 0;              // K rounded up to TC_KBLK
-    bool tensor_ok = false;    // E16 built and all |E| representable
+    bool tensor_ok = false;    // E16 built and all |E| <= 2 (TENSOR path)
+    bool split_ok = false;     // |E| within the range where the fp16 hi + lo split is exact enough (TENSOR_SPLIT path)
     float x_maxabs = 0.f;      // max |X| of the loaded dataset
 
     // population / loop state

@@ -642,3 +642,24 @@ def test_graph_loop_equals_stepwise(orc, cfg, N, P, path):
     assert res.generations_run == w.generations
     assert np.array_equal(pg.view(np.uint32), ps.view(np.uint32))
     assert np.array_equal(fg.view(np.uint32), fs.view(np.uint32)) and np.array_equal(og, os_)
+
+
+def test_split_path_beyond_unit_range(orc):
+    """Features outside [-1, 1] make Chebyshev terms large (|T_3(1.6)| = 11.6): the one-pass fp16 path is withdrawn
+    (max|E| > 2) but the split path keeps ~22 bits of every value and still meets the FP32 tolerance class."""
+    rng = np.random.default_rng(53)
+    fam, d, F, N, P = CHEB, 3, 6, 3000, 40
+    X = rng.uniform(-1.6, 1.6, (N, F)).astype(np.float32)
+    t = rng.integers(0, 2, N).astype(np.float32)
+    K = orc.num_terms(fam, d, F)
+    pop = (rng.uniform(-1, 1, (P, K)) / 8).astype(np.float32)
+    ctx = make_ctx(fam, d, X, t, SIGMOID, MSE, 0.0)
+    assert ctx.resolved_path(P) == g.GAME_PATH_TENSOR_SPLIT
+    ctx.set_path(g.GAME_PATH_TENSOR)
+    assert ctx.resolved_path(P) == -1
+    ctx.set_path(g.GAME_PATH_AUTO)
+    got = ctx.fitness(dev(pop)).cpu().numpy()
+    check_fitness(orc, got, fam, d, X, t, pop, SIGMOID, MSE, 0.0, g.GAME_PATH_TENSOR_SPLIT, "split, |E| up to 11.6")
+    ctx.set_activation(IDENTITY)
+    got = ctx.fitness(dev(pop)).cpu().numpy()
+    check_fitness(orc, got, fam, d, X, t, pop, IDENTITY, MSE, 0.0, g.GAME_PATH_TENSOR_SPLIT, "split identity")
