@@ -343,7 +343,8 @@ def run_ours(args, w):
     else:
         peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
         roof = {"bound": "alu", "achieved": flops / avg_s / 1e12, "peak": peak, "unit": "TFLOP/s",
-                "peak_source": "148 SM x 128 FFMA lanes x 2 flop x sm_max_mhz (derived, DESIGN.md section 7)"}
+                "peak_source": "148 SM x 128 FFMA lanes x 2 flop x sm_max_mhz (derived; a register-only FFMA micro-benchmark on B200 "
+                               "reaches 72.5 TFLOP/s = 97 % of it; DESIGN.md section 7)"}
     if path == g.GAME_PATH_TENSOR_SPLIT:
         roof["executed_over_algorithmic"] = {"tensor_flops": 3, "mufu_ops": 2}
     roof["frac"] = roof["achieved"] / roof["peak"]
