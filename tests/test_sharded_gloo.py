@@ -81,6 +81,19 @@ def test_shard_rows_partition():
         sharded.shard_rows(10, 2, 2)
 
 
+def test_chunk_ranges():
+    from paper_1304_0597_b200 import sharded
+    import numpy as np
+    X = np.zeros((10, 2), np.float32)
+    t = np.zeros(10, np.float32)
+    cg = sharded.ChunkedGame(None, X, t, 4)
+    assert cg.chunks() == [(0, 4), (4, 8), (8, 10)] and cg.N_total == 10
+    assert sharded.ChunkedGame(None, X, t, 10).chunks() == [(0, 10)]
+    assert sharded.ChunkedGame(None, X, t, 99).chunks() == [(0, 10)]
+    with pytest.raises(ValueError):
+        sharded.ChunkedGame(None, X, t, 0)
+
+
 def test_single_rank_loop_calls():
     from paper_1304_0597_b200 import sharded
     calls = []
