@@ -23,8 +23,12 @@
  * the identity+MSE case, least squares optimum, planted chromosome, tied-gene reduction
  * (eq. 9 as printed), row replication (L326), hand-written brute force, Philox against
  * torch's ATen philox_engine, tournament closed-form distribution, crossover / mutation /
- * elitism invariants.  Parity unpinned: roulette weight formula R4 (DESIGN G14) -- the paper
- * gives none; only its self-consistency (frequencies ~ weights) is tested.
+ * elitism invariants; exact hand-worked values (rational arithmetic, ATen's Philox words) for
+ * interior roulette weights and the normal-mode initial gene (tests/test_oracle_exact_pins.py);
+ * the whole pin suite also runs against an -fsanitize=address,undefined build
+ * (tests/test_oracle_sanitized.py).  The roulette weight RULE R4 (DESIGN G14) is this build's
+ * choice -- the paper gives none ("parity unpinned" against the paper); its implementation here
+ * is pinned exactly to that rule.
  *
  * Build: gcc -O2 -fopenmp -shared -fPIC -o libgame_oracle.so game_oracle.c -lm
  */

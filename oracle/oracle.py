@@ -10,7 +10,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "game_oracle.c")
-_LIB = os.path.join(_HERE, "libgame_oracle.so")
+# GAME_ORACLE_SANITIZE=1 (set by tests/test_oracle_sanitized.py for its child pytest): the same source built with
+# -fsanitize=address,undefined -O1 -g into a separate library; the child process preloads the sanitizer runtimes
+_SANITIZE = os.environ.get("GAME_ORACLE_SANITIZE") == "1"
+_LIB = os.path.join(_HERE, "libgame_oracle_san.so" if _SANITIZE else "libgame_oracle.so")
 
 TRIG, CHEB, TRIG_TIED, POLY_TIED = 0, 1, 2, 3
 SIGMOID, IDENTITY = 0, 1
@@ -35,7 +38,9 @@ def build(force=False):
     """Compile the oracle with gcc (-O2, OpenMP). Building the checker is not using it."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".tmp.%d" % os.getpid()
-        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC",
+        opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+               "-fno-omit-frame-pointer"] if _SANITIZE else ["-O2"]
+        subprocess.check_call(["gcc"] + opt + ["-fopenmp", "-ffp-contract=off", "-shared", "-fPIC",
                                "-o", tmp, _SRC, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB

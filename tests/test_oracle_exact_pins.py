@@ -1,0 +1,171 @@
+"""Exact hand-worked pins for the two oracle rules the paper does not fix:
+
+  P23b  oracle_roulette_weights at INTERIOR fitness values (DESIGN G14 / R4): w_r = trunc(fl32(fl32(f_max - f_r) /
+        fl32(f_max - f_min)) * 2^24) + 1, every step one IEEE fp32 operation.
+  P16b  oracle_init_gene, GAME_INIT_NORMAL_PM1 (DESIGN G13 / R2): S = sum of the top 24 bits of the 12 Philox words of
+        counters (k, p, j, TAG_INIT), j = 0..2; gene = clamp(fl32(fl32(S - 6 (2^24 - 1)) * fl32(2^-24 / 3)), -1, 1).
+
+The expected values are derived here in exact rational arithmetic (fractions.Fraction) with an integer implementation
+of round-to-nearest-even to 24 significant bits -- no numpy/C float operation of the kind the oracle uses -- and the
+Philox words come from torch's ATen engine (an independent library implementation), not from the oracle's.  The
+literal numbers in the first test were additionally worked on paper; the derivation is in the comments.
+"""
+import ctypes
+import os
+import subprocess
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+
+def fl32(x):
+    """Round a non-negative or negative rational to the nearest fp32 (ties to even), normal range only; exact Fraction."""
+    x = Fraction(x)
+    if x == 0:
+        return x
+    s = -1 if x < 0 else 1
+    x = abs(x)
+    e = 0
+    while x >= 2:
+        x /= 2
+        e += 1
+    while x < 1:
+        x *= 2
+        e -= 1
+    m = x * (1 << 23)                       # significand in [2^23, 2^24)
+    lo = m.numerator // m.denominator
+    rem = m - lo
+    if rem > Fraction(1, 2) or (rem == Fraction(1, 2) and (lo & 1)):
+        lo += 1
+    return s * Fraction(lo, 1 << 23) * Fraction(2) ** e
+
+
+def as_f32(fr):
+    v = np.float32(float(fr))
+    assert Fraction(float(v)) == fr, "not representable in fp32"
+    return v
+
+
+def weight_by_hand(f, fmax, fmin):
+    a = fl32(Fraction(float(fmax)) - Fraction(float(f)))
+    b = fl32(Fraction(float(fmax)) - Fraction(float(fmin)))
+    q = fl32(a / b)
+    scaled = q * (1 << 24)                  # exact: a power-of-two scale
+    return scaled.numerator // scaled.denominator + 1
+
+
+def test_p23b_roulette_interior_weights_by_hand(orc):
+    f32 = np.float32
+    # Case A (worked on paper): fits 0.1f, 0.5f, 0.9f.  0.9f = 15099494 * 2^-24, 0.1f = 13421773 * 2^-27, 0.5 exact.
+    #   b = fl32(0.9f - 0.1f): exact difference 107374179 * 2^-27 needs 27 bits; in [0.5, 1) the grain is 2^-24 = 8 units:
+    #       107374179 / 8 = 13421772.375 -> 13421772 * 2^-24.
+    #   a = 0.9f - 0.5 = 6710886 * 2^-24 (exact).  q = 6710886 / 13421772 = 1/2 exactly.  w = 2^23 + 1 = 8388609.
+    fit = np.array([0.1, 0.5, 0.9], dtype=f32)
+    w = orc.roulette_weights(fit, orc.rank(fit))
+    assert w.tolist() == [2**24 + 1, 8388609, 1]
+    assert weight_by_hand(fit[1], fit[2], fit[0]) == 8388609
+    # Case B: fits 0.25, 0.5, 1.0: q = fl32(0.5 / 0.75) = fl32(2/3) = 11184811 * 2^-24 (0xAAAAAB) -> w = 11184812
+    fit = np.array([0.25, 0.5, 1.0], dtype=f32)
+    w = orc.roulette_weights(fit, orc.rank(fit))
+    assert w.tolist() == [2**24 + 1, 11184812, 1]
+    # Case C (truncation matters): fits 0, 0.7f, 3.0: a = fl32(3 - 0.7f); 0.7f = 11744051 * 2^-24, 3 - 0.7f =
+    #   38587597 * 2^-24 -> grain 2^-22 in [2, 4): 9646899.25 -> 9646899 * 2^-22; q = fl32(a / 3) = 3215633 * 2^-22
+    #   (9646899 = 3 * 3215633), 24-bit exact; w = 3215633 * 4 + 1 = 12862533.
+    fit = np.array([0.0, 0.7, 3.0], dtype=f32)
+    w = orc.roulette_weights(fit, orc.rank(fit))
+    assert w.tolist() == [2**24 + 1, 12862533, 1]
+    assert weight_by_hand(fit[1], fit[2], fit[0]) == 12862533
+    # Case D: a sweep of interior values whose quotient falls below 1/2 (finer grain than 2^-24, so the floor really
+    # truncates), in a shuffled population with a NaN; every weight against the rational derivation
+    rng = np.random.default_rng(61)
+    fit = rng.random(200).astype(f32) * f32(3.7) + f32(0.01)
+    fit[17] = np.nan
+    order = orc.rank(fit)
+    w = orc.roulette_weights(fit, order)
+    finite = fit[np.isfinite(fit)]
+    fmax, fmin = finite.max(), finite.min()
+    truncated = 0
+    for r, p in enumerate(order):
+        if not np.isfinite(fit[p]):
+            assert w[r] == 0
+            continue
+        exp = weight_by_hand(fit[p], fmax, fmin)
+        assert int(w[r]) == exp, (r, p, float(fit[p]))
+        q = fl32(fl32(Fraction(float(fmax)) - Fraction(float(fit[p]))) / fl32(Fraction(float(fmax)) - Fraction(float(fmin))))
+        truncated += (q * (1 << 24)).denominator != 1
+    assert truncated > 20                   # the floor was exercised, not only exact scalings
+
+
+# ---- P16b: one init gene from ATen's Philox words ---------------------------------------------------------------
+_SHIM = r"""
+#include <ATen/core/PhiloxRNGEngine.h>
+extern "C" void aten_philox(unsigned long long seed, unsigned long long subseq,
+                            unsigned long long offset, unsigned int *out) {
+    at::Philox4_32 eng(seed, subseq, offset);   // counter = (offset lo, offset hi, subseq lo, subseq hi)
+    for (int i = 0; i < 4; ++i) out[i] = eng();
+}
+"""
+
+
+@pytest.fixture(scope="module")
+def aten_words(tmp_path_factory):
+    torch = pytest.importorskip("torch")
+    inc = os.path.join(os.path.dirname(torch.__file__), "include")
+    d = tmp_path_factory.mktemp("aten_philox_pins")
+    src = d / "shim.cpp"
+    src.write_text(_SHIM)
+    so = d / "shim.so"
+    subprocess.check_call(["g++", "-O1", "-std=c++17", "-shared", "-fPIC", "-I", inc, "-o", str(so), str(src)])
+    L = ctypes.CDLL(str(so))
+
+    def words(seed, c0, c1, c2, c3):
+        out = (ctypes.c_uint32 * 4)()
+        L.aten_philox(ctypes.c_uint64(seed), ctypes.c_uint64(c2 | (c3 << 32)), ctypes.c_uint64(c0 | (c1 << 32)), out)
+        return [int(v) for v in out]
+    return words
+
+
+def init_gene_by_hand(words12):
+    S = sum(w >> 8 for w in words12)                     # twelve 24-bit integers
+    assert S < 2**32
+    v = fl32(S - 6 * (2**24 - 1))                        # int32 -> fp32 conversion rounds to nearest even
+    c = fl32(Fraction(1, 3 * 2**24))                     # fl(2^-24 / 3) = 0x1.555556p-26
+    assert c == Fraction(0x1555556, 1 << 24) / (1 << 26)
+    g = fl32(v * c)                                      # one IEEE multiply
+    return max(Fraction(-1), min(Fraction(1), g))
+
+
+def test_p16b_init_normal_gene_by_hand(orc, aten_words):
+    TAG_INIT = 0
+    clamped = 0
+    cases = [(1, 0, 0), (1, 19, 98), (0xABCDEF0123456789, 332, 7), (5, 8191, 831), (2**64 - 1, 3, 5)]
+    rng = np.random.default_rng(62)
+    cases += [(int(rng.integers(0, 2**62)), int(rng.integers(0, 8192)), int(rng.integers(0, 832))) for _ in range(300)]
+    for seed, p, k in cases:
+        w12 = []
+        for j in range(3):
+            w12 += aten_words(seed, k, p, j, TAG_INIT)
+        exp = init_gene_by_hand(w12)
+        got = np.float32(orc.lib().oracle_init_gene(1, ctypes.c_uint64(seed), p, k))
+        assert Fraction(float(got)) == exp, (seed, p, k, float(got), float(exp))
+        clamped += abs(exp) == 1
+    # an off-by-one in the centring constant 6 (2^24 - 1) would move every gene by fl(2^-24/3): caught above since the
+    # comparison is exact.  The uniform modes from the same words (R1): first word of counter (k, p, 0, TAG_INIT)
+    for seed, p, k in cases[:40]:
+        w = aten_words(seed, k, p, 0, TAG_INIT)[0]
+        u = np.float32(orc.lib().oracle_init_gene(0, ctypes.c_uint64(seed), p, k))
+        v = np.float32(orc.lib().oracle_init_gene(2, ctypes.c_uint64(seed), p, k))
+        assert Fraction(float(u)) == Fraction((w >> 8) - 2**23, 2**23)
+        assert Fraction(float(v)) == Fraction(w >> 8, 2**24)
+
+
+def test_fl32_helper_is_ieee():
+    """The rational rounding helper itself, against the textbook cases (so the pins above do not rest on a bug in it)."""
+    assert fl32(Fraction(1, 3)) == Fraction(11184811, 1 << 25)            # 0x1.555556p-2
+    assert fl32(Fraction(2, 3)) == Fraction(11184811, 1 << 24)
+    assert fl32(Fraction(1, 10)) == Fraction(13421773, 1 << 27)           # 0.1f
+    assert fl32(1 + Fraction(1, 1 << 24)) == 1                            # tie -> even
+    assert fl32(1 + Fraction(3, 1 << 24)) == 1 + Fraction(1, 1 << 22)     # tie -> even (up)
+    assert fl32(-Fraction(7, 10)) == -Fraction(11744051, 1 << 24)
+    assert fl32(16777217) == 16777216 and fl32(16777219) == 16777220
