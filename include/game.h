@@ -10,8 +10,11 @@
  *
  * Conventions
  *  - Every function returns 0 (GAME_OK) or a positive error code; game_last_error() gives the text.
- *    No exceptions, no exit(), no global state, no CPU fallback: without a CUDA device every
- *    compute call fails with GAME_ERR_CUDA.
+ *    No exceptions, no exit(), no global state (no environment variables are read; every setting lives
+ *    in the context), no CPU fallback: without a CUDA device every compute call fails with GAME_ERR_CUDA.
+ *  - A context belongs to the CUDA device that was current when game_create ran; every call makes that
+ *    device current for its duration and restores the caller's, so contexts on several GPUs can be
+ *    driven from one thread.
  *  - Pointer arguments are marked DEV (CUDA device memory, caller-owned, must stay valid until the
  *    context's stream has consumed them) or HOST (ordinary or pinned host memory).  The library
  *    never frees or keeps caller memory; game_load* copies / re-lays what it needs.
@@ -46,6 +49,20 @@ enum { GAME_ELITE_COPIES_OF_BEST = 0, GAME_ELITE_TOP_E = 1 };      /* L148; DESI
  * fp32-accumulate MMA (same 11-bit significand as TF32), 1e-3 class.  AUTO picks by problem shape. */
 enum { GAME_PATH_AUTO = 0, GAME_PATH_FP32 = 1, GAME_PATH_TENSOR = 2, GAME_PATH_TENSOR_SPLIT = 3 };
 enum { GAME_EXPAND_AUTO = 0, GAME_EXPAND_MATERIALIZED = 1, GAME_EXPAND_REGENERATED = 2 };
+/* Launch-configuration knobs of game_set_tuning: measurement aids, none changes what is computed beyond the stated
+ * tolerance class.  value -1 restores the automatic choice.
+ *   GAME_TUNE_PDL          1/0  programmatic dependent launch between the kernels of a generation (auto: 1)
+ *   GAME_TUNE_CTA_GROUP    1/2  single CTAs or cta_group::2 pairs in the tensor kernel (auto: by shape)
+ *   GAME_TUNE_SIGMOID      0 ex2+rcp logistic, 2 tanh.approx logistic, 3 tanh.approx with a share of the evaluations
+ *                          on an FMA-pipe polynomial (TENSOR path; auto: by shape)
+ *   GAME_TUNE_RESIDENT     1/0  resident population tile for P <= 256 (auto: 1)
+ *   GAME_TUNE_TEAMS        1/0  two-team epilogue (auto: contraction depth <= 256)
+ *   GAME_TUNE_HALF_TILES   1/0  128-pattern tiles for sub-wave problems (auto: by shape)
+ *   GAME_TUNE_PERSISTENT   1/0  one persistent cooperative kernel per game_evolve for sub-wave problems (auto: by shape)
+ *   GAME_TUNE_POLY_SHARE   0..16  of every 16 logistic evaluations, how many go to the FMA-pipe polynomial in sigmoid
+ *                          mode 3 (auto: measured best) */
+enum { GAME_TUNE_PDL = 0, GAME_TUNE_CTA_GROUP = 1, GAME_TUNE_SIGMOID = 2, GAME_TUNE_RESIDENT = 3, GAME_TUNE_TEAMS = 4,
+       GAME_TUNE_HALF_TILES = 5, GAME_TUNE_PERSISTENT = 6, GAME_TUNE_POLY_SHARE = 7, GAME_TUNE_COUNT_ = 8 };
 
 /* GA parameters (L275-L291).  Probabilities are per parent pair (crossover, DESIGN G15) and per gene
  * (mutation, DESIGN G16).  stop_error < 0 disables the error-threshold stop (L219, L287). */
@@ -109,6 +126,11 @@ int game_resolved_path(const game_ctx *ctx, int P);
  * requested one is unavailable. */
 int game_set_expansion(game_ctx *ctx, int mode);
 int game_resolved_expansion(const game_ctx *ctx, int P);
+/* Launch-configuration knob (GAME_TUNE_*), per context; unknown knobs / values give GAME_ERR_INVALID_ARG. */
+int game_set_tuning(game_ctx *ctx, int knob, int value);
+/* Pattern-sharded runs: the number of patterns of the WHOLE problem (all shards).  GAME_PATH_AUTO then picks the path from
+ * it instead of this context's own N, so every shard evaluates in the same tolerance class.  0 = unset. */
+int game_set_global_patterns(game_ctx *ctx, long long N_total);
 
 /* a0 + a1: load the dataset and expand it (L254: "calculate the time consuming trigonometric functions
  * only once").  X is N x F row-major fp32, targets N fp32.  Builds the device-resident expansion
@@ -134,20 +156,36 @@ int game_fitness_host(game_ctx *ctx, const float *pop, int P, float *out);
  * shards (one all-reduce of P doubles per generation) before eq. 4's mean is taken.
  * game_fitness_sums: a1-a5 without the mean: sums[p] = sum over THIS context's patterns of e (eq. 3 / eq. 10), fp64,
  *   in a fixed order.  pop DEV P x K (or NULL: the context's own population, P ignored), sums DEV P doubles.
- *   Asynchronous on the context's stream.
+ *   accumulate != 0: sums[p] += this context's totals (out-of-core evaluation: the chunks of one dataset pass through
+ *   the context one after the other and their totals add up in the library, in call order).  Asynchronous on the
+ *   context's stream.
  * game_advance: the rest of one generation from the (summed) totals: fit = sums / N_total (root for RMSE), rank (a6),
  *   stop test (a7) and, if apply_operators != 0 and the stop test did not fire, a8-a11 on the context's population
  *   (generation counter + 1).  Every shard calls it with the same totals, seed and parameters and so holds the same
  *   population afterwards, bit for bit (the random numbers are counter-based).  With one shard and N_total = N it
- *   reproduces game_evolve(1) exactly.  sums DEV P doubles; res HOST; synchronises the stream. */
-int game_fitness_sums(game_ctx *ctx, const float *pop, int P, double *sums);
+ *   reproduces game_evolve(1) exactly.  sums DEV P doubles.
+ *   res != NULL (HOST): synchronises the stream and reports this call (and any asynchronous ones before it).
+ *   res == NULL: ASYNCHRONOUS -- nothing waits on the host; the generation counter and the stop flag live on the device
+ *   (once the stop test has fired, later asynchronous calls leave the population unchanged), and game_sync collects them.
+ * game_sync: synchronises the stream and closes a run of asynchronous game_advance calls: res (HOST, may be NULL) gets
+ *   the generations applied since the run began, whether the stop test fired, and the best error / index of the last
+ *   evaluation.  Every other call that needs the host-side generation counter does this implicitly. */
+int game_fitness_sums(game_ctx *ctx, const float *pop, int P, double *sums, int accumulate);
 int game_advance(game_ctx *ctx, const double *sums, long long N_total, unsigned long long seed, const game_ga_params *params,
                  int apply_operators, game_result *res);
+int game_sync(game_ctx *ctx, game_result *res);
 /* Forward pass of ONE chromosome (the paper's test / run use cases, L127-L129): z_out[n] = Out(pat_n),
  * y_out[n] = act(z), over the patterns of the LOADED dataset -- to apply a trained chromosome to other data (a test or
  * run set), game_load that data (into this or a second context of the same family / degree / F) and call this.
  * genes: K fp32, z_out / y_out: N fp32, either may be NULL.  DEV pointers. fp32. */
 int game_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out);
+/* The same forward pass on CALLER-SUPPLIED patterns (a trained chromosome applied to a test / run
+ * set, L127-L129) without a game_load: X_new is N_new x F row-major fp32 (DEV), expanded on the fly (a1: fp64 term,
+ * rounded once to fp32 -- the values game_load would store), z accumulated in fp32 in ascending gene order, so the
+ * result equals game_load(X_new) + game_predict bit for bit.  No dataset needs to be loaded; the loaded one, if any,
+ * is untouched.  genes K fp32, z_out / y_out N_new fp32 (either may be NULL), all DEV.  Rejects nothing: a NaN
+ * feature gives a NaN output for that pattern.  Asynchronous. */
+int game_predict_new(game_ctx *ctx, const float *genes, const float *X_new, long long N_new, float *z_out, float *y_out);
 
 /* Figures of merit of a trained chromosome on the loaded dataset (L301).  A pattern is classified as class 1
  * when act(z) > cut and belongs to class 1 when its target > 0.5.  counts (DEV, 4 x int64) = {TP, FP, TN, FN};
@@ -155,8 +193,15 @@ int game_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out);
  * empty denominator.  genes: K fp32 DEV.  fp32 forward pass.  Asynchronous. */
 int game_classify(game_ctx *ctx, const float *genes, float cut, long long *counts, double *fom);
 
-/* Install a population (P x K fp32, DEV) instead of the random initial one; resets nothing else. */
+/* Install a population (P x K fp32, DEV) instead of the random initial one; resets nothing else.  Measures max|gene|
+ * (synchronises the stream): NaN / Inf genes are rejected with GAME_ERR_NONFINITE_INPUT; a population with
+ * |gene| > 65504 cannot be an fp16 operand, so GAME_PATH_AUTO evaluates it on the FP32 path and an explicitly requested
+ * tensor path fails with GAME_ERR_UNSUPPORTED (nothing is clamped silently).  game_fitness on a caller-supplied
+ * population is asynchronous and cannot reject: there a chromosome holding such a gene evaluates to NaN on the tensor
+ * paths (and ranks last); game_fitness_host checks and returns GAME_ERR_UNSUPPORTED. */
 int game_set_population(game_ctx *ctx, const float *pop, int P);
+/* Number of chromosomes of the installed / evolved population, 0 if there is none yet. */
+int game_population_size(const game_ctx *ctx);
 /* Set the absolute generation counter (checkpoint resume; Philox draws are keyed on it). */
 int game_set_generation(game_ctx *ctx, long long generation);
 
@@ -197,9 +242,17 @@ long long game_launch_count(const game_ctx *ctx);
 /* Measurement aid: while enabled, every launch of the dominant kernel (the fused contraction +
  * epilogue of game_fitness / game_evolve) is bracketed by CUDA events on the context's stream.
  * game_get_kernel_timing synchronises the stream, returns the summed duration in milliseconds and the
- * number of launches since the last call, and resets both.  HOST out pointers. */
+ * number of launches since the last call, and resets both.  HOST out pointers.  While enabled, game_evolve
+ * issues its kernels one by one instead of replaying a captured CUDA graph (events cannot be timed inside one). */
 int game_set_kernel_timing(game_ctx *ctx, int enabled);
 int game_get_kernel_timing(game_ctx *ctx, double *total_ms, long long *launches);
+
+/* Measurement aid: register-only micro-benchmarks of the pipes the "alu" rooflines are quoted against, one
+ * CTA per SM, timed with CUDA events on the context's stream; synchronises.  kind = GAME_PEAK_*; param = FMA instructions
+ * per tanh for GAME_PEAK_TANH_MIX (0..8), ignored otherwise.  *ops_per_s (HOST) = fused multiply-adds (FFMA, FFMA2: count
+ * both lanes) or special-function results per second over the whole GPU; *ms (HOST, may be NULL) = the timed launch. */
+enum { GAME_PEAK_FFMA = 0, GAME_PEAK_FFMA2 = 1, GAME_PEAK_TANH = 2, GAME_PEAK_EX2 = 3, GAME_PEAK_TANH_MIX = 4 };
+int game_microbench(game_ctx *ctx, int kind, int param, double *ops_per_s, double *ms);
 
 #ifdef __cplusplus
 }

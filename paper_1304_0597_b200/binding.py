@@ -21,17 +21,21 @@ GAME_INIT_UNIFORM_PM1, GAME_INIT_NORMAL_PM1, GAME_INIT_UNIFORM_01 = 0, 1, 2
 GAME_ELITE_COPIES_OF_BEST, GAME_ELITE_TOP_E = 0, 1
 GAME_PATH_AUTO, GAME_PATH_FP32, GAME_PATH_TENSOR, GAME_PATH_TENSOR_SPLIT = 0, 1, 2, 3
 GAME_EXPAND_AUTO, GAME_EXPAND_MATERIALIZED, GAME_EXPAND_REGENERATED = 0, 1, 2
+(GAME_TUNE_PDL, GAME_TUNE_CTA_GROUP, GAME_TUNE_SIGMOID, GAME_TUNE_RESIDENT, GAME_TUNE_TEAMS, GAME_TUNE_HALF_TILES,
+ GAME_TUNE_PERSISTENT, GAME_TUNE_POLY_SHARE) = range(8)
+GAME_PEAK_FFMA, GAME_PEAK_FFMA2, GAME_PEAK_TANH, GAME_PEAK_EX2, GAME_PEAK_TANH_MIX = range(5)
 ERROR_NAMES = {1: "INVALID_ARG", 2: "NOT_LOADED", 3: "ALLOC", 4: "CUDA", 5: "UNSUPPORTED", 6: "NONFINITE_INPUT"}
 
 # every symbol include/game.h declares (tests check the library exports exactly these)
 SYMBOLS = [
     "game_create", "game_destroy", "game_num_terms", "game_generation", "game_last_error",
     "game_set_stream", "game_set_activation", "game_set_error", "game_set_path", "game_resolved_path",
-    "game_set_expansion", "game_resolved_expansion", "game_fitness_sums", "game_advance",
+    "game_set_expansion", "game_resolved_expansion", "game_fitness_sums", "game_advance", "game_sync",
+    "game_set_tuning", "game_set_global_patterns", "game_predict_new", "game_population_size",
     "game_load", "game_load_host", "game_fitness", "game_fitness_host", "game_predict", "game_classify",
     "game_set_population", "game_set_generation", "game_evolve", "game_get_population",
     "game_get_population_host", "game_rank", "game_ga_step", "game_init_population", "game_philox",
-    "game_launch_count", "game_set_kernel_timing", "game_get_kernel_timing",
+    "game_launch_count", "game_set_kernel_timing", "game_get_kernel_timing", "game_microbench",
 ]
 
 
@@ -84,8 +88,13 @@ def load_library():
         L.game_set_error.argtypes = [vp, i, C.c_float]
         L.game_set_path.argtypes = [vp, i]
         L.game_resolved_path.argtypes = [vp, i]
-        L.game_fitness_sums.argtypes = [vp, vp, i, vp]
+        L.game_fitness_sums.argtypes = [vp, vp, i, vp, i]
         L.game_advance.argtypes = [vp, vp, ll, u64, C.POINTER(game_ga_params), i, C.POINTER(game_result)]
+        L.game_sync.argtypes = [vp, C.POINTER(game_result)]
+        L.game_set_tuning.argtypes = [vp, i, i]
+        L.game_set_global_patterns.argtypes = [vp, ll]
+        L.game_predict_new.argtypes = [vp, vp, vp, ll, vp, vp]
+        L.game_population_size.argtypes = [vp]
         L.game_set_expansion.argtypes = [vp, i]
         L.game_resolved_expansion.argtypes = [vp, i]
         L.game_load.argtypes = [vp, vp, vp, ll]
@@ -105,6 +114,7 @@ def load_library():
         L.game_philox.argtypes = [vp, u64, vp, i, vp]
         L.game_set_kernel_timing.argtypes = [vp, i]
         L.game_get_kernel_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(ll)]
+        L.game_microbench.argtypes = [vp, i, i, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -182,6 +192,12 @@ class Game:
         self._ck(self._L.game_get_kernel_timing(self._h, C.byref(ms), C.byref(n)))
         return ms.value, int(n.value)
 
+    def microbench(self, kind, param=0):
+        """(ops per second over the whole GPU, milliseconds of the timed launch) of one GAME_PEAK_* micro-benchmark."""
+        ops, ms = C.c_double(0.0), C.c_double(0.0)
+        self._ck(self._L.game_microbench(self._h, kind, param, C.byref(ops), C.byref(ms)))
+        return ops.value, ms.value
+
     def set_stream(self, stream):
         self.stream = stream
         self._ck(self._L.game_set_stream(self._h, C.c_void_p(stream.cuda_stream)))
@@ -195,22 +211,49 @@ class Game:
     def set_path(self, path):
         self._ck(self._L.game_set_path(self._h, path))
 
-    def fitness_sums(self, pop=None, P=0, out=None):
-        """Per-chromosome fp64 error totals over this context's patterns (pop None: the context's own population of P)."""
+    def fitness_sums(self, pop=None, P=0, out=None, accumulate=False):
+        """Per-chromosome fp64 error totals over this context's patterns (pop None: the context's own population of P);
+        accumulate: add them to `out` inside the library (out-of-core chunks)."""
         t = self._torch
         if pop is not None:
             P = pop.shape[0]
             assert pop.shape == (P, self.K)
         if out is None:
+            if accumulate:
+                raise ValueError("accumulate needs the buffer to add to")
             out = t.empty(P, dtype=t.float64, device="cuda")
-        self._ck(self._L.game_fitness_sums(self._h, _dev(pop, t.float32), P, _dev(out, t.float64)))
+        self._ck(self._L.game_fitness_sums(self._h, _dev(pop, t.float32), P, _dev(out, t.float64), 1 if accumulate else 0))
         return out
 
-    def advance(self, sums, N_total, seed, params, apply_operators=True):
-        res = game_result()
+    def advance(self, sums, N_total, seed, params, apply_operators=True, sync=True):
+        """sync=False: asynchronous (res == NULL in the C call); collect with sync()."""
+        res = game_result() if sync else None
         self._ck(self._L.game_advance(self._h, _dev(sums, self._torch.float64), N_total, seed, C.byref(params),
-                                      1 if apply_operators else 0, C.byref(res)))
+                                      1 if apply_operators else 0, C.byref(res) if sync else None))
         return res
+
+    def sync(self):
+        res = game_result()
+        self._ck(self._L.game_sync(self._h, C.byref(res)))
+        return res
+
+    def set_tuning(self, knob, value):
+        self._ck(self._L.game_set_tuning(self._h, knob, value))
+
+    def set_global_patterns(self, N_total):
+        self._ck(self._L.game_set_global_patterns(self._h, N_total))
+
+    def population_size(self):
+        return int(self._L.game_population_size(self._h))
+
+    def predict_new(self, genes, X_new, want_z=True, want_y=True):
+        t = self._torch
+        N = X_new.shape[0]
+        assert X_new.shape == (N, self.F)
+        z = t.empty(N, dtype=t.float32, device=genes.device) if want_z else None
+        y = t.empty(N, dtype=t.float32, device=genes.device) if want_y else None
+        self._ck(self._L.game_predict_new(self._h, _dev(genes, t.float32), _dev(X_new, t.float32), N, _dev(z), _dev(y)))
+        return z, y
 
     def set_expansion(self, mode):
         self._ck(self._L.game_set_expansion(self._h, mode))

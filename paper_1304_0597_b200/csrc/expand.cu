@@ -32,6 +32,30 @@ int launch_check_finite(game_ctx *ctx, const float *X, long long nX, const float
     return GAME_OK;
 }
 
+// flag2[0] |= 1 when v holds a NaN/Inf; flag2[1] = max |v| over the finite values, as float bits (game_set_population,
+// game_fitness_host: is every gene inside the fp16 range the tensor paths need?)
+__global__ void max_abs_kernel(const float *__restrict__ v, long long n, int *flag2)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    bool bad = false;
+    float mx = 0.f;
+    for (long long j = i; j < n; j += stride) { const float x = v[j]; if (isfinite(x)) mx = fmaxf(mx, fabsf(x)); else bad = true; }
+    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(flag2, 1);
+    for (int o = 16; o; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if ((threadIdx.x & 31) == 0 && mx > 0.f) atomicMax(flag2 + 1, __float_as_int(mx));
+}
+
+int launch_max_abs(game_ctx *ctx, const float *v, long long n, int *flag2_dev)
+{
+    int blocks = (int)((n + 255) / 256);
+    if (blocks > ctx->sm_count * 8) blocks = ctx->sm_count * 8;
+    if (blocks < 1) blocks = 1;
+    max_abs_kernel<<<blocks, 256, 0, ctx->stream>>>(v, n, flag2_dev);
+    GAME_LAUNCHED(ctx);
+    return GAME_OK;
+}
+
 // One thread per (feature i, pattern n); n is the fastest thread index so the term-major stores
 // ET[k][n] are coalesced.  Term index k = i*B + m, block order [1, cos 1..d, sin 1..d] / [T_0..T_d].
 // split != 0 (TENSOR_SPLIT path): E is written as three fp16 k-ranges [hi | hi | lo] of ld/3 positions each, hi = fp16(E),
@@ -151,6 +175,20 @@ int launch_expand_fp32(game_ctx *ctx)
     return GAME_OK;
 }
 
+// The fp32 term-major expansion serves the FFMA kernels, game_predict and game_classify only; the tensor paths never
+// read it.  It is therefore built on first use (config 4: 2.2 GB and one fp64 sincos per term that a run on the tensor
+// path never needs; the out-of-core driver reloads a chunk per generation and would pay it every time).
+int ensure_ET(game_ctx *ctx)
+{
+    if (ctx->ET) return GAME_OK;
+    const size_t bytes = (size_t)ctx->K * ctx->Npad * sizeof(float);
+    GAME_CUDA(ctx, cudaMalloc(&ctx->ET, bytes));
+    cudaError_t e = cudaMemsetAsync(ctx->ET, 0, bytes, ctx->stream);
+    int rc = e == cudaSuccess ? launch_expand_fp32(ctx) : cuda_fail(ctx, e, "cudaMemsetAsync(ET)");
+    if (rc) { cudaFree(ctx->ET); ctx->ET = nullptr; }
+    return rc;
+}
+
 int launch_expand_split(game_ctx *ctx)
 {
     dim3 grid((unsigned)((ctx->N + 255) / 256), (unsigned)ctx->F);
@@ -228,6 +266,8 @@ __global__ void classify_kernel(const float *__restrict__ ET, long long Npad, lo
 
 int launch_classify(game_ctx *ctx, const float *genes, float cut, long long *counts, double *fom, unsigned int *ticket)
 {
+    int rce = ensure_ET(ctx);
+    if (rce) return rce;
     GAME_CUDA(ctx, cudaMemsetAsync(counts, 0, 4 * sizeof(long long), ctx->stream));
     int blocks = (int)((ctx->N + 255) / 256);
     classify_kernel<<<blocks, 256, ctx->K * sizeof(float), ctx->stream>>>(ctx->ET, ctx->Npad, ctx->N, ctx->K, genes, ctx->t,
@@ -239,9 +279,84 @@ int launch_classify(game_ctx *ctx, const float *genes, float cut, long long *cou
 
 int launch_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out)
 {
+    int rce = ensure_ET(ctx);
+    if (rce) return rce;
     int blocks = (int)((ctx->N + 255) / 256);
     predict_kernel<<<blocks, 256, ctx->K * sizeof(float), ctx->stream>>>(ctx->ET, ctx->Npad, ctx->N, ctx->K, genes,
                                                                         ctx->act, z_out, y_out);
+    GAME_LAUNCHED(ctx);
+    return GAME_OK;
+}
+
+// game_predict_new: the forward pass on caller-supplied patterns, expansion on the fly (no dataset load).  One thread
+// per pattern; every term is computed exactly as expand_kernel / expand_tied_kernel compute it (fp64, one rounding to
+// fp32) and accumulated in ascending ABI gene order k = i*B + m, so the bits equal game_load(X_new) + game_predict.
+__global__ void predict_new_kernel(const float *__restrict__ X, long long N, int F, int family, int d, int K,
+                                   const float *__restrict__ genes, int act, float *z_out, float *y_out)
+{
+    extern __shared__ float g[];
+    for (int k = threadIdx.x; k < K; k += blockDim.x) g[k] = genes[k];
+    __syncthreads();
+    const long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n >= N) return;
+    float z = 0.f;
+    if (family == GAME_TRIG_TIED || family == GAME_POLY_TIED) {
+        double sum[65];
+        for (int k = 0; k < K; ++k) sum[k] = 0.0;
+        sum[0] = 1.0;
+        for (int i = 0; i < F; ++i) {
+            const double x = (double)X[n * F + i];
+            if (family == GAME_TRIG_TIED) {
+                for (int m = 1; m <= d; ++m) {
+                    double s, c;
+                    sincos((double)m * x, &s, &c);
+                    sum[m] += c;
+                    sum[d + m] += s;
+                }
+            } else {
+                double pw = 1.0;
+                for (int j = 1; j <= d; ++j) { pw *= x; sum[j] += pw; }
+            }
+        }
+        for (int k = 0; k < K; ++k) z = fmaf((float)sum[k], g[k], z);
+    } else {
+        const int B = family == GAME_TRIG ? 2 * d + 1 : d + 1;
+        for (int i = 0; i < F; ++i) {
+            const double x = (double)X[n * F + i];
+            const float *gi = g + i * B;
+            z = fmaf(1.0f, gi[0], z);
+            if (family == GAME_TRIG) {
+                // ABI order inside the block is [1, cos 1..d, sin 1..d]: the sines wait in a local array so that the
+                // accumulation order stays ascending in k while sincos is called exactly as expand_kernel calls it
+                float sn[32];
+                for (int m = 1; m <= d; ++m) {
+                    double sv, cv;
+                    sincos((double)m * x, &sv, &cv);
+                    sn[m - 1] = (float)sv;
+                    z = fmaf((float)cv, gi[m], z);
+                }
+                for (int m = 1; m <= d; ++m) z = fmaf(sn[m - 1], gi[d + m], z);
+            } else {
+                double tm1 = 1.0, t0 = x;
+                z = fmaf((float)x, gi[1], z);
+                for (int m = 2; m <= d; ++m) {
+                    const double t1 = 2.0 * x * t0 - tm1;
+                    z = fmaf((float)t1, gi[m], z);
+                    tm1 = t0;
+                    t0 = t1;
+                }
+            }
+        }
+    }
+    if (z_out) z_out[n] = z;
+    if (y_out) y_out[n] = act == GAME_ACT_SIGMOID ? 1.0f / (1.0f + expf(-z)) : z;
+}
+
+int launch_predict_new(game_ctx *ctx, const float *genes, const float *X_new, long long N_new, float *z_out, float *y_out)
+{
+    const int blocks = (int)((N_new + 127) / 128);
+    predict_new_kernel<<<blocks, 128, ctx->K * sizeof(float), ctx->stream>>>(X_new, N_new, ctx->F, ctx->family, ctx->degree,
+                                                                            ctx->K, genes, ctx->act, z_out, y_out);
     GAME_LAUNCHED(ctx);
     return GAME_OK;
 }

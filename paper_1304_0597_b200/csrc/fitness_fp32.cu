@@ -187,7 +187,7 @@ int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scra
                 float stop_error)
 {
     if (P <= 256 && (long long)pi.n_chunks * P <= POST_SMALL_FLOATS) {
-        GAME_CUDA(ctx, launch_pdl(post_small_kernel, dim3(1), dim3(256), 0, ctx->stream, ctx->partial, pi.n_chunks, pi.Ppad, P, ctx->N,
+        GAME_CUDA(ctx, launch_pdl(post_small_kernel, dim3(1), dim3(256), 0, ctx, ctx->partial, pi.n_chunks, pi.Ppad, P, ctx->N,
                                   ctx->err, fit, order, state, stop_error));
         ++ctx->launches;
         return GAME_OK;
@@ -203,7 +203,7 @@ int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scra
 // With `sums` set the fp64 total itself is written instead (game_fitness_sums: the pattern-sharded exchange adds the
 // totals of all shards before the mean is taken).
 __global__ void finalize_kernel(const float *__restrict__ partial, int n_chunks, int Ppad, int P, long long N,
-                                int err, float *__restrict__ out, double *__restrict__ sums, const DevState *state)
+                                int err, float *__restrict__ out, double *__restrict__ sums, int accumulate, const DevState *state)
 {
     pdl_wait();
     pdl_trigger();
@@ -219,7 +219,7 @@ __global__ void finalize_kernel(const float *__restrict__ partial, int n_chunks,
     if (r == 0 && p < P) {
         double tot = 0.0;
         for (int q = 0; q < 32; ++q) tot += red[q][c];
-        if (sums) { sums[p] = tot; return; }
+        if (sums) { sums[p] = accumulate ? sums[p] + tot : tot; return; }
         double f = tot / (double)N;
         if (err == GAME_ERR_RMSE) f = sqrt(f);
         out[p] = (float)f;
@@ -253,7 +253,7 @@ __global__ void finalize_split_kernel(const float *__restrict__ partial, int n_c
 }
 
 __global__ void finalize_merge_kernel(const double *__restrict__ fin2, int Ppad, int P, long long N, int err,
-                                      float *__restrict__ out, double *__restrict__ sums, const DevState *state)
+                                      float *__restrict__ out, double *__restrict__ sums, int accumulate, const DevState *state)
 {
     pdl_wait();
     pdl_trigger();
@@ -262,7 +262,7 @@ __global__ void finalize_merge_kernel(const double *__restrict__ fin2, int Ppad,
     if (p >= P) return;
     double tot = 0.0;
     for (int y = 0; y < FIN_SPLIT; ++y) tot += fin2[(long long)y * Ppad + p];
-    if (sums) { sums[p] = tot; return; }
+    if (sums) { sums[p] = accumulate ? sums[p] + tot : tot; return; }
     double f = tot / (double)N;
     if (err == GAME_ERR_RMSE) f = sqrt(f);
     out[p] = (float)f;
@@ -383,8 +383,10 @@ size_t fitness_partial_floats(const game_ctx *ctx, int P)
 }
 
 // fit[p] = sums[p] / N_total (root for RMSE): the tail of a5 after the shards' totals have been added
-__global__ void fit_from_sums_kernel(const double *__restrict__ sums, int P, long long N_total, int err, float *__restrict__ out)
+__global__ void fit_from_sums_kernel(const double *__restrict__ sums, int P, long long N_total, int err, float *__restrict__ out,
+                                     const DevState *state)
 {
+    if (state && state->stopped) return;          // the loop has stopped: fit / order keep describing the final population
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P) return;
     double f = sums[p] / (double)N_total;
@@ -392,33 +394,36 @@ __global__ void fit_from_sums_kernel(const double *__restrict__ sums, int P, lon
     out[p] = (float)f;
 }
 
-int launch_fit_from_sums(game_ctx *ctx, const double *sums, int P, long long N_total, float *out)
+int launch_fit_from_sums(game_ctx *ctx, const double *sums, int P, long long N_total, float *out, const DevState *state)
 {
-    fit_from_sums_kernel<<<(P + 255) / 256, 256, 0, ctx->stream>>>(sums, P, N_total, ctx->err, out);
+    fit_from_sums_kernel<<<(P + 255) / 256, 256, 0, ctx->stream>>>(sums, P, N_total, ctx->err, out, state);
     GAME_LAUNCHED(ctx);
     return GAME_OK;
 }
 
-int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, const DevState *state, double *sums)
+int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, const DevState *state, double *sums, bool accumulate)
 {
+    const int acc = accumulate ? 1 : 0;
     dim3 block(32, 32);
     if (n_chunks >= 1024 && (P + 31) / 32 < 2 * ctx->sm_count) {
         dim3 grid((P + 31) / 32, FIN_SPLIT);
-        GAME_CUDA(ctx, launch_pdl(finalize_split_kernel, grid, block, 0, ctx->stream, ctx->partial, n_chunks, Ppad, P, ctx->fin2, state));
+        GAME_CUDA(ctx, launch_pdl(finalize_split_kernel, grid, block, 0, ctx, ctx->partial, n_chunks, Ppad, P, ctx->fin2, state));
         ++ctx->launches;
-        GAME_CUDA(ctx, launch_pdl(finalize_merge_kernel, dim3((P + 255) / 256), dim3(256), 0, ctx->stream, ctx->fin2, Ppad, P, ctx->N,
-                                  ctx->err, out, sums, state));
+        GAME_CUDA(ctx, launch_pdl(finalize_merge_kernel, dim3((P + 255) / 256), dim3(256), 0, ctx, ctx->fin2, Ppad, P, ctx->N,
+                                  ctx->err, out, sums, acc, state));
         ++ctx->launches;
         return GAME_OK;
     }
-    GAME_CUDA(ctx, launch_pdl(finalize_kernel, dim3((P + 31) / 32), block, 0, ctx->stream, ctx->partial, n_chunks, Ppad, P, ctx->N,
-                              ctx->err, out, sums, state));
+    GAME_CUDA(ctx, launch_pdl(finalize_kernel, dim3((P + 31) / 32), block, 0, ctx, ctx->partial, n_chunks, Ppad, P, ctx->N,
+                              ctx->err, out, sums, acc, state));
     ++ctx->launches;
     return GAME_OK;
 }
 
 int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer)
 {
+    int rce = ensure_ET(ctx);             // the fp32 expansion is built on first use
+    if (rce) return rce;
     int Ppad = ((P + 255) / 256) * 256;
     FitnessCfg cfg{ctx->act, ctx->err, ctx->R};
     // under two waves of big tiles, or so few chromosomes that a 128-wide tile would mostly compute padding
@@ -430,14 +435,10 @@ int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, cons
         const int kcap = ctx->K < SKC ? ctx->K : SKC;
         const int smem = kcap * (SLAB + SP + 4) * 4;
         dim3 grid((unsigned)n_chunks, (unsigned)ptiles);
-        static bool attr_set = false;
-        if (!attr_set) {
-            GAME_CUDA(ctx, cudaFuncSetAttribute(fitness_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMALL_SMEM));
-            attr_set = true;
-        }
+        GAME_CUDA(ctx, ensure_smem_attr(ctx, (const void *)fitness_small_kernel, SMALL_SMEM));
         {
             KernelTimer timer(ctx);
-            GAME_CUDA(ctx, launch_pdl(fitness_small_kernel, grid, dim3(128), (size_t)smem, ctx->stream, ctx->ET, ctx->Npad, ctx->N, ctx->K,
+            GAME_CUDA(ctx, launch_pdl(fitness_small_kernel, grid, dim3(128), (size_t)smem, ctx, ctx->ET, ctx->Npad, ctx->N, ctx->K,
                                       pop, P, ctx->t, ctx->n_slabs, spc, kcap, cfg, ctx->partial, Ppad, state));
         }
         ++ctx->launches;
@@ -449,7 +450,7 @@ int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, cons
     dim3 grid((unsigned)n_chunks, (unsigned)((P + BP - 1) / BP));
     {
         KernelTimer timer(ctx);
-        GAME_CUDA(ctx, launch_pdl(fitness_fp32_kernel, grid, dim3(NT), 0, ctx->stream, ctx->ET, ctx->Npad, ctx->N, ctx->K, pop, P, ctx->t,
+        GAME_CUDA(ctx, launch_pdl(fitness_fp32_kernel, grid, dim3(NT), 0, ctx, ctx->ET, ctx->Npad, ctx->N, ctx->K, pop, P, ctx->t,
                                   ctx->n_slabs, spc, cfg, ctx->partial, Ppad, state));
     }
     ++ctx->launches;

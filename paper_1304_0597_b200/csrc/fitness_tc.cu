@@ -83,10 +83,22 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t rank)
 // on B200, same box, all waits of the kernel switched together: config 5 kernel 2.34 -> 2.20 ms, config 4 0.243 -> 0.238 ms
 // (deep contractions: the producer, the MMA issuer and the epilogue all wait for long stretches), config 3 0.143 -> 0.145 ms
 // (shallow: wake-up latency counts).  The kernel therefore uses it exactly where it uses the eight-warp epilogue.
+// A wait that never completes is a protocol bug and must fail loudly instead of hanging the device; the bound is
+// wall-clock time (globaltimer, looked at every 2^16 probes), not a probe count, so a debugger, time-slicing or a
+// profiler replay that stalls the kernel for a while cannot trip it.
+constexpr unsigned long long MBAR_TIMEOUT_NS = 20ull * 1000 * 1000 * 1000;
+__device__ __noinline__ void mbar_timeout_check(unsigned long long &t0)
+{
+    unsigned long long now;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+    if (t0 == 0) t0 = now;
+    else if (now - t0 > MBAR_TIMEOUT_NS) __trap();
+}
 template <bool SUSPEND = false>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t ok = 0;
+    unsigned long long t0 = 0;
     for (uint32_t spin = 0; !ok; ++spin) {
         if (SUSPEND)
             asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
@@ -94,7 +106,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         else
             asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                          : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-        if (spin > (1u << 22)) __trap();      // a protocol bug must fail loudly, not hang the device
+        if ((spin & 0xFFFFu) == 0xFFFFu) mbar_timeout_check(t0);
     }
 }
 // non-blocking: has the phase with this parity completed?
@@ -811,33 +823,23 @@ bool tensor_path_built() { return true; }
 // CTA pairs (cta_group::2, 256 chromosomes x 256 patterns per pair) halve the E-tile bytes each SM stages;
 // measured on B200 they win for deep contractions over wide populations (config 5: 1500 vs 1442 TFLOP/s)
 // and lose where the pair leaves too few chromosome blocks (config 4) or K is shallow (config 3).
-// GAME_TC_CTA_GROUP=1|2 overrides, for measurement.
+// game_set_tuning(GAME_TUNE_CTA_GROUP, 1|2) overrides, for measurement.
 static int cta_group(const game_ctx *ctx, int Ppad, int Kp)
 {
-    (void)ctx;
-    static int forced = -1;
-    if (forced < 0) {
-        const char *e = getenv("GAME_TC_CTA_GROUP");
-        forced = e ? (e[0] == '2' ? 2 : 1) : 0;
-    }
-    if (forced) return forced;
+    const int forced = ctx->tune[GAME_TUNE_CTA_GROUP];
+    if (forced == 1 || forced == 2) return forced;
     return (Kp >= 512 && Ppad >= 1024) ? 2 : 1;
 }
 
-// Which logistic form the epilogue uses: mode 2 unless GAME_TC_SIGMOID=0 (measurement knob).
-static int sigmoid_mode()
+// Which logistic form the epilogue uses: mode 2 unless game_set_tuning(GAME_TUNE_SIGMOID, 0) (measurement knob).
+static int sigmoid_mode(const game_ctx *ctx)
 {
-    static int m = -1;
-    if (m < 0) {
-        const char *e = getenv("GAME_TC_SIGMOID");
-        m = (e && e[0] == '0') ? MODE_SIG_EXACT : MODE_SIG_TANH32;
-    }
-    return m;
+    return ctx->tune[GAME_TUNE_SIGMOID] == 0 ? MODE_SIG_EXACT : MODE_SIG_TANH32;
 }
 
 C16Sink tensor_sink(const game_ctx *ctx, bool split)
 {
-    const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : (split ? MODE_SIG_EXACT : sigmoid_mode());
+    const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : (split ? MODE_SIG_EXACT : sigmoid_mode(ctx));
     C16Sink s;
     s.ptr = split ? ctx->C16s : ctx->C16;
     s.Kpad = ctx->Kpad; s.family = ctx->family; s.d = ctx->degree; s.split = split ? 1 : 0;
@@ -887,11 +889,7 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     const int smem = SRC != SRC_TMA ? k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES
                    : BNT == BN    ? C::SMEM
                                   : 6 * (A_BYTES + BNT * BKB * 2) + 1024 + TC_TAIL_BYTES;
-    static int attr_smem = 0;
-    if (smem > attr_smem) {
-        GAME_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        attr_smem = smem;
-    }
+    GAME_CUDA(ctx, ensure_smem_attr(ctx, (const void *)kern, smem));
     long long total = (long long)n_tiles * m_blocks;
     int pairs = ctx->sm_count / CG;
     if (pairs > total) pairs = (int)total;
@@ -905,7 +903,7 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[1].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = pdl_enabled() ? 2 : 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl_enabled(ctx) ? 2 : 1;
     KernelTimer timer(ctx);
     GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, maps_E[BNT / CG == 128 ? 1 : 0], n_tiles,
                                       m_blocks, k_blocks, ctx->N, (const float *)ctx->t, ctx->R, ctx->partial, Ppad, state,
@@ -944,10 +942,9 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     if (expansion < 0) return fail(ctx, GAME_ERR_UNSUPPORTED, "regenerated expansion unavailable for this shape (needs P <= 256, K <= 576 after padding, trig: max|X| <= pi)");
     // Small populations (one CTA pair covers all chromosomes): keep the fp16 population tile RESIDENT in shared memory and
     // stream only the expansion (SRC_RES) -- a third of SRC_TMA's L2 -> SM traffic.  Config 4, same box: 0.229 vs 0.263 ms,
-    // identical bits; the kernel then runs at 5.1 TB/s of HBM reads (78 % of the measured peak).  GAME_TC_RESIDENT=0 turns
-    // it off, for measurement.
-    static int resident_ok = -1;
-    if (resident_ok < 0) { const char *e = getenv("GAME_TC_RESIDENT"); resident_ok = (e && e[0] == '0') ? 0 : 1; }
+    // identical bits; the kernel then runs at 5.1 TB/s of HBM reads (78 % of the measured peak).
+    // game_set_tuning(GAME_TUNE_RESIDENT, 0) turns it off, for measurement.
+    const bool resident_ok = ctx->tune[GAME_TUNE_RESIDENT] != 0;
     const bool fits = (Kp / BKB) * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES <= 227 * 1024;
     const long long tiles256 = (long long)(ctx->Npad256 / BN) * ((P + BM - 1) / BM);     // 128-chromosome x 256-pattern tiles
     const bool resident_only = expansion != GAME_EXPAND_REGENERATED && resident_ok && Ppad == 256 && fits && Kp >= 256 &&
@@ -957,24 +954,22 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     // Which epilogue: for shallow contractions (the MMAs of a tile take less time than its epilogue) two independent
     // teams of four warps, one per accumulator, so the warps sharing a scheduler are in different stages of different
     // tiles (config 3, same box: 0.139 vs 0.150 ms); for deep ones all eight warps on one tile, which hands the
-    // accumulator back sooner (configs 4, 5: the team form loses 1-2 % there).  GAME_TC_TEAMS=0|1 overrides.
-    static int teams_forced = -1;
-    if (teams_forced < 0) { const char *e = getenv("GAME_TC_TEAMS"); teams_forced = e ? (e[0] == '1' ? 1 : 0) : 2; }
-    const bool teams = teams_forced == 2 ? Kp <= 256 : teams_forced == 1;
+    // accumulator back sooner (configs 4, 5: the team form loses 1-2 % there).  GAME_TUNE_TEAMS = 0|1 overrides.
+    const int teams_forced = ctx->tune[GAME_TUNE_TEAMS];
+    const bool teams = teams_forced < 0 ? Kp <= 256 : teams_forced == 1;
     // Less than one wave of 256-pattern tiles (configs 1-2): twice as many 128-pattern tiles on single CTAs finish sooner.
-    // GAME_TC_HALF_TILES=0|1 overrides, for measurement.
-    static int half_forced = -1;
-    if (half_forced < 0) { const char *e = getenv("GAME_TC_HALF_TILES"); half_forced = e ? (e[0] == '1' ? 1 : 0) : 2; }
-    const bool half_tiles = src == SRC_TMA && (half_forced == 2 ? tiles256 < ctx->sm_count : half_forced == 1);
+    // GAME_TUNE_HALF_TILES = 0|1 overrides, for measurement.
+    const int half_forced = ctx->tune[GAME_TUNE_HALF_TILES];
+    const bool half_tiles = src == SRC_TMA && (half_forced < 0 ? tiles256 < ctx->sm_count : half_forced == 1);
     const int n_tiles = (int)(ctx->Npad256 / (half_tiles ? 128 : BN));
     const int m_blocks = half_tiles ? (P + BM - 1) / BM : Ppad / (BM * cg);
     long long n = (long long)P * ctx->K;
     const bool tmse = ctx->err == GAME_ERR_TMSE;
     // the split path is the 1e-5 tolerance class: its logistic is the ex2 + rcp form (2^-22), not tanh.approx (2^-11)
-    const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : (split ? MODE_SIG_EXACT : sigmoid_mode());
+    const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : (split ? MODE_SIG_EXACT : sigmoid_mode(ctx));
     const C16Sink sink = tensor_sink(ctx, split);
     if (!(ctx->c16_src == pop && ctx->c16_split == sink.split && ctx->c16_scale == sink.scale)) {   // else ga_step_kernel already wrote it
-        GAME_CUDA(ctx, launch_pdl(pop_to_f16_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, ctx->stream, pop, P, ctx->K, sink, state));
+        GAME_CUDA(ctx, launch_pdl(pop_to_f16_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, ctx, pop, P, ctx->K, sink, state));
         ++ctx->launches;
         ctx->c16_src = nullptr;           // an external population: nothing to remember
     }

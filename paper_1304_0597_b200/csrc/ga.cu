@@ -130,9 +130,9 @@ int launch_rank(game_ctx *ctx, const float *fit, int P, int *rank_scratch, int *
                 float stop_error, bool update_state)
 {
     dim3 grid((P + RANK_T - 1) / RANK_T, (P + RANK_Q - 1) / RANK_Q);
-    GAME_CUDA(ctx, launch_pdl(rank_count_kernel, grid, dim3(RANK_T), 0, ctx->stream, fit, P, rank_scratch, state));
+    GAME_CUDA(ctx, launch_pdl(rank_count_kernel, grid, dim3(RANK_T), 0, ctx, fit, P, rank_scratch, state));
     ++ctx->launches;
-    GAME_CUDA(ctx, launch_pdl(rank_scatter_kernel, dim3((P + 255) / 256), dim3(256), 0, ctx->stream, fit, P, rank_scratch, order, state,
+    GAME_CUDA(ctx, launch_pdl(rank_scatter_kernel, dim3((P + 255) / 256), dim3(256), 0, ctx, fit, P, rank_scratch, order, state,
                               stop_error, update_state ? 1 : 0));
     ++ctx->launches;
     return GAME_OK;
@@ -301,11 +301,11 @@ int launch_ga_step(game_ctx *ctx, const game_ga_params *gp, unsigned long long s
     a.pc = host_thr(gp->p_crossover); a.pm = host_thr(gp->p_mutation);
     a.seed = seed; a.gen = gen_base;
     if (gp->selection == GAME_SEL_ROULETTE) {
-        GAME_CUDA(ctx, launch_pdl(roulette_kernel, dim3(1), dim3(1024), 0, ctx->stream, fit, order, gp->P, rw, rprefix, state));
+        GAME_CUDA(ctx, launch_pdl(roulette_kernel, dim3(1), dim3(1024), 0, ctx, fit, order, gp->P, rw, rprefix, state));
         ++ctx->launches;
     }
     int threads = ctx->K >= 512 ? 256 : ctx->K >= 128 ? 128 : 64;
-    GAME_CUDA(ctx, launch_pdl(ga_step_kernel, dim3(a.e + a.npairs), dim3(threads), 0, ctx->stream, a, order, pop, next, rprefix, state,
+    GAME_CUDA(ctx, launch_pdl(ga_step_kernel, dim3(a.e + a.npairs), dim3(threads), 0, ctx, a, order, pop, next, rprefix, state,
                               (int *)nullptr));
     ++ctx->launches;
     return GAME_OK;

@@ -15,16 +15,6 @@ int fail(game_ctx *ctx, int code, const char *what)
     return code;
 }
 
-bool pdl_enabled()
-{
-    static int on = -1;
-    if (on < 0) {
-        const char *e = getenv("GAME_PDL");
-        on = (e && e[0] == '0') ? 0 : 1;
-    }
-    return on != 0;
-}
-
 int cuda_fail(game_ctx *ctx, cudaError_t e, const char *where)
 {
     if (ctx) {
@@ -43,7 +33,7 @@ static void dfree(T *&p)
 static void free_dataset(game_ctx *c)
 {
     dfree(c->X); dfree(c->t); dfree(c->ET); dfree(c->E16); dfree(c->E16s);
-    c->N = 0; c->tensor_ok = false; c->split_ok = false;
+    c->N = 0; c->tensor_ok = false; c->split_ok = false; c->have_fit = false;
 }
 
 static void free_population(game_ctx *c)
@@ -100,19 +90,24 @@ static int ensure_scratch(game_ctx *c, int P)
     return GAME_OK;
 }
 
-static int resolve_path(const game_ctx *c, int P)
+// own: the population evaluated is the context's own (installed or evolved), whose gene range is known
+static int resolve_path(const game_ctx *c, int P, bool own = false)
 {
-    bool can_tensor = tensor_path_built() && c->tensor_ok;
+    (void)P;
+    // genes beyond the finite fp16 range cannot be tensor-path operands (game_set_population measured them)
+    const bool genes_ok = !own || c->pop_maxabs <= 65504.0f;
+    bool can_tensor = tensor_path_built() && c->tensor_ok && genes_ok;
     if (c->path == GAME_PATH_FP32) return GAME_PATH_FP32;
     if (c->path == GAME_PATH_TENSOR) return can_tensor ? GAME_PATH_TENSOR : -1;
-    const bool can_split = tensor_path_built() && c->split_ok;
+    const bool can_split = tensor_path_built() && c->split_ok && genes_ok;
     if (c->path == GAME_PATH_TENSOR_SPLIT) return can_split ? GAME_PATH_TENSOR_SPLIT : -1;
     // AUTO: the tensor cores wherever they can be used -- measured on B200 they beat the FFMA kernels at every population
     // size down to P = 8 (N = 2e5, K = 544: 0.05 / 0.14 ms against 0.43 ms; config 1 in the loop: 60.6k against 48.5k
     // generations/s).  Large datasets take the one-pass fp16 form (1e-3 class), small ones -- where a generation is a few
     // microseconds either way -- the split form, which stays in the FP32 path's 1e-5 class.  The FFMA kernels remain for
     // what the tensor paths cannot take (tied families, |E| > 2) and for GAME_PATH_FP32.
-    if (can_tensor && c->N >= 16384) return GAME_PATH_TENSOR;
+    // (a pattern shard decides from the GLOBAL N, game_set_global_patterns, so that all shards share one tolerance class)
+    if (can_tensor && (c->N_global > 0 ? c->N_global : c->N) >= 16384) return GAME_PATH_TENSOR;
     if (can_split) return GAME_PATH_TENSOR_SPLIT;
     return GAME_PATH_FP32;
 }
@@ -121,8 +116,8 @@ static int run_fitness(game_ctx *c, const float *pop, int P, float *out, const D
 {
     int rc = ensure_scratch(c, P);
     if (rc) return rc;
-    int path = resolve_path(c, P);
-    if (path < 0) return fail(c, GAME_ERR_UNSUPPORTED, "tensor path unavailable for this dataset (not built, or |E| exceeds fp16 range)");
+    int path = resolve_path(c, P, pop == c->pop);
+    if (path < 0) return fail(c, GAME_ERR_UNSUPPORTED, "tensor path unavailable for this dataset / population (|E| or |gene| exceeds the fp16 range, or a tied family)");
     if (path == GAME_PATH_TENSOR) return launch_fitness_tensor(c, pop, P, out, state, defer, false);
     if (path == GAME_PATH_TENSOR_SPLIT) return launch_fitness_tensor(c, pop, P, out, state, defer, true);
     return launch_fitness_fp32(c, pop, P, out, state, defer);
@@ -144,48 +139,65 @@ static int validate_params(game_ctx *c, const game_ga_params *g)
     return GAME_OK;
 }
 
+// close a run of asynchronous game_advance calls: the device-side counters become the host's
+static int close_loop(game_ctx *c, game_result *res)
+{
+    DevState h{};
+    GAME_CUDA(c, cudaMemcpyAsync(&h, c->state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->loop_open) {
+        c->generation += h.gens_run;
+        c->loop_open = false;
+        // once the stop test has fired the population no longer moves: fit / order describe it
+        if (h.stopped || h.stop_request) c->have_fit = true;
+    } else {
+        h = DevState{};
+    }
+    if (res) {
+        res->generations_run = h.gens_run;
+        res->stopped_on_error = (h.stopped || h.stop_request) ? 1 : 0;
+        res->best_error = h.best_error;
+        res->best_index = h.best_index;
+    }
+    return GAME_OK;
+}
+#define GAME_CLOSE_LOOP(c) do { if ((c)->loop_open) { int rc__ = close_loop(c, nullptr); if (rc__) return rc__; } } while (0)
+
 static int load_common(game_ctx *c, const float *X, const float *targets, long long N)
 {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!X || !targets || N < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_load: X, targets must be non-NULL and N >= 1");
-    free_dataset(c);
+    free_dataset(c);                              // also drops have_fit: fit / order described the previous dataset
     dfree(c->partial); c->partial_cap = 0;
     c->c16_src = nullptr;
-    const int K = c->K;
-    c->N = N;
-    c->n_slabs = (int)((N + SLAB - 1) / SLAB);
-    c->Npad = (long long)c->n_slabs * SLAB;
+    // c->N stays 0 (nothing loaded) until everything below has succeeded; every failure frees what was built
+    const int n_slabs = (int)((N + SLAB - 1) / SLAB);
+    c->n_slabs = n_slabs;
+    c->Npad = (long long)n_slabs * SLAB;
     c->Npad256 = ((N + 255) / 256) * 256;
     int *flag = nullptr;
-    GAME_CUDA(c, cudaMalloc(&c->X, (size_t)N * c->F * sizeof(float)));
-    GAME_CUDA(c, cudaMalloc(&c->t, (size_t)c->Npad256 * sizeof(float)));
-    GAME_CUDA(c, cudaMalloc(&c->ET, (size_t)K * c->Npad * sizeof(float)));
-    GAME_CUDA(c, cudaMalloc(&flag, 3 * sizeof(int)));      // [0] non-finite input, [1] max|E| bits, [2] max|X| bits
-    GAME_CUDA(c, cudaMemsetAsync(flag, 0, 3 * sizeof(int), c->stream));
-    GAME_CUDA(c, cudaMemsetAsync(c->t, 0, (size_t)c->Npad256 * sizeof(float), c->stream));
-    GAME_CUDA(c, cudaMemsetAsync(c->ET, 0, (size_t)K * c->Npad * sizeof(float), c->stream));
-    GAME_CUDA(c, cudaMemcpyAsync(c->X, X, (size_t)N * c->F * sizeof(float), cudaMemcpyDefault, c->stream));
-    GAME_CUDA(c, cudaMemcpyAsync(c->t, targets, (size_t)N * sizeof(float), cudaMemcpyDefault, c->stream));
-    int rc = launch_check_finite(c, c->X, N * c->F, c->t, N, flag);
-    if (rc) { cudaFree(flag); return rc; }
-    rc = launch_expand_fp32(c);
-    if (rc) { cudaFree(flag); return rc; }
-    if (tensor_path_built()) {
+    int h[3] = {0, 0, 0};
+    auto body = [&]() -> int {
+        GAME_CUDA(c, cudaMalloc(&c->X, (size_t)N * c->F * sizeof(float)));
+        GAME_CUDA(c, cudaMalloc(&c->t, (size_t)c->Npad256 * sizeof(float)));
+        GAME_CUDA(c, cudaMalloc(&flag, 3 * sizeof(int)));      // [0] non-finite input, [1] max|E| bits, [2] max|X| bits
+        GAME_CUDA(c, cudaMemsetAsync(flag, 0, 3 * sizeof(int), c->stream));
+        GAME_CUDA(c, cudaMemsetAsync(c->t, 0, (size_t)c->Npad256 * sizeof(float), c->stream));
+        GAME_CUDA(c, cudaMemcpyAsync(c->X, X, (size_t)N * c->F * sizeof(float), cudaMemcpyDefault, c->stream));
+        GAME_CUDA(c, cudaMemcpyAsync(c->t, targets, (size_t)N * sizeof(float), cudaMemcpyDefault, c->stream));
+        c->N = N;                                 // the expansion launchers read it; withdrawn again on failure
+        int rc = launch_check_finite(c, c->X, N * c->F, c->t, N, flag);
+        if (rc) return rc;
+        // the fp16 tile-blocked expansion of the tensor paths (also measures max|E|); the fp32 term-major one (ET) is
+        // built on first use by the FFMA kernels / game_predict / game_classify (ensure_ET)
         size_t n16 = (size_t)c->Npad256 * c->Kpad;
         GAME_CUDA(c, cudaMalloc(&c->E16, n16 * sizeof(__half)));
         GAME_CUDA(c, cudaMemsetAsync(c->E16, 0, n16 * sizeof(__half), c->stream));
         rc = launch_expand_fp16(c, reinterpret_cast<float *>(flag + 1));
-        if (rc) { cudaFree(flag); return rc; }
-    }
-    int h[3] = {0, 0, 0};
-    GAME_CUDA(c, cudaMemcpyAsync(h, flag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
-    GAME_CUDA(c, cudaStreamSynchronize(c->stream));
-    cudaFree(flag);
-    if (h[0]) {
-        free_dataset(c);
-        return fail(c, GAME_ERR_NONFINITE_INPUT, "game_load: X or targets contain NaN/Inf");
-    }
-    if (tensor_path_built()) {
+        if (rc) return rc;
+        GAME_CUDA(c, cudaMemcpyAsync(h, flag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+        GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (h[0]) return fail(c, GAME_ERR_NONFINITE_INPUT, "game_load: X or targets contain NaN/Inf");
         float mx;
         memcpy(&mx, &h[1], sizeof(float));
         memcpy(&c->x_maxabs, &h[2], sizeof(float));
@@ -197,14 +209,17 @@ static int load_common(game_ctx *c, const float *X, const float *targets, long l
         // the split form keeps ~22 bits of every value whatever its magnitude (hi + lo), so it only needs the values well
         // inside fp16's range and above its subnormals' grain: |E| <= 1024 (e.g. Chebyshev terms of unnormalised features)
         c->split_ok = mx <= 1024.0f && rows_ok && tc_permuted(c->family);
-        if (c->tensor_ok) {
-            rc = tensor_prepare(c);
-            if (rc) return rc;
-        } else {
-            dfree(c->E16);
-        }
+        if (c->tensor_ok) return tensor_prepare(c);
+        dfree(c->E16);
+        return GAME_OK;
+    };
+    const int rc = body();
+    if (flag) cudaFree(flag);
+    if (rc) {
+        cudaStreamSynchronize(c->stream);         // nothing may still be writing what is freed
+        free_dataset(c);
     }
-    return GAME_OK;
+    return rc;
 }
 
 }  // namespace game
@@ -224,8 +239,10 @@ int game_create(int family, int degree, int F, game_ctx **out)
     c->K = family == GAME_TRIG ? F * (2 * degree + 1) : family == GAME_CHEB ? F * (degree + 1)
          : family == GAME_TRIG_TIED ? 2 * degree + 1 : degree + 1;
     c->Kpad = ((tc_num_positions(family, degree, F, c->K) + TC_KBLK - 1) / TC_KBLK) * TC_KBLK;
+    for (int &t : c->tune) t = -1;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
+    c->device = dev;
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (e == cudaSuccess) e = cudaMalloc(&c->state, sizeof(DevState) + 16);
     if (e == cudaSuccess) e = cudaMemset(c->state, 0, sizeof(DevState) + 16);
@@ -242,6 +259,7 @@ int game_create(int family, int degree, int F, game_ctx **out)
 void game_destroy(game_ctx *c)
 {
     if (!c) return;
+    DeviceGuard dg(c);
     cudaStreamSynchronize(c->stream);
     free_dataset(c);
     free_population(c);
@@ -252,7 +270,14 @@ void game_destroy(game_ctx *c)
 }
 
 int game_num_terms(const game_ctx *c) { return c ? c->K : -1; }
-long long game_generation(const game_ctx *c) { return c ? c->generation : -1; }
+long long game_generation(const game_ctx *cc)
+{
+    if (!cc) return -1;
+    game_ctx *c = const_cast<game_ctx *>(cc);
+    if (c->loop_open) { DeviceGuard dg(c); if (close_loop(c, nullptr)) return -1; }   // asynchronous advances pending
+    return c->generation;
+}
+int game_population_size(const game_ctx *c) { return (c && c->have_pop) ? c->P : 0; }
 const char *game_last_error(const game_ctx *c) { return c ? c->msg.c_str() : "null context"; }
 long long game_launch_count(const game_ctx *c) { return c ? c->launches : -1; }
 
@@ -290,7 +315,25 @@ int game_set_path(game_ctx *c, int path)
     return GAME_OK;
 }
 
-int game_resolved_path(const game_ctx *c, int P) { return c ? resolve_path(c, P) : -1; }
+int game_resolved_path(const game_ctx *c, int P) { return c ? resolve_path(c, P, c->have_pop && P == c->P) : -1; }
+
+int game_set_tuning(game_ctx *c, int knob, int value)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (knob < 0 || knob >= GAME_TUNE_COUNT_) return fail(c, GAME_ERR_INVALID_ARG, "game_set_tuning: unknown knob");
+    static const int lo[GAME_TUNE_COUNT_] = {0, 1, 0, 0, 0, 0, 0, 0}, hi[GAME_TUNE_COUNT_] = {1, 2, 3, 1, 1, 1, 1, 16};
+    if (value != -1 && (value < lo[knob] || value > hi[knob] || (knob == GAME_TUNE_SIGMOID && value == 1)))
+        return fail(c, GAME_ERR_INVALID_ARG, "game_set_tuning: value out of range for this knob");
+    c->tune[knob] = value;
+    return GAME_OK;
+}
+
+int game_set_global_patterns(game_ctx *c, long long N_total)
+{
+    if (!c || N_total < 0) return GAME_ERR_INVALID_ARG;
+    c->N_global = N_total;
+    return GAME_OK;
+}
 
 int game_set_expansion(game_ctx *c, int mode)
 {
@@ -302,14 +345,15 @@ int game_set_expansion(game_ctx *c, int mode)
 
 int game_resolved_expansion(const game_ctx *c, int P) { return (c && c->N && P >= 1) ? tensor_expansion(c, P) : -1; }
 
-int game_load(game_ctx *c, const float *X, const float *t, long long N) { return load_common(c, X, t, N); }
-int game_load_host(game_ctx *c, const float *X, const float *t, long long N) { return load_common(c, X, t, N); }
+int game_load(game_ctx *c, const float *X, const float *t, long long N) { DeviceGuard dg(c); return load_common(c, X, t, N); }
+int game_load_host(game_ctx *c, const float *X, const float *t, long long N) { DeviceGuard dg(c); return load_common(c, X, t, N); }
 
 int game_fitness(game_ctx *c, const float *pop, int P, float *out)
 {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!c->N) return fail(c, GAME_ERR_NOT_LOADED, "game_fitness before game_load");
     if (!pop || !out || P < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_fitness: pop/out NULL or P < 1");
+    DeviceGuard dg(c);
     return run_fitness(c, pop, P, out, nullptr);
 }
 
@@ -318,24 +362,37 @@ int game_fitness_host(game_ctx *c, const float *pop, int P, float *out)
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!c->N) return fail(c, GAME_ERR_NOT_LOADED, "game_fitness_host before game_load");
     if (!pop || !out || P < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_fitness_host: pop/out NULL or P < 1");
+    DeviceGuard dg(c);
     if ((size_t)P > c->stage_cap) {
         dfree(c->stage_pop); dfree(c->stage_fit);
+        c->stage_cap = 0;
         GAME_CUDA(c, cudaMalloc(&c->stage_pop, (size_t)P * c->K * sizeof(float)));
-        GAME_CUDA(c, cudaMalloc(&c->stage_fit, (size_t)P * sizeof(float)));
+        GAME_CUDA(c, cudaMalloc(&c->stage_fit, ((size_t)P + 2) * sizeof(float)));     // + the two gene-range words
         c->stage_cap = P;
     }
+    int *range = reinterpret_cast<int *>(c->stage_fit + P);
     GAME_CUDA(c, cudaMemcpyAsync(c->stage_pop, pop, (size_t)P * c->K * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    int rc = run_fitness(c, c->stage_pop, P, c->stage_fit, nullptr);
+    GAME_CUDA(c, cudaMemsetAsync(range, 0, 2 * sizeof(int), c->stream));
+    int rc = launch_max_abs(c, c->stage_pop, (long long)P * c->K, range);
+    if (!rc) rc = run_fitness(c, c->stage_pop, P, c->stage_fit, nullptr);
     if (rc) return rc;
+    int hr[2] = {0, 0};
     GAME_CUDA(c, cudaMemcpyAsync(out, c->stage_fit, (size_t)P * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    GAME_CUDA(c, cudaMemcpyAsync(hr, range, sizeof(hr), cudaMemcpyDeviceToHost, c->stream));
     GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+    float mx;
+    memcpy(&mx, &hr[1], sizeof(float));
+    if ((hr[0] || mx > 65504.0f) && resolve_path(c, P) != GAME_PATH_FP32)
+        return fail(c, GAME_ERR_UNSUPPORTED, "game_fitness_host: genes outside the finite fp16 range (|gene| > 65504 or NaN/Inf) "
+                                             "cannot be evaluated on a tensor path; use GAME_PATH_FP32");
     return GAME_OK;
 }
 
-int game_fitness_sums(game_ctx *c, const float *pop, int P, double *sums)
+int game_fitness_sums(game_ctx *c, const float *pop, int P, double *sums, int accumulate)
 {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!c->N) return fail(c, GAME_ERR_NOT_LOADED, "game_fitness_sums before game_load");
+    DeviceGuard dg(c);
     if (!pop) {                                   // the context's own population
         if (!c->have_pop) return fail(c, GAME_ERR_NOT_LOADED, "game_fitness_sums: no population yet");
         pop = c->pop; P = c->P;
@@ -344,7 +401,7 @@ int game_fitness_sums(game_ctx *c, const float *pop, int P, double *sums)
     PartialInfo pi{};
     int rc = run_fitness(c, pop, P, nullptr, nullptr, &pi);
     if (rc) return rc;
-    return launch_finalize(c, pi.n_chunks, pi.Ppad, P, nullptr, nullptr, sums);
+    return launch_finalize(c, pi.n_chunks, pi.Ppad, P, nullptr, nullptr, sums, accumulate != 0);
 }
 
 int game_advance(game_ctx *c, const double *sums, long long N_total, unsigned long long seed, const game_ga_params *gp,
@@ -355,30 +412,41 @@ int game_advance(game_ctx *c, const double *sums, long long N_total, unsigned lo
     if (rc) return rc;
     if (!c->have_pop || c->P != gp->P) return fail(c, GAME_ERR_NOT_LOADED, "game_advance: no population of params->P chromosomes installed");
     if (!sums || N_total < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_advance: sums NULL or N_total < 1");
+    DeviceGuard dg(c);
     const int P = gp->P;
-    GAME_CUDA(c, cudaMemsetAsync(c->state, 0, sizeof(DevState), c->stream));
-    rc = launch_fit_from_sums(c, sums, P, N_total, c->fit);                                         // a5 tail
+    if (!c->loop_open) {
+        // a run of advances shares ONE device-side state: evaluations done, generations applied and the stop flag live
+        // there, so an asynchronous call needs nothing from the host (ga_step_kernel derives its generation index from
+        // gen_base_open + evals_done - 1, as the game_evolve loop does)
+        GAME_CUDA(c, cudaMemsetAsync(c->state, 0, sizeof(DevState), c->stream));
+        c->gen_base_open = (unsigned int)c->generation;
+        c->loop_open = true;
+    }
+    rc = launch_fit_from_sums(c, sums, P, N_total, c->fit, c->state);                              // a5 tail
     if (!rc) rc = launch_rank(c, c->fit, P, c->rank, c->order, c->state, gp->stop_error, true);    // a6, a7
     if (rc) return rc;
     if (apply_operators) {                                                                          // a8-a11
-        rc = launch_ga_step(c, gp, seed, (unsigned int)c->generation, c->order, c->fit, c->pop, c->pop_next, c->state, c->rw,
-                            c->rprefix);
+        const int path = resolve_path(c, P, true);
+        C16Sink sink = tensor_sink(c, path == GAME_PATH_TENSOR_SPLIT);
+        const bool with_sink = (path == GAME_PATH_TENSOR || path == GAME_PATH_TENSOR_SPLIT) && sink.ptr != nullptr && c->N > 0;
+        rc = launch_ga_step(c, gp, seed, c->gen_base_open, c->order, c->fit, c->pop, c->pop_next, c->state, c->rw,
+                            c->rprefix, with_sink ? &sink : nullptr);
         if (rc) return rc;
         float *tmp = c->pop; c->pop = c->pop_next; c->pop_next = tmp;
-        c->c16_src = nullptr;
+        c->c16_src = with_sink ? c->pop : nullptr; c->c16_split = sink.split; c->c16_scale = sink.scale;
+        c->have_fit = false;       // (if the stop test fired the population did not move, but the host cannot know yet)
+    } else {
+        c->have_fit = true;
     }
-    DevState h{};
-    GAME_CUDA(c, cudaMemcpyAsync(&h, c->state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
-    GAME_CUDA(c, cudaStreamSynchronize(c->stream));
-    c->generation += h.gens_run;
-    c->have_fit = !apply_operators || h.gens_run == 0;      // fit/order describe the CURRENT population only if it did not move
-    if (res) {
-        res->generations_run = h.gens_run;
-        res->stopped_on_error = (h.stopped || h.stop_request) ? 1 : 0;
-        res->best_error = h.best_error;
-        res->best_index = h.best_index;
-    }
-    return GAME_OK;
+    if (!res) return GAME_OK;      // asynchronous: game_sync (or any call that needs the counters) collects later
+    return close_loop(c, res);
+}
+
+int game_sync(game_ctx *c, game_result *res)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    DeviceGuard dg(c);
+    return close_loop(c, res);
 }
 
 int game_predict(game_ctx *c, const float *genes, float *z_out, float *y_out)
@@ -386,7 +454,16 @@ int game_predict(game_ctx *c, const float *genes, float *z_out, float *y_out)
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!c->N) return fail(c, GAME_ERR_NOT_LOADED, "game_predict before game_load");
     if (!genes) return fail(c, GAME_ERR_INVALID_ARG, "game_predict: genes is NULL");
+    DeviceGuard dg(c);
     return launch_predict(c, genes, z_out, y_out);
+}
+
+int game_predict_new(game_ctx *c, const float *genes, const float *X_new, long long N_new, float *z_out, float *y_out)
+{
+    if (!c) return GAME_ERR_INVALID_ARG;
+    if (!genes || !X_new || N_new < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_predict_new: genes / X_new NULL or N_new < 1");
+    DeviceGuard dg(c);
+    return launch_predict_new(c, genes, X_new, N_new, z_out, y_out);
 }
 
 int game_classify(game_ctx *c, const float *genes, float cut, long long *counts, double *fom)
@@ -394,6 +471,7 @@ int game_classify(game_ctx *c, const float *genes, float cut, long long *counts,
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!c->N) return fail(c, GAME_ERR_NOT_LOADED, "game_classify before game_load");
     if (!genes || !counts || !fom) return fail(c, GAME_ERR_INVALID_ARG, "game_classify: NULL pointer");
+    DeviceGuard dg(c);
     return launch_classify(c, genes, cut, counts, fom, c->ticket);
 }
 
@@ -401,9 +479,27 @@ int game_set_population(game_ctx *c, const float *pop, int P)
 {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!pop || P < 2) return fail(c, GAME_ERR_INVALID_ARG, "game_set_population: pop NULL or P < 2");
+    DeviceGuard dg(c);
+    GAME_CLOSE_LOOP(c);
     int rc = ensure_population(c, P);
     if (rc) return rc;
-    GAME_CUDA(c, cudaMemcpyAsync(c->pop, pop, (size_t)P * c->K * sizeof(float), cudaMemcpyDefault, c->stream));
+    // gene range first (into the spare buffer): a rejected population leaves the installed one untouched
+    int *range = reinterpret_cast<int *>(c->rank);          // P >= 2 ints, zero between uses (the rank kernels keep it so)
+    GAME_CUDA(c, cudaMemcpyAsync(c->pop_next, pop, (size_t)P * c->K * sizeof(float), cudaMemcpyDefault, c->stream));
+    rc = launch_max_abs(c, c->pop_next, (long long)P * c->K, range);
+    if (rc) return rc;
+    int hr[2] = {0, 0};
+    GAME_CUDA(c, cudaMemcpyAsync(hr, range, sizeof(hr), cudaMemcpyDeviceToHost, c->stream));
+    GAME_CUDA(c, cudaMemsetAsync(range, 0, 2 * sizeof(int), c->stream));
+    GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (hr[0]) return fail(c, GAME_ERR_NONFINITE_INPUT, "game_set_population: genes contain NaN/Inf");
+    float mx;
+    memcpy(&mx, &hr[1], sizeof(float));
+    if (mx > 65504.0f && (c->path == GAME_PATH_TENSOR || c->path == GAME_PATH_TENSOR_SPLIT))
+        return fail(c, GAME_ERR_UNSUPPORTED, "game_set_population: |gene| > 65504 cannot be an fp16 operand of the requested tensor path; "
+                                             "use GAME_PATH_FP32 or GAME_PATH_AUTO");
+    float *tmp = c->pop; c->pop = c->pop_next; c->pop_next = tmp;
+    c->pop_maxabs = mx;
     c->P = P; c->have_pop = true; c->have_fit = false; c->c16_src = nullptr;
     return GAME_OK;
 }
@@ -411,6 +507,8 @@ int game_set_population(game_ctx *c, const float *pop, int P)
 int game_set_generation(game_ctx *c, long long g)
 {
     if (!c || g < 0) return GAME_ERR_INVALID_ARG;
+    DeviceGuard dg(c);
+    GAME_CLOSE_LOOP(c);
     c->generation = g;
     return GAME_OK;
 }
@@ -423,14 +521,18 @@ int game_evolve(game_ctx *c, int generations, unsigned long long seed, const gam
     if (rc) return rc;
     if (generations < 0) return fail(c, GAME_ERR_INVALID_ARG, "generations < 0");
     if (c->have_pop && c->P != gp->P) return fail(c, GAME_ERR_INVALID_ARG, "params->P differs from the installed population");
+    DeviceGuard dg(c);
+    GAME_CLOSE_LOOP(c);
     const int P = gp->P;
     if (!c->have_pop) {
         rc = ensure_population(c, P);
         if (rc) return rc;
         rc = launch_init_population(c, gp->init_mode, seed, P, c->pop);     // a12
         if (rc) return rc;
-        c->P = P; c->have_pop = true; c->c16_src = nullptr;
+        c->P = P; c->have_pop = true; c->c16_src = nullptr; c->pop_maxabs = 1.0f;
     }
+    if (resolve_path(c, P, true) < 0)
+        return fail(c, GAME_ERR_UNSUPPORTED, "tensor path unavailable for this dataset / population (|E| or |gene| exceeds the fp16 range, or a tied family)");
     GAME_CUDA(c, cudaMemsetAsync(c->state, 0, sizeof(DevState), c->stream));
     DevState h{};
     const bool can_stop = gp->stop_error >= 0.f;
@@ -445,7 +547,7 @@ int game_evolve(game_ctx *c, int generations, unsigned long long seed, const gam
         int r = evaluate();
         if (r) return r;
         // a8-a11; on the tensor paths the operators also write the fp16 copy the next evaluation contracts against
-        const int path = resolve_path(c, P);
+        const int path = resolve_path(c, P, true);
         C16Sink sink = tensor_sink(c, path == GAME_PATH_TENSOR_SPLIT);
         const bool with_sink = (path == GAME_PATH_TENSOR || path == GAME_PATH_TENSOR_SPLIT) && sink.ptr != nullptr;
         r = launch_ga_step(c, gp, seed, gen_base, c->order, c->fit, c->pop, c->pop_next, c->state, c->rw, c->rprefix,
@@ -520,6 +622,8 @@ static int get_population(game_ctx *c, float *pop, float *fit, int *order, bool 
 {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!c->have_pop) return fail(c, GAME_ERR_NOT_LOADED, "no population yet");
+    DeviceGuard dg(c);
+    GAME_CLOSE_LOOP(c);
     if ((fit || order) && !c->have_fit) return fail(c, GAME_ERR_NOT_LOADED, "fitness / order are only valid after game_evolve");
     if (pop) GAME_CUDA(c, cudaMemcpyAsync(pop, c->pop, (size_t)c->P * c->K * sizeof(float), cudaMemcpyDefault, c->stream));
     if (fit) GAME_CUDA(c, cudaMemcpyAsync(fit, c->fit, (size_t)c->P * sizeof(float), cudaMemcpyDefault, c->stream));
@@ -535,6 +639,7 @@ int game_rank(game_ctx *c, const float *fit, int P, int *order)
 {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!fit || !order || P < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_rank: NULL pointer or P < 1");
+    DeviceGuard dg(c);
     int *scratch = nullptr;
     GAME_CUDA(c, cudaMallocAsync(&scratch, (size_t)P * sizeof(int), c->stream));
     GAME_CUDA(c, cudaMemsetAsync(scratch, 0, (size_t)P * sizeof(int), c->stream));
@@ -551,6 +656,7 @@ int game_ga_step(game_ctx *c, const game_ga_params *gp, unsigned long long seed,
     if (rc) return rc;
     if (!order || !pop || !next || generation < 0) return fail(c, GAME_ERR_INVALID_ARG, "game_ga_step: NULL pointer or generation < 0");
     if (gp->selection == GAME_SEL_ROULETTE && !fit) return fail(c, GAME_ERR_INVALID_ARG, "roulette selection needs fit");
+    DeviceGuard dg(c);
     unsigned int *rw = nullptr;
     unsigned long long *rp = nullptr;
     if (gp->selection == GAME_SEL_ROULETTE) {
@@ -567,6 +673,7 @@ int game_init_population(game_ctx *c, int mode, unsigned long long seed, int P, 
 {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!pop || P < 1 || mode < 0 || mode > 2) return fail(c, GAME_ERR_INVALID_ARG, "game_init_population: bad argument");
+    DeviceGuard dg(c);
     return launch_init_population(c, mode, seed, P, pop);
 }
 
@@ -580,6 +687,7 @@ int game_set_kernel_timing(game_ctx *c, int enabled)
 int game_get_kernel_timing(game_ctx *c, double *total_ms, long long *launches)
 {
     if (!c || !total_ms || !launches) return GAME_ERR_INVALID_ARG;
+    DeviceGuard dg(c);
     GAME_CUDA(c, cudaStreamSynchronize(c->stream));
     double tot = 0.0;
     for (size_t i = 0; i + 1 < c->ev.size(); i += 2) {
@@ -598,6 +706,7 @@ int game_philox(game_ctx *c, unsigned long long seed, const unsigned int *ctr, i
 {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (!ctr || !out || n < 1) return fail(c, GAME_ERR_INVALID_ARG, "game_philox: bad argument");
+    DeviceGuard dg(c);
     return launch_philox(c, seed, ctr, n, out);
 }
 

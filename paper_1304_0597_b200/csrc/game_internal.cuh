@@ -5,6 +5,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <unordered_map>
 #include <vector>
 
 #include "../../include/game.h"
@@ -77,11 +78,14 @@ struct C16Sink {
     int Kpad, family, d, split;
     float scale;         // 1, or 0.5 for the tanh logistic (exact)
 };
-// gene k (ABI order) of chromosome p -> its fp16 position(s): round to nearest even, clamped to the finite fp16 range;
+// gene k (ABI order) of chromosome p -> its fp16 position(s): round to nearest even.  A gene outside the finite fp16
+// range (|gene| > 65504, Inf, NaN) cannot be an operand of the tensor paths: it is stored as NaN, so THAT chromosome's
+// fitness comes out NaN (ranked last) instead of being silently clamped; game_set_population / game_fitness_host
+// reject such populations up front (GAME_ERR_UNSUPPORTED) or route AUTO to the FP32 path.
 // split: rows of 3 Kpad positions [hi | lo | hi], hi = fp16(c), lo = fp16(c - hi) (see expand_kernel)
 __device__ __forceinline__ void c16_store(const C16Sink &s, int p, int k, float gene)
 {
-    const float v = fminf(fmaxf(gene, -65504.f), 65504.f) * s.scale;
+    const float v = fabsf(gene) <= 65504.f ? gene * s.scale : __int_as_float(0x7fc00000);
     int pos = k;
     if (tc_permuted(s.family)) {              // ABI order k = i*B + m  ->  the tensor path's term order
         const int B = tc_terms_per_feature(s.family, s.d);
@@ -109,13 +113,17 @@ struct game_ctx {
     float R = 0.f;
     cudaStream_t stream = 0;
     int sm_count = 148;
+    int device = 0;                                  // the CUDA device this context lives on (current at game_create)
+    int tune[GAME_TUNE_COUNT_];                       // game_set_tuning knobs, -1 = automatic
+    std::unordered_map<const void *, int> smem_attr;  // kernels whose dynamic-smem opt-in was raised ON THIS DEVICE
+    long long N_global = 0;                           // pattern-sharded runs: the global N the AUTO path choice uses
 
     // dataset (a0/a1)
     long long N = 0, Npad = 0;
     int n_slabs = 0;
     float *X = nullptr;        // N x F copy (kept for game_predict-style regeneration)
     float *t = nullptr;        // Npad, zero padded
-    float *ET = nullptr;       // K x Npad fp32, term-major (FP32 path), zero padded
+    float *ET = nullptr;       // K x Npad fp32, term-major (FP32 path, predict / classify), zero padded; built on first use
     __half *E16 = nullptr;     // Npad256 x Kpad fp16, pattern-major (TENSOR path), zero padded
     __half *E16s = nullptr;    // Npad256 x 3 Kpad fp16: [hi | hi | lo] halves of E (TENSOR_SPLIT path), built on first use
     long long Npad256 = 0;
@@ -127,7 +135,10 @@ struct game_ctx {
     // population / loop state
     int P = 0;
     bool have_pop = false, have_fit = false;
+    float pop_maxabs = 0.f;                  // max |gene| of an installed population (game_set_population); evolution keeps it <= max(this, 1)
     long long generation = 0;
+    bool loop_open = false;                  // asynchronous game_advance calls pending: DevState counts since gen_base_open
+    unsigned int gen_base_open = 0;
     float *pop = nullptr, *pop_next = nullptr, *fit = nullptr;
     int *order = nullptr, *rank = nullptr;
     unsigned int *rw = nullptr;              // roulette weights
@@ -190,24 +201,50 @@ struct KernelTimer {
     ~KernelTimer() { if (c->timing) cudaEventRecord(c->ev.back(), c->stream); }
 };
 
-bool pdl_enabled();      // GAME_PDL=0 turns the attribute off (measurement knob)
+inline bool pdl_enabled(const game_ctx *c) { return c->tune[GAME_TUNE_PDL] != 0; }   // GAME_TUNE_PDL = 0 turns the attribute off
 
-// kernel<<<grid, block, smem, stream>>>(args...) with the PDL attribute
+// Makes the context's device current for the duration of an ABI call (a context belongs to the device that was current
+// at game_create; callers may hold contexts on several GPUs in one process) and restores the caller's device afterwards.
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const game_ctx *c)
+    {
+        int cur = -1;
+        if (c && cudaGetDevice(&cur) == cudaSuccess && cur != c->device) { prev = cur; cudaSetDevice(c->device); }
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+// Opt a kernel in to `bytes` of dynamic shared memory.  The attribute is per DEVICE (and per function), so the record of
+// what has been raised lives in the context -- which is bound to one device -- not in a process-wide static.
+inline cudaError_t ensure_smem_attr(game_ctx *c, const void *func, int bytes)
+{
+    int &have = c->smem_attr[func];
+    if (bytes <= have) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) have = bytes;
+    return e;
+}
+
+// kernel<<<grid, block, smem, ctx->stream>>>(args...) with the PDL attribute
 template <typename... KArgs, typename... Args>
-inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args &&...args)
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, const game_ctx *ctx, Args &&...args)
 {
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = pdl_enabled() ? 1 : 0;
+    cfg.attrs = attr; cfg.numAttrs = pdl_enabled(ctx) ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
 // expand.cu
 int launch_check_finite(game_ctx *ctx, const float *X, long long nX, const float *t, long long nT, int *flag_dev);
 int launch_expand_fp32(game_ctx *ctx);      // X -> ET
+int ensure_ET(game_ctx *ctx);               // allocate + build ET on first use (FP32 path, predict, classify)
+int launch_max_abs(game_ctx *ctx, const float *v, long long n, int *flag2_dev);   // flag2[0] |= non-finite, flag2[1] = max|v| bits
+int launch_predict_new(game_ctx *ctx, const float *genes, const float *X_new, long long N_new, float *z_out, float *y_out);
 int launch_expand_fp16(game_ctx *ctx, float *maxabs_dev);   // X -> E16
 int launch_expand_split(game_ctx *ctx);                     // X -> E16s
 int launch_predict(game_ctx *ctx, const float *genes, float *z_out, float *y_out);
@@ -216,8 +253,9 @@ int launch_classify(game_ctx *ctx, const float *genes, float cut, long long *cou
 // fitness_fp32.cu
 size_t fitness_partial_floats(const game_ctx *ctx, int P);
 int launch_fitness_fp32(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer);
-int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, const DevState *state, double *sums = nullptr);
-int launch_fit_from_sums(game_ctx *ctx, const double *sums, int P, long long N_total, float *out);
+int launch_finalize(game_ctx *ctx, int n_chunks, int Ppad, int P, float *out, const DevState *state, double *sums = nullptr,
+                    bool accumulate = false);
+int launch_fit_from_sums(game_ctx *ctx, const double *sums, int P, long long N_total, float *out, const DevState *state);
 // a5 tail + a6 + a7 in one go: final reduction of the slab sums, rank, stop test (single CTA when small)
 int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scratch, int *order, DevState *state,
                 float stop_error);

@@ -29,6 +29,12 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
+# What the TMSE slack is worth: per check, the largest slack / (rtol |ref| + atol) -- how much wider than
+# the plain tolerance the bound was -- and the largest |gpu - ref| / (rtol |ref| + atol) -- whether the slack was needed at
+# all (<= 1: the check passes WITHOUT it).  conftest.py writes the records to $GAME_PARITY_LOG at session end.
+PARITY_LOG = []
+
+
 def check_fitness(orc, gpu_fit, fam, d, X, t, pop, act, err, R, path, what=""):
     rtol, atol, delta = TOL[path]
     if err == TMSE:
@@ -38,7 +44,13 @@ def check_fitness(orc, gpu_fit, fam, d, X, t, pop, act, err, R, path, what=""):
         ref = orc.fitness(fam, d, X, t, pop, act=act, err=err, R=R)
         slack = 0.0
     got = np.asarray(gpu_fit, dtype=np.float64)
-    bound = rtol * np.abs(ref) + atol + slack
+    plain = rtol * np.abs(ref) + atol
+    bound = plain + slack
+    PARITY_LOG.append(dict(what=what, path=int(path), err=int(err), act=int(act), N=int(X.shape[0]), K=int(pop.shape[1]),
+                           rows=int(got.size), slack_over_tol=float(np.max(slack / plain)),
+                           err_over_tol=float(np.max(np.abs(got - ref) / plain)),
+                           err_over_bound=float(np.max(np.abs(got - ref) / bound)),
+                           mean_signed_rel=float(np.mean((got - ref) / np.maximum(np.abs(ref), 1e-300)))))
     bad = np.abs(got - ref) > bound
     assert not bad.any(), "%s: %d/%d off; worst %g (bound %g) at p=%d" % (
         what, bad.sum(), bad.size, np.abs(got - ref).max(), bound[np.abs(got - ref).argmax()],
@@ -258,10 +270,16 @@ def test_error_paths():
 
 
 # ---- whole GA runs, generation by generation, GPU population injected into the oracle (c.4) --------
-def trajectory(orc, w, generations, full_check_every=1, subset=None, selection=0, elite_mode=0):
+def trajectory(orc, w, generations, full_check_every=1, subset=None, selection=0, elite_mode=0, stream=None):
     fam, d = w.family, w.degree
     X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
-    ctx = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    if stream is None:
+        ctx = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    else:                                   # bench.py's launch configuration: the context on its own (capturable) stream
+        ctx = g.Game(fam, d, X.shape[1], stream=stream)
+        ctx.set_activation(w.act)
+        ctx.set_error(w.err, w.R)
+        ctx.load(dev(X), dev(t))
     path = ctx.resolved_path(w.P)
     gp_g = g.ga_params(P=w.P, tournament_size=w.tournament_size, elitism=w.elitism, init_mode=w.init_mode,
                        p_crossover=w.p_crossover, p_mutation=w.p_mutation, selection=selection, elite_mode=elite_mode)
@@ -276,7 +294,7 @@ def trajectory(orc, w, generations, full_check_every=1, subset=None, selection=0
         # (ii) fitness of the GPU's population within tolerance
         if gen % full_check_every == 0 or gen == generations:
             rows = np.arange(w.P) if subset is None else np.sort(rng.choice(w.P, subset, replace=False))
-            check_fitness(orc, fit[rows], fam, d, X, t, pop[rows], w.act, w.err, w.R, path, "gen %d" % gen)
+            check_fitness(orc, fit[rows], fam, d, X, t, pop[rows], w.act, w.err, w.R, path, "%s gen %d" % (w.name, gen))
         # (iii) the rank kernel sorted the GPU's own fitness bits exactly
         assert np.array_equal(order, orc.rank(fit)), gen
         assert res.best_index == order[0] and res.best_error == fit[order[0]]
@@ -318,6 +336,51 @@ def test_trajectory_roulette_and_init_modes_at_scale(orc, cfg, init_mode, select
     from dataclasses import replace
     w = replace(wl.config(cfg), init_mode=init_mode)
     trajectory(orc, w, 3, subset=48 if cfg == 3 else None, selection=selection, elite_mode=elite_mode)
+
+
+@pytest.mark.parametrize("cfg,generations,subset,check_every", [(3, 4, 24, 2), (4, 3, 6, 3), (5, 3, 8, 3)])
+def test_trajectory_full_size_big_configs(orc, cfg, generations, subset, check_every):
+    """SURVEY 8(c) c.4 / 8(g).3 at FULL size on configs 3 (tournament), 4 and 5, in bench.py's launch configuration
+    (context on its own stream, AUTO path): every generation (iii) the rank is the exact sort of the GPU's fitness bits and
+    (iv) oracle.ga_step from the GPU's order reproduces the GPU's next population (P x K genes) bit for bit; (ii) the
+    fitness of a chromosome sample is checked against the oracle at the first and last generation (the oracle needs
+    ~10 s per evaluation at these N x K; the operators cost P x K Philox calls, under a second).  PAPER.md L217-L220 (the
+    loop), L286-L291 (the operators' parameters)."""
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        ctx, pop, fit, order = trajectory(orc, wl.config(cfg), generations, full_check_every=check_every, subset=subset,
+                                          stream=stream)
+    assert ctx.generation() == generations
+
+
+FULL_MODES = [(SIGMOID, MSE, 0.0), (SIGMOID, TMSE, 0.49), (SIGMOID, RMSE, 0.0), (IDENTITY, MSE, 0.0), (IDENTITY, RMSE, 0.0)]
+
+
+@pytest.mark.parametrize("cfg,nsample", [(1, 20), (2, 16), (3, 12), (4, 4), (5, 4)])
+def test_full_size_all_error_and_activation_modes(orc, cfg, nsample):
+    """fitness parity with MSE, TMSE, RMSE and with the identity activation on EVERY config at its full N and
+    P, in the launch configuration bench.py times (AUTO path, full population in one call); the oracle evaluates a sample
+    of the chromosomes (rows of the same launch)."""
+    w = wl.config(cfg)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    rng = np.random.default_rng(100 + cfg)
+    pop_s = wl.uniform_population(w.P, w.K, w.seed)
+    pop_i = (pop_s / np.sqrt(w.K)).astype(np.float32)            # identity output: keep z = O(1)
+    rows = np.unique(np.concatenate([[0, w.P - 1], rng.choice(w.P, nsample, replace=False)]))
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        ctx = g.Game(fam, d, w.F, stream=stream)
+        ctx.load(dev(X), dev(t))
+        path = ctx.resolved_path(w.P)
+        for act, err, R in FULL_MODES:
+            ctx.set_activation(act)
+            ctx.set_error(err, R)
+            pop = pop_s if act == SIGMOID else pop_i
+            got = ctx.fitness(dev(pop)).cpu().numpy()
+            assert np.all(np.isfinite(got))
+            check_fitness(orc, got[rows], fam, d, X, t, pop[rows], act, err, R, path,
+                          "%s full size act %d err %d" % (w.name, act, err))
 
 
 def test_resume_and_single_call_agree(orc):
@@ -663,3 +726,143 @@ def test_split_path_beyond_unit_range(orc):
     ctx.set_activation(IDENTITY)
     got = ctx.fitness(dev(pop)).cpu().numpy()
     check_fitness(orc, got, fam, d, X, t, pop, IDENTITY, MSE, 0.0, g.GAME_PATH_TENSOR_SPLIT, "split identity")
+
+
+# ---- round 2: boundary hardening -----------------------------------------------------------------
+@pytest.mark.parametrize("fam,d,F", [(TRIG, 8, 32), (CHEB, 12, 64), (CHEB, 6, 16), (2, 8, 11), (3, 6, 11), (TRIG, 1, 1)])
+def test_predict_new_equals_load_then_predict(orc, fam, d, F):
+    """game_predict_new (SURVEY 8(f) NEXT-1's signature; a trained chromosome applied to new data) on
+    caller-supplied patterns, with NO dataset loaded, gives the bits of game_load(X_new) + game_predict and matches the
+    oracle's forward pass."""
+    rng = np.random.default_rng(71)
+    N = 3001
+    X = rng.uniform(-1, 1, (N, F)).astype(np.float32)
+    K = orc.num_terms(fam, d, F)
+    genes = (rng.standard_normal(K) / np.sqrt(K) / (F if fam in (2, 3) else 1)).astype(np.float32)
+    fresh = g.Game(fam, d, F)
+    for act in (SIGMOID, IDENTITY):
+        fresh.set_activation(act)
+        z, y = fresh.predict_new(dev(genes), dev(X))
+        ctx = make_ctx(fam, d, X, np.zeros(N, np.float32), act)
+        z2, y2 = ctx.predict(dev(genes))
+        assert torch.equal(z.view(torch.int32), z2.view(torch.int32)) and torch.equal(y.view(torch.int32), y2.view(torch.int32))
+        zr, yr = orc.forward(fam, d, X, genes, act=act)
+        assert np.allclose(z.cpu().numpy(), zr, rtol=1e-5, atol=2e-5) and np.allclose(y.cpu().numpy(), yr, rtol=1e-5, atol=2e-6)
+    assert fresh.generation() == 0 and fresh.population_size() == 0
+
+
+def test_genes_outside_fp16_range_are_not_clamped_silently(orc):
+    """|gene| > 65504 cannot be an fp16 operand: game_set_population routes AUTO to the FP32 path (parity kept) and rejects an
+    explicit tensor path; NaN genes are rejected; a caller-supplied population evaluates that chromosome to NaN on the
+    tensor paths (asynchronous call) and game_fitness_host reports GAME_ERR_UNSUPPORTED."""
+    rng = np.random.default_rng(72)
+    fam, d, F, N, P = CHEB, 3, 8, 3000, 40
+    X = rng.uniform(-1, 1, (N, F)).astype(np.float32)
+    t = rng.integers(0, 2, N).astype(np.float32)
+    pop = rng.uniform(-1, 1, (P, orc.num_terms(fam, d, F))).astype(np.float32)
+    pop[7, 3] = 1.0e5
+    ctx = make_ctx(fam, d, X, t)
+    ctx.set_population(dev(pop))
+    assert ctx.resolved_path(P) == g.GAME_PATH_FP32                      # AUTO falls back, nothing clamped
+    res = ctx.evolve(0, 1, g.ga_params(P=P))
+    _, fit, order = ctx.get_population_host()
+    check_fitness(orc, fit, fam, d, X, t, pop, SIGMOID, MSE, 0.0, g.GAME_PATH_FP32, "big gene, FP32 fallback")
+    assert res.best_index == order[0]
+    for path in (g.GAME_PATH_TENSOR, g.GAME_PATH_TENSOR_SPLIT):
+        c2 = make_ctx(fam, d, X, t, path=path)
+        with pytest.raises(g.GameError) as e:
+            c2.set_population(dev(pop))
+        assert e.value.code == 5
+        assert c2.population_size() == 0                                 # the rejected population was not installed
+        got = c2.fitness(dev(pop)).cpu().numpy()                         # asynchronous call: NaN for THAT chromosome only
+        assert np.isnan(got[7]) and np.isfinite(np.delete(got, 7)).all()
+        ok = np.delete(np.arange(P), 7)
+        check_fitness(orc, got[ok], fam, d, X, t, pop[ok], SIGMOID, MSE, 0.0, path, "others unaffected")
+        with pytest.raises(g.GameError) as e:
+            c2.fitness_host(pop)
+        assert e.value.code == 5
+    bad = pop.copy()
+    bad[7, 3] = np.nan
+    with pytest.raises(g.GameError) as e:
+        ctx.set_population(dev(bad))
+    assert e.value.code == 6
+    pop[7, 3] = 65504.0                                                  # the largest finite fp16: still a tensor-path operand
+    c3 = make_ctx(fam, d, X, t, path=g.GAME_PATH_TENSOR_SPLIT)
+    c3.set_population(dev(pop))
+    assert c3.resolved_path(P) == g.GAME_PATH_TENSOR_SPLIT
+
+
+def test_two_contexts_with_different_shared_memory_needs(orc):
+    """The dynamic-shared-memory opt-in is recorded per context (i.e. per device), not per process: two contexts whose
+    launches of the SAME kernel instantiation need different amounts both run, in either order, and agree with the
+    FFMA path.  (Two devices are not available here; the per-context record is what makes that case work.)"""
+    rng = np.random.default_rng(73)
+    N, P = 148 * 256 + 77, 200
+    shapes = [(CHEB, 3, 32), (TRIG, 8, 32)]           # K = 128 (2 resident k-blocks) and K = 544 (9): same kernel template
+    ctxs, pops = [], []
+    for fam, d, F in shapes:
+        X = rng.uniform(-1, 1, (N, F)).astype(np.float32)
+        t = rng.integers(0, 2, N).astype(np.float32)
+        ctxs.append(make_ctx(fam, d, X, t, path=g.GAME_PATH_TENSOR))
+        pops.append(rng.uniform(-1, 1, (P, ctxs[-1].K)).astype(np.float32))
+    first = [c.fitness(dev(p)).cpu().numpy() for c, p in zip(ctxs, pops)]
+    again = [c.fitness(dev(p)).cpu().numpy() for c, p in reversed(list(zip(ctxs, pops)))][::-1]
+    for c, p, a, b in zip(ctxs, pops, first, again):
+        assert np.array_equal(a.view(np.uint32), b.view(np.uint32))
+        c.set_path(g.GAME_PATH_FP32)
+        ref = c.fitness(dev(p)).cpu().numpy()
+        assert np.allclose(a, ref, rtol=1e-3, atol=1e-5)
+
+
+def test_tuning_knobs_are_per_context():
+    ctx = g.Game(CHEB, 2, 4)
+    for knob, value in ((99, 0), (-1, 0), (g.GAME_TUNE_CTA_GROUP, 3), (g.GAME_TUNE_SIGMOID, 1), (g.GAME_TUNE_POLY_SHARE, 17)):
+        with pytest.raises(g.GameError) as e:
+            ctx.set_tuning(knob, value)
+        assert e.value.code == 1
+    rng = np.random.default_rng(74)
+    X = rng.uniform(-1, 1, (5000, 4)).astype(np.float32)
+    t = rng.integers(0, 2, 5000).astype(np.float32)
+    pop = rng.uniform(-1, 1, (300, ctx.K)).astype(np.float32)
+    a, b = g.Game(CHEB, 2, 4), g.Game(CHEB, 2, 4)
+    b.set_tuning(g.GAME_TUNE_PDL, 0)                   # a launch attribute only: same bits
+    b.set_tuning(g.GAME_TUNE_HALF_TILES, 0)
+    b.set_tuning(g.GAME_TUNE_HALF_TILES, -1)           # back to automatic
+    for c in (a, b):
+        c.load(dev(X), dev(t))
+    fa, fb = a.fitness(dev(pop)), b.fitness(dev(pop))
+    assert torch.equal(fa.view(torch.int32), fb.view(torch.int32))
+
+
+def test_async_advance_with_stop_equals_evolve(orc):
+    """The device-resident sharded loop (asynchronous game_advance, stop flag on the device, polled) against game_evolve
+    with the same stop threshold: same generations applied, same population, same fitness bits."""
+    from paper_1304_0597_b200 import sharded
+    w = wl.config(1)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    probe = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    hist = [probe.evolve(0, w.seed, g.ga_params(P=w.P)).best_error]
+    for _ in range(60):
+        hist.append(probe.evolve(1, w.seed, g.ga_params(P=w.P)).best_error)
+    target = float(hist[37])
+    first = next(i for i, h in enumerate(hist) if h <= target)
+    gp = g.ga_params(P=w.P, stop_error=target)
+    ref = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    r = ref.evolve(60, w.seed, gp)
+    assert r.stopped_on_error == 1 and r.generations_run == first
+
+    def configure(c):
+        c.set_activation(w.act)
+        c.set_error(w.err, w.R)
+    sg = sharded.ShardedGame.load(fam, d, X, t, 1, 0, configure=configure)
+    done, res = sg.evolve(60, w.seed, gp)
+    assert done == first and res.stopped_on_error == 1 and sg.game.generation() == first
+    pr, fr, orr = ref.get_population_host()
+    ps, fs, os_ = sg.game.get_population_host()
+    assert np.array_equal(pr.view(np.uint32), ps.view(np.uint32))
+    assert np.array_equal(fr.view(np.uint32), fs.view(np.uint32)) and np.array_equal(orr, os_)
+    assert res.best_error == r.best_error and res.best_index == r.best_index
+    # a second call continues from the device-side counters and stops at once
+    done2, res2 = sg.evolve(5, w.seed, gp)
+    assert done2 == 0 and res2.stopped_on_error == 1 and sg.game.generation() == first

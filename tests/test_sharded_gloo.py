@@ -30,7 +30,7 @@ WORKER = textwrap.dedent("""
     Xl, tl = X[lo:hi], t[lo:hi]
     gp = oracle.GaParams(P=w.P, tournament_size=3, elitism=2, elite_mode=0, selection=0, init_mode=1,
                          p_crossover=0.9, p_mutation=0.05, stop_error=-1.0)
-    state = {"pop": oracle.init_population(1, w.seed, w.P, w.K), "gen": 0, "fit": None, "order": None, "sums": []}
+    state = {"pop": oracle.init_population(1, w.seed, w.P, w.K), "gen": 0, "fit": None, "order": None, "sums": [], "since": 0}
 
     class Res:
         generations_run = 0
@@ -45,14 +45,17 @@ WORKER = textwrap.dedent("""
         fit = (sums.numpy() / w.N).astype(np.float32)
         order = oracle.rank(fit)
         state["fit"], state["order"] = fit, order
-        r = Res()
         if apply:
             state["pop"] = oracle.ga_step(gp, w.seed, state["gen"], order, fit, state["pop"])
             state["gen"] += 1
-            r.generations_run = 1
+            state["since"] += 1
+
+    def sync():
+        r = Res()
+        r.generations_run, state["since"] = state["since"], 0
         return r
 
-    done, res = sharded.run_generations(evaluate, advance, world, w.generations)
+    done, res = sharded.run_generations(evaluate, advance, sync, world, w.generations, poll_every=2)
     assert done == w.generations and state["gen"] == w.generations and len(state["sums"]) == w.generations + 1
     # every rank holds the same population and fitness, bit for bit
     mine = torch.from_numpy(np.concatenate([state["pop"].view(np.uint32).ravel(), state["fit"].view(np.uint32)]).astype(np.int64))
@@ -96,20 +99,32 @@ def test_chunk_ranges():
 
 def test_single_rank_loop_calls():
     from paper_1304_0597_b200 import sharded
-    calls = []
+    calls, st = [], {"since": 0, "stopped": 0, "polls": 0}
 
     class R:
         def __init__(self, g, s):
             self.generations_run, self.stopped_on_error = g, s
 
-    def adv(s, apply):
+    def adv(s, apply):                       # a device that stops at its 3rd evaluation: later advances are no-ops
         calls.append(apply)
-        return R(1 if apply else 0, 1 if len(calls) == 3 else 0)
-    done, res = sharded.run_generations(lambda: 0, adv, 1, 10)
-    assert done == 3 and calls == [True, True, True] and res.stopped_on_error == 1      # stops, no final evaluation
+        if len(calls) == 3:
+            st["stopped"] = 1
+        if apply and not st["stopped"]:
+            st["since"] += 1
+
+    def sync():
+        st["polls"] += 1
+        r = R(st["since"], st["stopped"])
+        st["since"] = 0
+        return r
+    done, res = sharded.run_generations(lambda: 0, adv, sync, 1, 10, poll_every=4)
+    # the stop is noticed at the first poll (after 4 enqueued generations): 2 applied, no final evaluation
+    assert done == 2 and calls == [True] * 4 and res.stopped_on_error == 1 and st["polls"] == 1
     calls.clear()
-    done, _ = sharded.run_generations(lambda: 0, lambda s, a: (calls.append(a), R(1 if a else 0, 0))[1], 1, 2)
-    assert done == 2 and calls == [True, True, False]
+    st.update(since=0, stopped=0, polls=0)
+    done, _ = sharded.run_generations(lambda: 0, lambda s, a: (calls.append(a), st.__setitem__("since", st["since"] + a)), sync, 1,
+                                      2, can_stop=False)
+    assert done == 2 and calls == [True, True, False] and st["polls"] == 1              # no threshold: one sync at the end
 
 
 def test_two_rank_sharded_run(tmp_path):
