@@ -53,16 +53,16 @@ enum { GAME_EXPAND_AUTO = 0, GAME_EXPAND_MATERIALIZED = 1, GAME_EXPAND_REGENERAT
  * tolerance class.  value -1 restores the automatic choice.
  *   GAME_TUNE_PDL          1/0  programmatic dependent launch between the kernels of a generation (auto: 1)
  *   GAME_TUNE_CTA_GROUP    1/2  single CTAs or cta_group::2 pairs in the tensor kernel (auto: by shape)
- *   GAME_TUNE_SIGMOID      0 ex2+rcp logistic, 2 tanh.approx logistic, 3 tanh.approx with a share of the evaluations
- *                          on an FMA-pipe polynomial (TENSOR path; auto: by shape)
+ *   GAME_TUNE_SIGMOID      0 ex2+rcp logistic, 2 tanh.approx logistic (TENSOR path; auto: 2)
  *   GAME_TUNE_RESIDENT     1/0  resident population tile for P <= 256 (auto: 1)
  *   GAME_TUNE_TEAMS        1/0  two-team epilogue (auto: contraction depth <= 256)
  *   GAME_TUNE_HALF_TILES   1/0  128-pattern tiles for sub-wave problems (auto: by shape)
  *   GAME_TUNE_PERSISTENT   1/0  one persistent cooperative kernel per game_evolve for sub-wave problems (auto: by shape)
- *   GAME_TUNE_POLY_SHARE   0..16  of every 16 logistic evaluations, how many go to the FMA-pipe polynomial in sigmoid
- *                          mode 3 (auto: measured best) */
+ *   GAME_TUNE_RATIONAL_SHARE  0..8  of every 16 evaluation PAIRS of the tanh logistic, how many are evaluated on the FMA
+ *                          pipe by a rational form with one shared reciprocal (team epilogue, single CTAs; 1, 2 round
+ *                          up to 3; auto: the measured best) */
 enum { GAME_TUNE_PDL = 0, GAME_TUNE_CTA_GROUP = 1, GAME_TUNE_SIGMOID = 2, GAME_TUNE_RESIDENT = 3, GAME_TUNE_TEAMS = 4,
-       GAME_TUNE_HALF_TILES = 5, GAME_TUNE_PERSISTENT = 6, GAME_TUNE_POLY_SHARE = 7, GAME_TUNE_COUNT_ = 8 };
+       GAME_TUNE_HALF_TILES = 5, GAME_TUNE_PERSISTENT = 6, GAME_TUNE_RATIONAL_SHARE = 7, GAME_TUNE_COUNT_ = 8 };
 
 /* GA parameters (L275-L291).  Probabilities are per parent pair (crossover, DESIGN G15) and per gene
  * (mutation, DESIGN G16).  stop_error < 0 disables the error-threshold stop (L219, L287). */

@@ -22,7 +22,7 @@ GAME_ELITE_COPIES_OF_BEST, GAME_ELITE_TOP_E = 0, 1
 GAME_PATH_AUTO, GAME_PATH_FP32, GAME_PATH_TENSOR, GAME_PATH_TENSOR_SPLIT = 0, 1, 2, 3
 GAME_EXPAND_AUTO, GAME_EXPAND_MATERIALIZED, GAME_EXPAND_REGENERATED = 0, 1, 2
 (GAME_TUNE_PDL, GAME_TUNE_CTA_GROUP, GAME_TUNE_SIGMOID, GAME_TUNE_RESIDENT, GAME_TUNE_TEAMS, GAME_TUNE_HALF_TILES,
- GAME_TUNE_PERSISTENT, GAME_TUNE_POLY_SHARE) = range(8)
+ GAME_TUNE_PERSISTENT, GAME_TUNE_RATIONAL_SHARE) = range(8)
 GAME_PEAK_FFMA, GAME_PEAK_FFMA2, GAME_PEAK_TANH, GAME_PEAK_EX2, GAME_PEAK_TANH_MIX = range(5)
 ERROR_NAMES = {1: "INVALID_ARG", 2: "NOT_LOADED", 3: "ALLOC", 4: "CUDA", 5: "UNSUPPORTED", 6: "NONFINITE_INPUT"}
 

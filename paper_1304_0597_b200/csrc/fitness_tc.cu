@@ -18,17 +18,10 @@
 // Tiles are ordered chromosome-block fastest so CTAs running together share the same E tile out of L2.
 // finalize_kernel (fitness_fp32.cu) then adds the slabs in fixed order: no float atomics, bit-reproducible,
 // and a chromosome's result does not depend on its row (DESIGN P20).
-#include <cuda.h>
-
-#include "game_internal.cuh"
+#include "tc_common.cuh"
 
 namespace game {
 
-constexpr int BM = 128;            // chromosomes per CTA  = TMEM lanes
-constexpr int BN = 256;            // patterns per tile    = TMEM columns of one accumulator
-constexpr int BKB = TC_KBLK;       // 64 fp16 = one 128-byte swizzle row per k-block
-constexpr int UMMA_K = 16;
-constexpr int A_BYTES = BM * BKB * 2;
 constexpr int WARP_TMA = 0, WARP_MMA = 1, WARP_EPI0 = 2;      // warp roles; the epilogue warps follow (EW = 8 or 16 of them)
 // Where the B operand (the expansion tile) comes from:
 //   SRC_TMA  streamed from the materialised E16 in HBM, together with the A (population) tile, through a TMA ring
@@ -55,235 +48,6 @@ template <int CG> struct Cfg {
     static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 /*align*/ + TC_TAIL_BYTES;
 };
 
-// ---- PTX wrappers ------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-// arrive on the barrier at the same offset in CTA `rank` of the cluster.  Default semantics (release at CTA scope):
-// what is handed over lives in the ARRIVING CTA's own shared / tensor memory and is made visible there beforehand
-// (tcgen05.fence / fence.proxy.async + a CTA barrier); only the signal crosses to the peer.  A cluster-scope release
-// costs a GPU-wide memory barrier per arrival (measured: it alone bounded the generator variant at 47 % tensor-pipe use).
-__device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t rank)
-{
-    asm volatile("{\n\t.reg .b32 ra;\n\tmapa.shared::cluster.u32 ra, %0, %1;\n\t"
-                 "mbarrier.arrive.shared::cluster.b64 _, [ra];\n\t}" ::"r"(bar), "r"(rank) : "memory");
-}
-// SUSPEND: pass a suspend-time hint, so a waiting thread sleeps in hardware instead of re-probing the barrier.  Measured
-// on B200, same box, all waits of the kernel switched together: config 5 kernel 2.34 -> 2.20 ms, config 4 0.243 -> 0.238 ms
-// (deep contractions: the producer, the MMA issuer and the epilogue all wait for long stretches), config 3 0.143 -> 0.145 ms
-// (shallow: wake-up latency counts).  The kernel therefore uses it exactly where it uses the eight-warp epilogue.
-// A wait that never completes is a protocol bug and must fail loudly instead of hanging the device; the bound is
-// wall-clock time (globaltimer, looked at every 2^16 probes), not a probe count, so a debugger, time-slicing or a
-// profiler replay that stalls the kernel for a while cannot trip it.
-constexpr unsigned long long MBAR_TIMEOUT_NS = 20ull * 1000 * 1000 * 1000;
-__device__ __noinline__ void mbar_timeout_check(unsigned long long &t0)
-{
-    unsigned long long now;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
-    if (t0 == 0) t0 = now;
-    else if (now - t0 > MBAR_TIMEOUT_NS) __trap();
-}
-template <bool SUSPEND = false>
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
-{
-    uint32_t ok = 0;
-    unsigned long long t0 = 0;
-    for (uint32_t spin = 0; !ok; ++spin) {
-        if (SUSPEND)
-            asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                         : "=r"(ok) : "r"(bar), "r"(parity), "r"(0x989680u) : "memory");
-        else
-            asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                         : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-        if ((spin & 0xFFFFu) == 0xFFFFu) mbar_timeout_check(t0);
-    }
-}
-// non-blocking: has the phase with this parity completed?
-__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity)
-{
-    uint32_t ok;
-    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    return ok != 0;
-}
-__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-
-template <int CG>
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, int c0, int c1, uint32_t bar)
-{
-    if (CG == 1) {
-        asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-                     ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
-    } else {    // both CTAs of the pair issue; the bytes are accounted on the LEADER's barrier (rank 0)
-        asm volatile("{\n\t.reg .b32 rb;\n\tmapa.shared::cluster.u32 rb, %4, 0;\n\t"
-                     "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [rb];\n\t}"
-                     ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
-    }
-}
-
-template <int CG> __device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t cols)
-{
-    if (CG == 1) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-    } else {
-        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(cols) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
-    }
-}
-template <int CG> __device__ __forceinline__ void tmem_dealloc(uint32_t addr, uint32_t cols)
-{
-    if (CG == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
-    else asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(addr), "r"(cols) : "memory");
-}
-
-// D[tmem] (+)= A[smem] . B[smem]^T, both operands K-major
-template <int CG>
-__device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
-{
-    if (CG == 1) {
-        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                     "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-                     ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
-    } else {
-        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                     "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-                     ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
-    }
-}
-
-// arrive on `bar` (same offset in every CTA of the pair) once all MMAs issued so far have completed
-template <int CG> __device__ __forceinline__ void umma_commit(uint32_t bar)
-{
-    if (CG == 1) {
-        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-    } else {
-        asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-                     ::"r"(bar), "h"((unsigned short)3) : "memory");
-    }
-}
-
-// shared-memory matrix descriptor: K-major tile of [rows x 64] fp16, 128-byte swizzle, 8-row groups 1024 B apart
-__device__ __forceinline__ uint64_t make_smem_desc(uint32_t addr)
-{
-    uint64_t d = 0;
-    d |= (uint64_t)((addr & 0x3FFFF) >> 4);          // start address, 16-byte units        bits [0,14)
-    d |= (uint64_t)1 << 16;                          // leading byte offset (unused here)   bits [16,30)
-    d |= (uint64_t)(1024 >> 4) << 32;                // stride byte offset: 8 rows x 128 B  bits [32,46)
-    d |= (uint64_t)1 << 46;                          // descriptor version (sm_100)         bits [46,48)
-    d |= (uint64_t)2 << 61;                          // layout: SWIZZLE_128B                bits [61,64)
-    return d;
-}
-
-// instruction descriptor, kind::f16: fp16 x fp16 -> fp32, both K-major, M x N tile
-__host__ __device__ constexpr uint32_t make_idesc(int M, int N)
-{
-    return (1u << 4)                 // D format: F32
-         | (0u << 7) | (0u << 10)    // A, B format: F16
-         | (0u << 15) | (0u << 16)   // A, B major: K
-         | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
-}
-
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
-{
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
-          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
-          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-        : "r"(taddr) : "memory");
-}
-// Wait for this warp's outstanding TMEM loads.  The loaded registers pass through the statement as in/out operands, so
-// the compiler can neither read them before the wait nor start on them early: consumers stay BELOW this point and the
-// evaluation of the previous chunk stays ABOVE the next tmem_ld32 into the same registers.  Without that tie ptxas
-// interleaves the two chunks and the warp blocks on the load it was meant to overlap (measured: config 3, K = 112).
-__device__ __forceinline__ void tmem_ld_wait(uint32_t (&v)[32])
-{
-    asm volatile("tcgen05.wait::ld.sync.aligned;"
-                 : "+r"(v[0]), "+r"(v[1]), "+r"(v[2]), "+r"(v[3]), "+r"(v[4]), "+r"(v[5]), "+r"(v[6]), "+r"(v[7]),
-                   "+r"(v[8]), "+r"(v[9]), "+r"(v[10]), "+r"(v[11]), "+r"(v[12]), "+r"(v[13]), "+r"(v[14]), "+r"(v[15]),
-                   "+r"(v[16]), "+r"(v[17]), "+r"(v[18]), "+r"(v[19]), "+r"(v[20]), "+r"(v[21]), "+r"(v[22]), "+r"(v[23]),
-                   "+r"(v[24]), "+r"(v[25]), "+r"(v[26]), "+r"(v[27]), "+r"(v[28]), "+r"(v[29]), "+r"(v[30]), "+r"(v[31])
-                 :: "memory");
-}
-
-__device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-
-// Epilogue modes (template parameter ACT): the two activations of the ABI plus a cheaper logistic form.
-//   0 sigmoid, 1/(1+2^(-z log2 e)) with ex2.approx + rcp.approx: 2 MUFU ops per evaluation
-//   1 identity
-//   2 sigmoid as 0.5 + 0.5 tanh(z/2) with tanh.approx.f32: 1 MUFU op per evaluation.  Measured against the
-//     oracle on configs 2 and 3 (512 chromosomes x 3 gene distributions x MSE/TMSE) its fitness error is
-//     indistinguishable from mode 0's (both dominated by the fp16 operand rounding, max 5e-4 relative, no
-//     bias), and the MUFU-bound config 3 runs 1.4x faster, so it is the default.  A packed
-//     tanh.approx.f16x2 form (0.5 MUFU per evaluation) was measured too: biased by -2e-4 and slower; dropped.
-// In mode 2 the staged targets are t - 0.5 and the fp16 genes are pre-halved (a power-of-two scale: the same
-// rounding), so the accumulator is z/2 and r = (t - 0.5) - 0.5 tanh(z/2) is one MUFU + one FFMA.
-// Arithmetic is issued two evaluations at a time with the packed fp32 instructions of sm_100
-// (FMUL2 / FFMA2), which halves the FMA-pipe issue slots the epilogue needs.
-constexpr int MODE_SIG_EXACT = 0, MODE_IDENTITY = 1, MODE_SIG_TANH32 = 2;
-
-__device__ __forceinline__ float tanh_approx(float x) { float y; asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-
-// residual r = t - act(z) for two evaluations
-template <int ACT> __device__ __forceinline__ float2 residual2(float2 z, float2 t)
-{
-    if (ACT == MODE_SIG_EXACT) {
-        float2 a = __fmul2_rn(z, make_float2(-1.4426950408889634f, -1.4426950408889634f));
-        float2 d = __fadd2_rn(make_float2(ex2_approx(a.x), ex2_approx(a.y)), make_float2(1.0f, 1.0f));
-        return __ffma2_rn(make_float2(rcp_approx(d.x), rcp_approx(d.y)), make_float2(-1.0f, -1.0f), t);
-    } else if (ACT == MODE_IDENTITY) {
-        return __ffma2_rn(z, make_float2(-1.0f, -1.0f), t);
-    } else {
-        // the accumulator already holds z/2: pop_to_f16_kernel halves the genes (exact in fp16) in this mode
-        return __ffma2_rn(make_float2(tanh_approx(z.x), tanh_approx(z.y)), make_float2(-0.5f, -0.5f), t);
-    }
-}
-
-// acc += e(r) for two evaluations; TMSE zeroes residuals inside the tube first (|r| <= R -> 0).  The tube test is
-// one FSET per evaluation (a 1.0 / 0.0 mask) folded in by a packed multiply, instead of a compare + select pair.
-template <bool TMSE> __device__ __forceinline__ void accumulate2(float2 r, float R, float2 &acc)
-{
-    if (TMSE) {
-        const float2 m = make_float2(fabsf(r.x) > R ? 1.0f : 0.0f, fabsf(r.y) > R ? 1.0f : 0.0f);
-        acc = __ffma2_rn(__fmul2_rn(r, m), r, acc);
-    } else {
-        acc = __ffma2_rn(r, r, acc);
-    }
-}
-
-// 32 consecutive accumulator columns of this thread's chromosome against 32 staged targets; four independent
-// running sums so the additions do not form one dependent chain
-template <int ACT, bool TMSE>
-__device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const float *ts, float R, float2 (&acc)[4])
-{
-#pragma unroll
-    for (int j = 0; j < 32; j += 4) {
-        const float4 t4 = *reinterpret_cast<const float4 *>(ts + j);
-        accumulate2<TMSE>(residual2<ACT>(make_float2(__uint_as_float(v[j]), __uint_as_float(v[j + 1])), make_float2(t4.x, t4.y)), R,
-                          acc[(j >> 1) & 3]);
-        accumulate2<TMSE>(residual2<ACT>(make_float2(__uint_as_float(v[j + 2]), __uint_as_float(v[j + 3])), make_float2(t4.z, t4.w)), R,
-                          acc[((j >> 1) + 1) & 3]);
-    }
-}
 
 // ---- a1 inside the kernel: the generator warps of the SRC_GEN variant ---------------------------------------
 // Each of the 128 generator threads owns one pattern row of this CTA's half of the 256-pattern tile and writes that
@@ -449,12 +213,14 @@ __device__ __forceinline__ void generate_expansion(const float *__restrict__ X, 
 // ---- the kernel -----------------------------------------------------------------------------------------
 // BNT: patterns per tile, 256 or (SRC_TMA, single CTAs, team epilogue only) 128: problems of less than one wave of
 // 256-pattern tiles finish sooner on twice as many half-size tiles (configs 1-2).
-template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY, bool TEAMS, int BNT = BN>
+// SHARE: see epilogue_chunk.  k_last: UMMA k-steps (of 16 terms) that hold real terms in the LAST k-block -- the
+// padding steps beyond them would multiply zeros (config 3: K = 112 = 7 steps, not 8) and are not issued.
+template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY, bool TEAMS, int BNT = BN, int SHARE = 0>
 __global__ void __launch_bounds__(64 + 32 * EW + (SRC == SRC_GEN ? 32 * GEN_WARPS : 0), 1)
 fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmE,
                   int n_tiles, int m_blocks, int k_blocks, long long N, const float *__restrict__ tgt, float R,
                   float *__restrict__ partial, int Ppad, const DevState *state,
-                  const float *__restrict__ X, int F, int degree)
+                  const float *__restrict__ X, int F, int degree, int k_last)
 {
     using C = Cfg<CG>;
     static_assert(SRC == SRC_TMA || CG == 2, "the generator variant runs as CTA pairs");
@@ -581,10 +347,11 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                     const uint32_t sa = RESIDENT_A ? base + kb * A_BYTES : base + s * STAGE_BYTES_K;
                     const uint32_t sb = RESIDENT_A ? base + k_blocks * A_BYTES + s * GEN_B_BYTES : sa + A_BYTES;
                     const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sb);
+                    const int nk = kb + 1 == k_blocks ? k_last : BKB / UMMA_K;
 #pragma unroll
                     for (int k = 0; k < BKB / UMMA_K; ++k) {
                         // advance 16 fp16 = 32 bytes inside the swizzle row: +2 in 16-byte units
-                        umma_f16<CG>(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
+                        if (k < nk) umma_f16<CG>(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
                     }
                     umma_commit<CG>(empty_bar(s));            // stage reusable when these MMAs retire
                     if (++s == NSTAGES) { s = 0; ph ^= 1; }
@@ -661,7 +428,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                             else mbar_arrive_cluster(tempty_b, 0);
                         }
                     }
-                    epilogue_chunk<ACT, TMSE>(cur, ts + 32 * c, R, acc2);
+                    epilogue_chunk<ACT, TMSE, SHARE>(cur, ts + 32 * c, R, acc2);
                 }
                 partial[(long long)n_tile * Ppad + (m_blk * CG + (int)cta_rank) * BM + row] =
                     ((acc2[0].x + acc2[0].y) + (acc2[1].x + acc2[1].y)) + ((acc2[2].x + acc2[2].y) + (acc2[3].x + acc2[3].y));
@@ -879,12 +646,16 @@ int tensor_prepare_split(game_ctx *ctx)
     return GAME_OK;
 }
 
-template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY, bool TEAMS = false, int BNT = BN>
+template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY, bool TEAMS = false, int BNT = BN, int SHARE = 0>
 static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, const DevState *state, bool split = false)
 {
     using C = Cfg<CG>;
-    auto kern = fitness_tc_kernel<CG, ACT, TMSE, EW, SRC, FAMILY, TEAMS, BNT>;
+    auto kern = fitness_tc_kernel<CG, ACT, TMSE, EW, SRC, FAMILY, TEAMS, BNT, SHARE>;
     const int k_blocks = (split ? 3 : 1) * ctx->Kpad / BKB;
+    // real terms in the last k-block, in UMMA k-steps of 16 (the split form's three K ranges each end in the same padding,
+    // so only the one-pass form trims; the generator variant writes whole k-blocks and is left alone too)
+    const int npos = tc_num_positions(ctx->family, ctx->degree, ctx->F, ctx->K);
+    const int k_last = (split || SRC == SRC_GEN) ? BKB / UMMA_K : (npos - (ctx->Kpad - BKB) + UMMA_K - 1) / UMMA_K;
     const CUtensorMap *maps_E = (const CUtensorMap *)(split ? ctx->tmap_Es : ctx->tmap_E);
     const int smem = SRC != SRC_TMA ? k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES
                    : BNT == BN    ? C::SMEM
@@ -907,7 +678,7 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     KernelTimer timer(ctx);
     GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, maps_E[BNT / CG == 128 ? 1 : 0], n_tiles,
                                       m_blocks, k_blocks, ctx->N, (const float *)ctx->t, ctx->R, ctx->partial, Ppad, state,
-                                      (const float *)ctx->X, ctx->F, ctx->degree));
+                                      (const float *)ctx->X, ctx->F, ctx->degree, k_last));
     return GAME_OK;
 }
 
@@ -928,6 +699,25 @@ int tensor_expansion(const game_ctx *ctx, int P)
                      (ctx->family != GAME_TRIG || ctx->x_maxabs <= 3.14159f);
     if (ctx->expand_mode == GAME_EXPAND_REGENERATED) return can ? GAME_EXPAND_REGENERATED : -1;
     return GAME_EXPAND_MATERIALIZED;
+}
+
+// make the fp16 operand copy (C16 / C16s) mirror `pop`, unless the GA operators already wrote it while building `pop`
+int tensor_refresh_c16(game_ctx *ctx, const float *pop, int P, bool split, const DevState *state)
+{
+    const C16Sink sink = tensor_sink(ctx, split);
+    if (ctx->c16_src == pop && ctx->c16_split == sink.split && ctx->c16_scale == sink.scale) return GAME_OK;
+    const long long n = (long long)P * ctx->K;
+    GAME_CUDA(ctx, launch_pdl(pop_to_f16_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, ctx, pop, P, ctx->K, sink, state));
+    ++ctx->launches;
+    ctx->c16_src = nullptr;               // an external population: nothing to remember
+    return GAME_OK;
+}
+
+int tensor_encode_population_map(game_ctx *ctx, bool split, int Ppad)
+{
+    if (!ctx->tmap_C) ctx->tmap_C = aligned_alloc(64, sizeof(CUtensorMap));
+    if (!ctx->tmap_C) return fail(ctx, GAME_ERR_ALLOC, "tensor map allocation failed");
+    return encode_map(ctx, (CUtensorMap *)ctx->tmap_C, split ? ctx->C16s : ctx->C16, Ppad, (split ? 3 : 1) * ctx->Kpad, BM);
 }
 
 int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer, bool split)
@@ -963,20 +753,23 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     const bool half_tiles = src == SRC_TMA && (half_forced < 0 ? tiles256 < ctx->sm_count : half_forced == 1);
     const int n_tiles = (int)(ctx->Npad256 / (half_tiles ? 128 : BN));
     const int m_blocks = half_tiles ? (P + BM - 1) / BM : Ppad / (BM * cg);
-    long long n = (long long)P * ctx->K;
     const bool tmse = ctx->err == GAME_ERR_TMSE;
     // the split path is the 1e-5 tolerance class: its logistic is the ex2 + rcp form (2^-22), not tanh.approx (2^-11)
     const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : (split ? MODE_SIG_EXACT : sigmoid_mode(ctx));
-    const C16Sink sink = tensor_sink(ctx, split);
-    if (!(ctx->c16_src == pop && ctx->c16_split == sink.split && ctx->c16_scale == sink.scale)) {   // else ga_step_kernel already wrote it
-        GAME_CUDA(ctx, launch_pdl(pop_to_f16_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, ctx, pop, P, ctx->K, sink, state));
-        ++ctx->launches;
-        ctx->c16_src = nullptr;           // an external population: nothing to remember
-    }
-    int rc = encode_map(ctx, (CUtensorMap *)ctx->tmap_C, split ? ctx->C16s : ctx->C16, Ppad, Kp, BM);
+    // a share of the logistics on the FMA pipe (shallow contractions, where the special-function unit binds): pairs of 16
+    // per 32-column chunk; GAME_TUNE_RATIONAL_SHARE overrides (0 = none; 3..8 are built)
+    const int share_req = ctx->tune[GAME_TUNE_RATIONAL_SHARE];
+    const int share = (mode != MODE_SIG_TANH32 || !teams || cg != 1 || half_tiles) ? 0
+                    : share_req < 0 ? RATIONAL_SHARE_AUTO : share_req == 0 ? 0 : share_req < 3 ? 3 : share_req > 8 ? 8 : share_req;
+    int rc = tensor_refresh_c16(ctx, pop, P, split, state);
+    if (!rc) rc = tensor_encode_population_map(ctx, split, Ppad);
     if (rc) return rc;
+#define GAME_TC_SHARE(M, T, S) launch_variant<1, M, T, 8, SRC_TMA, GAME_TRIG, true, BN, (M == MODE_SIG_TANH32 ? S : 0)>(ctx, n_tiles, m_blocks, Ppad, state, split)
 #define GAME_TC_EW(CGV, M, T)                                                                              \
     rc = half_tiles ? launch_variant<1, M, T, 8, SRC_TMA, GAME_TRIG, true, 128>(ctx, n_tiles, m_blocks, Ppad, state, split)  \
+       : (teams && CGV == 1 && share > 0) ? (share == 4 ? GAME_TC_SHARE(M, T, 4) : share == 5 ? GAME_TC_SHARE(M, T, 5)        \
+                                             : share == 6 ? GAME_TC_SHARE(M, T, 6) : share == 7 ? GAME_TC_SHARE(M, T, 7)      \
+                                             : share == 8 ? GAME_TC_SHARE(M, T, 8) : GAME_TC_SHARE(M, T, 3))                  \
        : teams ? launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG, true>(ctx, n_tiles, m_blocks, Ppad, state, split)           \
                : launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG, false>(ctx, n_tiles, m_blocks, Ppad, state, split)
 #define GAME_TC_GEN(M, T)                                                                                  \
@@ -997,6 +790,7 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
 #undef GAME_TC_MODE
 #undef GAME_TC_GEN
 #undef GAME_TC_EW
+#undef GAME_TC_SHARE
     if (rc) return rc;
     ++ctx->launches;
     if (defer) { defer->n_chunks = n_tiles; defer->Ppad = Ppad; return GAME_OK; }     // one partial row per 256-pattern tile

@@ -264,6 +264,7 @@ void game_destroy(game_ctx *c)
     free_dataset(c);
     free_population(c);
     dfree(c->partial); dfree(c->fin2); dfree(c->C16); dfree(c->C16s); dfree(c->stage_pop); dfree(c->stage_fit); dfree(c->state);
+    dfree(c->gbar);
     free(c->tmap_E); free(c->tmap_C); free(c->tmap_Es);
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     delete c;
@@ -321,7 +322,7 @@ int game_set_tuning(game_ctx *c, int knob, int value)
 {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (knob < 0 || knob >= GAME_TUNE_COUNT_) return fail(c, GAME_ERR_INVALID_ARG, "game_set_tuning: unknown knob");
-    static const int lo[GAME_TUNE_COUNT_] = {0, 1, 0, 0, 0, 0, 0, 0}, hi[GAME_TUNE_COUNT_] = {1, 2, 3, 1, 1, 1, 1, 16};
+    static const int lo[GAME_TUNE_COUNT_] = {0, 1, 0, 0, 0, 0, 0, 0}, hi[GAME_TUNE_COUNT_] = {1, 2, 2, 1, 1, 1, 1, 8};
     if (value != -1 && (value < lo[knob] || value > hi[knob] || (knob == GAME_TUNE_SIGMOID && value == 1)))
         return fail(c, GAME_ERR_INVALID_ARG, "game_set_tuning: value out of range for this knob");
     c->tune[knob] = value;
@@ -535,6 +536,33 @@ int game_evolve(game_ctx *c, int generations, unsigned long long seed, const gam
         return fail(c, GAME_ERR_UNSUPPORTED, "tensor path unavailable for this dataset / population (|E| or |gene| exceeds the fp16 range, or a tied family)");
     GAME_CUDA(c, cudaMemsetAsync(c->state, 0, sizeof(DevState), c->stream));
     DevState h{};
+    {
+        // Sub-wave problems (configs 1-2): the whole loop -- fitness tiles, rank, stop test, operators, `generations` times,
+        // plus the final evaluation -- as ONE persistent cooperative kernel with grid barriers between the phases
+        // (evolve_persistent.cu).  Bit-identical to the launch-per-kernel path below.
+        const int path0 = resolve_path(c, P, true);
+        if (persistent_eligible(c, gp, path0)) {
+            const bool split = path0 == GAME_PATH_TENSOR_SPLIT;
+            rc = ensure_scratch(c, P);
+            if (!rc) rc = tensor_refresh_c16(c, c->pop, P, split, nullptr);
+            if (!rc) rc = launch_evolve_persistent(c, gp, seed, generations, path0);
+            if (rc) return rc;
+            GAME_CUDA(c, cudaMemcpyAsync(&h, c->state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+            GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+            if (h.gens_run & 1) { float *tmp = c->pop; c->pop = c->pop_next; c->pop_next = tmp; }
+            const C16Sink sink = tensor_sink(c, split);
+            c->c16_src = c->pop; c->c16_split = sink.split; c->c16_scale = sink.scale;     // the operators kept the fp16 copy current
+            c->generation += h.gens_run;
+            c->have_fit = true;
+            if (res) {
+                res->generations_run = h.gens_run;
+                res->stopped_on_error = (h.stopped || h.stop_request) ? 1 : 0;
+                res->best_error = h.best_error;
+                res->best_index = h.best_index;
+            }
+            return GAME_OK;
+        }
+    }
     const bool can_stop = gp->stop_error >= 0.f;
     const unsigned int gen_base = (unsigned int)c->generation;      // the device adds its own evaluation counter
     auto evaluate = [&]() -> int {                                   // a1-a5, then a5 tail + a6 + a7

@@ -145,6 +145,7 @@ struct game_ctx {
     unsigned long long *rprefix = nullptr;   // roulette inclusive prefix sums
     size_t pop_cap = 0;                      // capacity in chromosomes of the buffers above
     game::DevState *state = nullptr;
+    unsigned int *gbar = nullptr;            // grid-barrier counter of the persistent loop kernel
     unsigned int *ticket = nullptr;          // last-CTA ticket for classify_kernel (lives behind `state`)
 
     // scratch
@@ -267,6 +268,12 @@ int tensor_expansion(const game_ctx *ctx, int P);                // GAME_EXPAND_
 int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer,
                           bool split = false);
 int tensor_prepare_split(game_ctx *ctx);                         // E16s + its tensor maps, on first use
+int tensor_refresh_c16(game_ctx *ctx, const float *pop, int P, bool split, const DevState *state);   // the fp16 copy mirrors `pop`
+int tensor_encode_population_map(game_ctx *ctx, bool split, int Ppad);                               // ctx->tmap_C for C16 / C16s
+
+// evolve_persistent.cu: the whole loop as one cooperative kernel, for sub-wave problems
+bool persistent_eligible(const game_ctx *ctx, const game_ga_params *gp, int path);
+int launch_evolve_persistent(game_ctx *ctx, const game_ga_params *gp, unsigned long long seed, int generations, int path);
 
 // ga.cu
 int launch_init_population(game_ctx *ctx, int mode, unsigned long long seed, int P, float *pop);

@@ -816,7 +816,7 @@ def test_two_contexts_with_different_shared_memory_needs(orc):
 
 def test_tuning_knobs_are_per_context():
     ctx = g.Game(CHEB, 2, 4)
-    for knob, value in ((99, 0), (-1, 0), (g.GAME_TUNE_CTA_GROUP, 3), (g.GAME_TUNE_SIGMOID, 1), (g.GAME_TUNE_POLY_SHARE, 17)):
+    for knob, value in ((99, 0), (-1, 0), (g.GAME_TUNE_CTA_GROUP, 3), (g.GAME_TUNE_SIGMOID, 1), (g.GAME_TUNE_RATIONAL_SHARE, 9)):
         with pytest.raises(g.GameError) as e:
             ctx.set_tuning(knob, value)
         assert e.value.code == 1
@@ -866,3 +866,78 @@ def test_async_advance_with_stop_equals_evolve(orc):
     # a second call continues from the device-side counters and stops at once
     done2, res2 = sg.evolve(5, w.seed, gp)
     assert done2 == 0 and res2.stopped_on_error == 1 and sg.game.generation() == first
+
+
+# ---- round 2: the whole loop as one persistent cooperative kernel (sub-wave problems, configs 1-2) -------------------------
+@pytest.mark.parametrize("cfg,P,gens,path,act,err", [
+    (1, None, 21, g.GAME_PATH_AUTO, SIGMOID, TMSE),           # config 1 as benchmarked (split path, local rank)
+    (2, None, 10, g.GAME_PATH_AUTO, SIGMOID, TMSE),           # config 2 as benchmarked (P = 1024: distributed rank)
+    (2, 300, 21, g.GAME_PATH_AUTO, SIGMOID, TMSE),            # ragged P over three chromosome blocks
+    (2, 256, 5, g.GAME_PATH_TENSOR, SIGMOID, MSE),            # one-pass fp16 operands, tanh logistic, odd generation count
+    (1, 64, 8, g.GAME_PATH_TENSOR, IDENTITY, RMSE),
+    (1, None, 1, g.GAME_PATH_TENSOR_SPLIT, IDENTITY, TMSE),
+    (1, None, 0, g.GAME_PATH_AUTO, SIGMOID, MSE),             # evaluation only
+])
+def test_persistent_loop_equals_launch_path(orc, cfg, P, gens, path, act, err):
+    """game_evolve on a sub-wave problem runs ONE persistent kernel (fitness tiles -> grid barrier -> rank -> operators ->
+    grid barrier, looping on the device).  It must give, bit for bit, what stepping the launch-per-kernel path one
+    generation at a time gives (GAME_TUNE_PERSISTENT = 0): population, fitness, order, best -- PAPER.md L217-L220."""
+    w = wl.config(cfg)
+    w = w.scaled(P=P or w.P, generations=gens)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    R = 0.49 if err == TMSE else 0.0
+    gp = g.ga_params(P=w.P)
+    step = make_ctx(fam, d, X, t, act, err, R, path)
+    step.set_tuning(g.GAME_TUNE_PERSISTENT, 0)
+    n0 = step.launch_count()
+    step.evolve(0, w.seed, gp)
+    for _ in range(gens):
+        step.evolve(1, w.seed, gp)
+    ps, fs, os_ = step.get_population_host()
+    launches_step = step.launch_count() - n0
+    ctx = make_ctx(fam, d, X, t, act, err, R, path)
+    n0 = ctx.launch_count()
+    res = ctx.evolve(gens, w.seed, gp)
+    launches = ctx.launch_count() - n0
+    assert launches <= 4 <= launches_step, (launches, launches_step)      # init, split expansion, fp16 copy, the ONE loop kernel
+    pg, fg, og = ctx.get_population_host()
+    assert res.generations_run == gens and ctx.generation() == gens
+    assert np.array_equal(pg.view(np.uint32), ps.view(np.uint32))
+    assert np.array_equal(fg.view(np.uint32), fs.view(np.uint32)) and np.array_equal(og, os_)
+    assert res.best_index == og[0] and res.best_error == fg[og[0]]
+    # continuing in two more calls (resume across kernels, buffer parity) stays on the same trajectory
+    for extra in (3, 2):
+        for _ in range(extra):
+            step.evolve(1, w.seed, gp)
+        ctx.evolve(extra, w.seed, gp)
+    ps, fs, os_ = step.get_population_host()
+    pg, fg, og = ctx.get_population_host()
+    assert np.array_equal(pg.view(np.uint32), ps.view(np.uint32)) and np.array_equal(fg.view(np.uint32), fs.view(np.uint32))
+    # and a stand-alone fitness call reproduces the loop's fitness bits
+    f2 = ctx.fitness(dev(pg)).cpu().numpy()
+    assert np.array_equal(f2.view(np.uint32), fg.view(np.uint32))
+
+
+def test_persistent_loop_stop_criterion(orc):
+    w = wl.config(1)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    ref = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    ref.set_tuning(g.GAME_TUNE_PERSISTENT, 0)
+    hist = [ref.evolve(0, w.seed, g.ga_params(P=w.P)).best_error]
+    for _ in range(60):
+        hist.append(ref.evolve(1, w.seed, g.ga_params(P=w.P)).best_error)
+    target = float(hist[33])
+    first = next(i for i, h in enumerate(hist) if h <= target)
+    ctx = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    r = ctx.evolve(60, w.seed, g.ga_params(P=w.P, stop_error=target))
+    assert r.stopped_on_error == 1 and r.generations_run == first and ctx.generation() == first and r.best_error <= target
+    ref2 = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    ref2.set_tuning(g.GAME_TUNE_PERSISTENT, 0)
+    r2 = ref2.evolve(60, w.seed, g.ga_params(P=w.P, stop_error=target))
+    assert (r2.generations_run, r2.best_error, r2.best_index) == (r.generations_run, r.best_error, r.best_index)
+    pa, fa, oa = ctx.get_population_host()
+    pb, fb, ob = ref2.get_population_host()
+    assert np.array_equal(pa.view(np.uint32), pb.view(np.uint32)) and np.array_equal(fa.view(np.uint32), fb.view(np.uint32))
+    assert np.array_equal(oa, ob)
