@@ -46,15 +46,16 @@ def read_peaks():
 
 def ncu_traffic(w, path_name):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-    `ncu --set full` capture summarised in profiles/r01_traffic.csv (null when that config was not captured)."""
-    p = os.path.join(ROOT, "profiles", "r01_traffic.csv")
-    if not os.path.exists(p):
-        return None
+    `ncu --set full` capture summarised in profiles/r02_traffic.csv / r01_traffic.csv (null when that config was not captured)."""
     key = "%s/%s" % (w.name, path_name)
-    for line in open(p).read().splitlines()[1:]:
-        f = line.split(",")
-        if f[0] == key:
-            return float(f[1])
+    for name in ("r02_traffic.csv", "r01_traffic.csv"):          # the latest round's capture first
+        p = os.path.join(ROOT, "profiles", name)
+        if not os.path.exists(p):
+            continue
+        for line in open(p).read().splitlines()[1:]:
+            f = line.split(",")
+            if f[0] == key:
+                return float(f[1])
     return None
 
 
@@ -288,6 +289,11 @@ def run_ours(args, w):
         ctx.set_error(wr.err, wr.R)
         if args.path != "auto":
             ctx.set_path({"fp32": g.GAME_PATH_FP32, "tensor": g.GAME_PATH_TENSOR, "split": g.GAME_PATH_TENSOR_SPLIT}[args.path])
+        if args.expansion != "auto":
+            ctx.set_expansion({"materialized": g.GAME_EXPAND_MATERIALIZED, "regenerated": g.GAME_EXPAND_REGENERATED}[args.expansion])
+        for kv in args.tune:                                    # launch-configuration knobs (game_set_tuning), e.g. persistent=0
+            name, val = kv.split("=")
+            ctx.set_tuning(getattr(g, "GAME_TUNE_" + name.upper()), int(val))
         Xp, tp = torch.from_numpy(X[lo:hi]).pin_memory(), torch.from_numpy(t[lo:hi]).pin_memory()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
@@ -450,7 +456,7 @@ def run_ours(args, w):
            "dtype": {g.GAME_PATH_TENSOR: "f16 operands, f32 accumulate", g.GAME_PATH_TENSOR_SPLIT: "split f16 (hi+lo) operands, f32 accumulate",
                      g.GAME_PATH_FP32: "f32"}[path],
            "data": "synthetic", "config": dict(workload_dict(w, path_name), **({"parallelism": "patterns sharded over %d ranks, all-reduce of P doubles per generation" % world} if args.shard else {})), "clocks": clocks, "e2e": e2e,
-           "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
+           "gpu_launches": int(launches), "tuning": args.tune, "expansion": args.expansion, "roofline": roof, "cpu_baseline": cpu,
            "best_error": float(res.best_error), "load_ms": load_ms}
     print(json.dumps(out))
 
@@ -463,6 +469,9 @@ def main():
     ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number (1-5); 5 = the largest, the one the north star's target is quoted on")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--path", default="auto", choices=["auto", "fp32", "tensor", "split"])
+    ap.add_argument("--expansion", default="auto", choices=["auto", "materialized", "regenerated"])
+    ap.add_argument("--tune", action="append", default=[], metavar="KNOB=VALUE",
+                    help="game_set_tuning knob, e.g. persistent=0, rational_share=0, cta_group=2 (measurement aid; repeatable)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--peaks", action="store_true", help="run the FFMA / special-function micro-benchmarks behind the alu rooflines and exit")
     ap.add_argument("--shard", action="store_true", help="N>1: split the patterns of ONE problem over the ranks (all-reduce of P doubles per generation) instead of running replicas")

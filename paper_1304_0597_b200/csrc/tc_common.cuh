@@ -207,7 +207,7 @@ __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.
 // Arithmetic is issued two evaluations at a time with the packed fp32 instructions of sm_100
 // (FMUL2 / FFMA2), which halves the FMA-pipe issue slots the epilogue needs.
 constexpr int MODE_SIG_EXACT = 0, MODE_IDENTITY = 1, MODE_SIG_TANH32 = 2;
-constexpr int RATIONAL_SHARE_AUTO = 0;      // of 16 evaluation pairs; set from the measurement in DESIGN.md section 7
+constexpr int RATIONAL_SHARE_AUTO = 3;      // of 16 evaluation pairs: the measured best on config 3
 
 __device__ __forceinline__ float tanh_approx(float x) { float y; asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
