@@ -78,7 +78,7 @@ __global__ void expand_kernel(const float *__restrict__ X, long long N, int F, i
             if (PATTERN_MAJOR) {
                 // TENSOR path: permuted term order (tc_position), tile-blocked [n/256][k/64][256][64] so that every
                 // TMA box is one contiguous 32 KB run
-                const long long k = tc_position(family, d, i, m);
+                const long long k = tc_position(family, d, F, i, m);
                 auto at = [&](long long kk) -> OutT & { return E[(((n >> 8) * (ld >> 6) + (kk >> 6)) << 14) + ((n & 255) << 6) + (kk & 63)]; };
                 if (!split) {
                     at(k) = (OutT)f;

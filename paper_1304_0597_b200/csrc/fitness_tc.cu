@@ -31,9 +31,10 @@ constexpr int WARP_TMA = 0, WARP_MMA = 1, WARP_EPI0 = 2;      // warp roles; the
 //   SRC_RES  the resident population tile of SRC_GEN, with the B halves streamed from E16 by TMA into the same ring
 //            (isolates what residency alone buys: a third of the L2 -> SM traffic of SRC_TMA at P = 256)
 constexpr int SRC_TMA = 0, SRC_GEN = 1, SRC_RES = 2;
-constexpr int GEN_WARPS = 4;            // generator threads: GEN_SPLIT per pattern row of this CTA's 128-row B half
-constexpr int GEN_SPLIT = GEN_WARPS / 4; // threads sharing a row: each takes 8 / GEN_SPLIT of a chunk's features
-constexpr int GEN_NJ = 4 / GEN_SPLIT;   // feature PAIRS (float2) per thread and chunk
+constexpr int GEN_WARPS = 8;            // generator threads: (pattern row of this CTA's 128-row B half, group set)
+constexpr int GEN_SETS = GEN_WARPS / 4;  // thread sets per row: set s owns feature groups s, s + GEN_SETS, ...
+constexpr int GEN_NQ = 2;               // feature groups (of 8) per thread at most: F <= 8 * GEN_SETS * GEN_NQ = 32
+constexpr int GEN_EW = 4;               // epilogue warps of the generator variant (the epilogue is far from binding there)
 constexpr int GEN_STAGES = 4;           // B k-block stages of the generator ring
 constexpr int GEN_B_BYTES = 128 * BKB * 2;
 constexpr int GEN_BAR0 = 2;             // named barriers 2.. : one per generator stage (0 = CTA, 1 = epilogue)
@@ -50,16 +51,18 @@ template <int CG> struct Cfg {
 
 
 // ---- a1 inside the kernel: the generator warps of the SRC_GEN variant ---------------------------------------
-// Each of the 128 generator threads owns one pattern row of this CTA's half of the 256-pattern tile and writes that
-// row's expansion, 16 bytes (8 fp16 = one swizzle chunk) at a time, into the B ring exactly where a 128B-swizzled TMA
-// box would have put it: chunk j of row r of a k-block lives at r*128 + ((j ^ (r & 7)) << 4).  The term order is
-// game_internal.cuh's tc_position(): features in groups of 8, one chunk per term type, the chunk's 8 lanes being the
-// group's features -- so one chunk is one step of a recurrence carried in registers for 8 features at once:
+// 256 generator threads per CTA: thread (row, set) owns one pattern row of this CTA's half of the 256-pattern tile and up
+// to GEN_NQ of the row's feature groups (groups set, set + GEN_SETS).  It writes its groups' chunks, 16 bytes (8 fp16 = one
+// swizzle chunk) at a time, into the B ring exactly where a 128B-swizzled TMA box would have put them: chunk j of row r of
+// a k-block lives at r*128 + ((j ^ (r & 7)) << 4).  With the term-type-major order of game_internal.cuh's tc_position()
+// chunk c = tau * G + group, so a thread's chunks come in ascending k-block order as it steps its recurrences, eight
+// features (four packed pairs) per group and step:
 //   Chebyshev (G7, G9):  T_0 = 1, T_1 = x, T_{m+1} = 2x T_m - T_{m-1}
 //   trigonometric (eq. 8-9):  1, cos x, sin x, then cos / sin (m+1)x = 2 cos x . cos / sin mx - cos / sin (m-1)x
-// in fp32 (packed FFMA2), rounded once to fp16.  Rows beyond N generate zeros (their start value is 0), matching the
-// zero padding of the materialised E16.  A stage is published to the MMA warp of the leader CTA by the async-proxy
-// fence + one mbarrier arrival per warp.
+// in fp32 (packed FFMA2; the recurrences' error grows like m^2 eps / 2: 3e-5 at m = 32, far below fp16's 2^-11), rounded
+// once to fp16.  Rows beyond N generate zeros (their start value is 0), matching the zero padding of the materialised E16.
+// A stage is published by the async-proxy fence + a (non-blocking) arrival on the stage's named barrier; the otherwise
+// idle TMA warp completes that barrier and performs the one mbarrier arrival per CTA and stage.
 __device__ __forceinline__ uint32_t pack_half2(float lo, float hi)
 {
     __half2 h = __floats2half2_rn(lo, hi);
@@ -71,142 +74,138 @@ __device__ __forceinline__ void generate_expansion(const float *__restrict__ X, 
                                                    int pair, int n_pairs, int total_tiles, int cta_rank, int gt,
                                                    uint8_t *bring, uint32_t bar0)
 {
-    const int hf = gt >> 7;                   // which part of every chunk this thread writes (warp-uniform)
-    gt &= 127;
+    const int set = gt >> 7, row = gt & 127;           // set is warp-uniform
     const int T = tc_terms_per_feature(FAMILY, d);
-    const int ngroups = (F + 7) >> 3;
+    const int G = (F + 7) >> 3;
     const int nchunks = k_blocks * 8;
-    uint8_t *my_row = bring + gt * 128 + hf * (16 / GEN_SPLIT);
-    const int sw = gt & 7;
+    const int nq = G > set ? (G - set + GEN_SETS - 1) / GEN_SETS : 0;      // groups this thread owns: 0 .. GEN_NQ
+    uint8_t *my_row = bring + row * 128;
+    const int sw16 = (row & 7) << 4;
     const bool vec = (F & 3) == 0;
-    int s = 0; uint32_t ph = 0;
-    int cidx = 0;
-    mbar_wait<true>(bar0 + 8u * MAX_STAGES, 1);     // stage 0 starts free
+    int s = 0; uint32_t ph = 0;                        // ring slot being written and its phase
+    int cur_kb = 0;                                    // which k-block of the tile that slot holds
+    uint8_t *dst = my_row;
+    mbar_wait<true>(bar0 + 8u * MAX_STAGES, 1);        // stage 0 starts free
 
-    uint8_t *dst = my_row;                                          // this thread's row in the current stage
-    const int sw16 = sw << 4;
-    int cb16 = 0;                                                   // 16 * (chunk index inside the k-block)
-    auto put = [&](const float2 (&v)[GEN_NJ]) {                   // this thread's part of the row's next 16-byte chunk
-        if (GEN_NJ == 4) {
-            *reinterpret_cast<uint4 *>(dst + (cb16 ^ sw16)) = make_uint4(pack_half2(v[0].x, v[0].y), pack_half2(v[1].x, v[1].y),
-                                                                          pack_half2(v[GEN_NJ / 2].x, v[GEN_NJ / 2].y), pack_half2(v[GEN_NJ - 1].x, v[GEN_NJ - 1].y));
-        } else {
-            *reinterpret_cast<uint2 *>(dst + (cb16 ^ sw16)) = make_uint2(pack_half2(v[0].x, v[0].y), pack_half2(v[GEN_NJ - 1].x, v[GEN_NJ - 1].y));
-        }
-        ++cidx;
-        cb16 += 16;
-        if (cb16 == 128) {
-            cb16 = 0;
-            fence_proxy_async();              // generic-proxy stores -> visible to the tensor core's async proxy
-            __threadfence_block();
-            asm volatile("bar.arrive %0, %1;" ::"r"(GEN_BAR0 + s), "n"(32 * GEN_WARPS + 32) : "memory");
-            if (++s == GEN_STAGES) { s = 0; ph ^= 1; }
-            dst = my_row + s * GEN_B_BYTES;
-            mbar_wait<true>(bar0 + 8u * (MAX_STAGES + s), ph ^ 1);      // the MMAs that read the next stage have retired
-        }
+    auto next_stage = [&]() {                          // publish the stage being written, move on to the next k-block
+        fence_proxy_async();                           // generic-proxy stores -> visible to the tensor core's async proxy
+        __threadfence_block();
+        asm volatile("bar.arrive %0, %1;" ::"r"(GEN_BAR0 + s), "n"(32 * GEN_WARPS + 32) : "memory");
+        if (++s == GEN_STAGES) { s = 0; ph ^= 1; }
+        dst = my_row + s * GEN_B_BYTES;
+        mbar_wait<true>(bar0 + 8u * (MAX_STAGES + s), ph ^ 1);      // the MMAs that read this slot last have retired
+        ++cur_kb;
     };
-    constexpr int NX = 2 * GEN_NJ;                                  // features per thread and group
-    auto load_x = [&](int tile, int g, float (&x)[NX]) {          // this thread's features of its pattern (0 outside)
-        const long long n = (long long)tile * BN + cta_rank * 128 + gt;
-        const int i0 = g * 8 + hf * NX;
+    auto put = [&](int c, const float2 (&v)[4]) {      // chunk c of this thread's row
+        const int kb = c >> 3;
+        while (cur_kb < kb) next_stage();
+        *reinterpret_cast<uint4 *>(dst + (((c & 7) << 4) ^ sw16)) =
+            make_uint4(pack_half2(v[0].x, v[0].y), pack_half2(v[1].x, v[1].y), pack_half2(v[2].x, v[2].y), pack_half2(v[3].x, v[3].y));
+    };
+    auto load_x = [&](int tile, float (&x)[GEN_NQ][8]) {        // this thread's features of its pattern (0 outside)
+        const long long n = (long long)tile * BN + cta_rank * 128 + row;
 #pragma unroll
-        for (int j = 0; j < NX; ++j) x[j] = 0.f;
-        if (tile >= total_tiles || n >= N) return;
-        const float *xr = X + n * F + i0;
-        if (vec) {
+        for (int q = 0; q < GEN_NQ; ++q) {
 #pragma unroll
-            for (int q = 0; q < NX / 4; ++q)
-                if (i0 + 4 * q < F) {
-                    const float4 v = __ldg(reinterpret_cast<const float4 *>(xr) + q);
-                    x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
-                }
-        } else {
+            for (int j = 0; j < 8; ++j) x[q][j] = 0.f;
+            if (q >= nq || tile >= total_tiles || n >= N) continue;
+            const int i0 = (set + q * GEN_SETS) * 8;
+            const float *xr = X + n * F + i0;
+            if (vec) {
 #pragma unroll
-            for (int j = 0; j < NX; ++j) if (i0 + j < F) x[j] = __ldg(xr + j);
+                for (int h = 0; h < 2; ++h)
+                    if (i0 + 4 * h < F) {
+                        const float4 v = __ldg(reinterpret_cast<const float4 *>(xr) + h);
+                        x[q][4 * h] = v.x; x[q][4 * h + 1] = v.y; x[q][4 * h + 2] = v.z; x[q][4 * h + 3] = v.w;
+                    }
+            } else {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) if (i0 + j < F) x[q][j] = __ldg(xr + j);
+            }
         }
     };
 
-    float xn[NX];
-    load_x(pair, 0, xn);
+    float xn[GEN_NQ][8];
+    load_x(pair, xn);
     for (int tile = pair; tile < total_tiles; tile += n_pairs) {
-        const long long n = (long long)tile * BN + cta_rank * 128 + gt;
+        const long long n = (long long)tile * BN + cta_rank * 128 + row;
         const float one = n < N ? 1.f : 0.f;
         const float2 one2 = make_float2(one, one);
-        cidx = 0;
-        for (int g = 0; g < ngroups; ++g) {
-            float2 x[GEN_NJ];
+        float2 x[GEN_NQ][4];
 #pragma unroll
-            for (int j = 0; j < GEN_NJ; ++j) x[j] = make_float2(xn[2 * j], xn[2 * j + 1]);
-            // fetch the next group's features (the next tile's first group at the end) while this one is generated
-            if (g + 1 < ngroups) load_x(tile, g + 1, xn); else load_x(tile + n_pairs, 0, xn);
-            float2 ones[GEN_NJ];
+        for (int q = 0; q < GEN_NQ; ++q)
 #pragma unroll
-            for (int j = 0; j < GEN_NJ; ++j) ones[j] = one2;
-            put(ones);                              // tau = 0: the constant term
-            if (FAMILY == GAME_CHEB) {
-                float2 tm1[GEN_NJ], t0[GEN_NJ], x2[GEN_NJ];
+            for (int j = 0; j < 4; ++j) x[q][j] = make_float2(xn[q][2 * j], xn[q][2 * j + 1]);
+        load_x(tile + n_pairs, xn);                    // the next tile's features travel while this one is generated
+        const int c0 = set;                            // chunk of (tau, q): tau * G + set + q * GEN_SETS
+        float2 ones[4] = {one2, one2, one2, one2};
 #pragma unroll
-                for (int j = 0; j < GEN_NJ; ++j) { tm1[j] = one2; t0[j] = __fmul2_rn(x[j], one2); x2[j] = __fadd2_rn(x[j], x[j]); }
-                put(t0);                      // T_1 (degree >= 1 always)
-                // two steps per iteration, the two state registers trading places: no register moves
-                int m = 2;
-                for (; m + 1 <= d; m += 2) {
+        for (int q = 0; q < GEN_NQ; ++q) if (q < nq) put(c0 + q * GEN_SETS, ones);                 // tau = 0: the constant term
+        if (FAMILY == GAME_CHEB) {
+            float2 tm1[GEN_NQ][4], t0[GEN_NQ][4], x2[GEN_NQ][4];
 #pragma unroll
-                    for (int j = 0; j < GEN_NJ; ++j) tm1[j] = __ffma2_rn(x2[j], t0[j], make_float2(-tm1[j].x, -tm1[j].y));
-                    put(tm1);
+            for (int q = 0; q < GEN_NQ; ++q) {
 #pragma unroll
-                    for (int j = 0; j < GEN_NJ; ++j) t0[j] = __ffma2_rn(x2[j], tm1[j], make_float2(-t0[j].x, -t0[j].y));
-                    put(t0);
+                for (int j = 0; j < 4; ++j) { tm1[q][j] = one2; t0[q][j] = __fmul2_rn(x[q][j], one2); x2[q][j] = __fadd2_rn(x[q][j], x[q][j]); }
+                if (q < nq) put(G + c0 + q * GEN_SETS, t0[q]);                                    // T_1 (degree >= 1 always)
+            }
+            for (int m = 2; m <= d; ++m) {
+#pragma unroll
+                for (int q = 0; q < GEN_NQ; ++q) {
+                    if (q >= nq) continue;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const float2 t1 = __ffma2_rn(x2[q][j], t0[q][j], make_float2(-tm1[q][j].x, -tm1[q][j].y));
+                        tm1[q][j] = t0[q][j]; t0[q][j] = t1;
+                    }
+                    put(m * G + c0 + q * GEN_SETS, t0[q]);
                 }
-                if (m <= d) {
+            }
+        } else {
+            float2 C2[GEN_NQ][4], c[GEN_NQ][4], cm[GEN_NQ][4], sn[GEN_NQ][4], sm[GEN_NQ][4];
 #pragma unroll
-                    for (int j = 0; j < GEN_NJ; ++j) tm1[j] = __ffma2_rn(x2[j], t0[j], make_float2(-tm1[j].x, -tm1[j].y));
-                    put(tm1);
+            for (int q = 0; q < GEN_NQ; ++q) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    float2 Cv, Sv;
+                    __sincosf(x[q][j].x, &Sv.x, &Cv.x);                // |x| <= pi is checked at load for this variant
+                    __sincosf(x[q][j].y, &Sv.y, &Cv.y);
+                    C2[q][j] = __fadd2_rn(Cv, Cv);
+                    cm[q][j] = one2; c[q][j] = __fmul2_rn(Cv, one2);
+                    sm[q][j] = make_float2(0.f, 0.f); sn[q][j] = __fmul2_rn(Sv, one2);
                 }
-            } else {
-                // cos (m+1)x = 2 cos x cos mx - cos (m-1)x, and the same for sin: one FFMA per value.  In fp32 the
-                // recurrence's error grows like m^2 eps / 2 at worst (x -> 0): 3e-5 at m = 32, far below fp16's 2^-11.
-                float2 C2[GEN_NJ], c[GEN_NJ], cm[GEN_NJ], sn[GEN_NJ], sm[GEN_NJ];
+            }
 #pragma unroll
-                for (int j = 0; j < GEN_NJ; ++j) {
-                    float2 C, S;
-                    __sincosf(x[j].x, &S.x, &C.x);                    // |x| <= pi is checked at load for this variant
-                    __sincosf(x[j].y, &S.y, &C.y);
-                    C2[j] = __fadd2_rn(C, C);
-                    cm[j] = one2; c[j] = __fmul2_rn(C, one2);
-                    sm[j] = make_float2(0.f, 0.f); sn[j] = __fmul2_rn(S, one2);
+            for (int q = 0; q < GEN_NQ; ++q) if (q < nq) put(G + c0 + q * GEN_SETS, c[q]);          // cos x
+#pragma unroll
+            for (int q = 0; q < GEN_NQ; ++q) if (q < nq) put(2 * G + c0 + q * GEN_SETS, sn[q]);     // sin x
+            for (int m = 2; m <= d; ++m) {
+#pragma unroll
+                for (int q = 0; q < GEN_NQ; ++q) {
+                    if (q >= nq) continue;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const float2 c1 = __ffma2_rn(C2[q][j], c[q][j], make_float2(-cm[q][j].x, -cm[q][j].y));
+                        cm[q][j] = c[q][j]; c[q][j] = c1;
+                    }
+                    put((2 * m - 1) * G + c0 + q * GEN_SETS, c[q]);
                 }
-                put(c);                          // cos x
-                put(sn);                      // sin x
-                int m = 2;
-                for (; m + 1 <= d; m += 2) {
 #pragma unroll
-                    for (int j = 0; j < GEN_NJ; ++j) cm[j] = __ffma2_rn(C2[j], c[j], make_float2(-cm[j].x, -cm[j].y));
-                    put(cm);
+                for (int q = 0; q < GEN_NQ; ++q) {
+                    if (q >= nq) continue;
 #pragma unroll
-                    for (int j = 0; j < GEN_NJ; ++j) sm[j] = __ffma2_rn(C2[j], sn[j], make_float2(-sm[j].x, -sm[j].y));
-                    put(sm);
-#pragma unroll
-                    for (int j = 0; j < GEN_NJ; ++j) c[j] = __ffma2_rn(C2[j], cm[j], make_float2(-c[j].x, -c[j].y));
-                    put(c);
-#pragma unroll
-                    for (int j = 0; j < GEN_NJ; ++j) sn[j] = __ffma2_rn(C2[j], sm[j], make_float2(-sn[j].x, -sn[j].y));
-                    put(sn);
-                }
-                if (m <= d) {
-#pragma unroll
-                    for (int j = 0; j < GEN_NJ; ++j) cm[j] = __ffma2_rn(C2[j], c[j], make_float2(-cm[j].x, -cm[j].y));
-                    put(cm);
-#pragma unroll
-                    for (int j = 0; j < GEN_NJ; ++j) sm[j] = __ffma2_rn(C2[j], sn[j], make_float2(-sm[j].x, -sm[j].y));
-                    put(sm);
+                    for (int j = 0; j < 4; ++j) {
+                        const float2 s1 = __ffma2_rn(C2[q][j], sn[q][j], make_float2(-sm[q][j].x, -sm[q][j].y));
+                        sm[q][j] = sn[q][j]; sn[q][j] = s1;
+                    }
+                    put(2 * m * G + c0 + q * GEN_SETS, sn[q]);
                 }
             }
         }
-        float2 zeros[GEN_NJ];
-#pragma unroll
-        for (int j = 0; j < GEN_NJ; ++j) zeros[j] = make_float2(0.f, 0.f);
-        while (cidx < nchunks) put(zeros);                   // K padded up to whole k-blocks
+        float2 zeros[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+        for (int c = T * G + set; c < nchunks; c += GEN_SETS) put(c, zeros);          // K padded up to whole k-blocks
+        while (cur_kb < k_blocks) next_stage();            // publish what is left of the tile; on to the next tile's first stage
+        cur_kb = 0;
     }
 }
 
@@ -377,7 +376,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             // Targets are staged per team through two buffers (the team's one barrier per tile separates writer and
             // readers); the next tile's target is fetched a tile ahead.  Patterns beyond N carry the target that makes their
             // residual exactly zero (their expansion rows are zero, so z = 0): no masked code path.
-            static_assert(EW == 8, "two teams of four warps");
+            static_assert(!TEAMS || EW == 8, "two teams of four warps");
             constexpr int NCH = BNT / 32;               // 32-column chunks per tile: 8 (4 for half-size tiles)
             const int ew = warp - WARP_EPI0;
             const int team = ew >> 2;
@@ -457,9 +456,11 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             constexpr float tneutral = ACT == MODE_SIG_EXACT ? 0.5f : 0.f;         // staged target of a padding pattern
             // raw target of this thread's pattern in `tile` (tneutral + tbias for a padding pattern); the bias comes
             // off when the value is staged one tile later, so nothing waits on the load where it is issued
-            auto fetch_target = [&](int tile) -> float {
-                const long long n = (long long)(tile / m_blocks) * BN + et;
-                return (et < BN && n < N) ? tgt[n] : tneutral + tbias;
+            constexpr int TPT = BN / (32 * EW) > 0 ? BN / (32 * EW) : 1;            // targets each epilogue thread stages per tile
+            auto fetch_target = [&](int tile, int u) -> float {
+                const int col = et + u * 32 * EW;
+                const long long n = (long long)(tile / m_blocks) * BN + col;
+                return (col < BN && n < N) ? tgt[n] : tneutral + tbias;
             };
             auto epi_barrier = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(32 * EW) : "memory"); };
             const int row = quarter * 32 + lane;        // chromosome row inside the 128-row block
@@ -476,10 +477,15 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(cb * CBW);
             int acc = 0; uint32_t aph = 0; int tb = 0, sb = 0;
             uint32_t va[32], vb[32];
-            float t_next = 0.f;
+            float t_next[TPT];
+#pragma unroll
+            for (int u = 0; u < TPT; ++u) t_next[u] = 0.f;
             if (pair < total_tiles) {
-                if (et < BN) tgt_s[et] = fetch_target(pair) - tbias;
-                if (pair + n_pairs < total_tiles) t_next = fetch_target(pair + n_pairs);
+#pragma unroll
+                for (int u = 0; u < TPT; ++u) {
+                    if (et + u * 32 * EW < BN) tgt_s[et + u * 32 * EW] = fetch_target(pair, u) - tbias;
+                    if (pair + n_pairs < total_tiles) t_next[u] = fetch_target(pair + n_pairs, u);
+                }
                 epi_barrier();
                 mbar_wait<SUSP>(tfull_bar(0), 0);
                 tc_fence_after();
@@ -508,8 +514,11 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                             if (CG == 1) mbar_arrive(tempty_bar(acc));
                             else mbar_arrive_cluster(tempty_bar(acc), 0);
                         }
-                        if (has_next && et < BN) tgt_s[tbn * BN + et] = t_next - tbias;
-                        if (tile + 2 * n_pairs < total_tiles) t_next = fetch_target(tile + 2 * n_pairs);
+#pragma unroll
+                        for (int u = 0; u < TPT; ++u) {
+                            if (has_next && et + u * 32 * EW < BN) tgt_s[tbn * BN + et + u * 32 * EW] = t_next[u] - tbias;
+                            if (tile + 2 * n_pairs < total_tiles) t_next[u] = fetch_target(tile + 2 * n_pairs, u);
+                        }
                         epi_barrier();
                         flush(sb ^ 1);
                         if (has_next) {                   // uniform over the CTA's epilogue warps
@@ -609,7 +618,7 @@ C16Sink tensor_sink(const game_ctx *ctx, bool split)
     const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : (split ? MODE_SIG_EXACT : sigmoid_mode(ctx));
     C16Sink s;
     s.ptr = split ? ctx->C16s : ctx->C16;
-    s.Kpad = ctx->Kpad; s.family = ctx->family; s.d = ctx->degree; s.split = split ? 1 : 0;
+    s.Kpad = ctx->Kpad; s.family = ctx->family; s.d = ctx->degree; s.F = ctx->F; s.split = split ? 1 : 0;
     s.scale = mode == MODE_SIG_TANH32 ? 0.5f : 1.0f;
     return s;
 }
@@ -694,7 +703,7 @@ int tensor_expansion(const game_ctx *ctx, int P)
 {
     const int Ppad = ((P + 255) / 256) * 256;
     const int k_blocks = ctx->Kpad / BKB;
-    const bool can = tc_permuted(ctx->family) && Ppad == 256 && ctx->X != nullptr &&
+    const bool can = tc_permuted(ctx->family) && Ppad == 256 && ctx->X != nullptr && ctx->F <= 8 * GEN_SETS * GEN_NQ &&
                      k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES <= 227 * 1024 &&
                      (ctx->family != GAME_TRIG || ctx->x_maxabs <= 3.14159f);
     if (ctx->expand_mode == GAME_EXPAND_REGENERATED) return can ? GAME_EXPAND_REGENERATED : -1;
@@ -774,8 +783,8 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
                : launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG, false>(ctx, n_tiles, m_blocks, Ppad, state, split)
 #define GAME_TC_GEN(M, T)                                                                                  \
     rc = resident_only ? launch_variant<2, M, T, 8, SRC_RES, GAME_TRIG>(ctx, n_tiles, 1, Ppad, state, split) \
-       : ctx->family == GAME_TRIG ? launch_variant<2, M, T, 8, SRC_GEN, GAME_TRIG>(ctx, n_tiles, 1, Ppad, state) \
-                                  : launch_variant<2, M, T, 8, SRC_GEN, GAME_CHEB>(ctx, n_tiles, 1, Ppad, state)
+       : ctx->family == GAME_TRIG ? launch_variant<2, M, T, GEN_EW, SRC_GEN, GAME_TRIG>(ctx, n_tiles, 1, Ppad, state) \
+                                  : launch_variant<2, M, T, GEN_EW, SRC_GEN, GAME_CHEB>(ctx, n_tiles, 1, Ppad, state)
 #define GAME_TC_MODE(CGV, M)                                                                               \
     if (src != SRC_TMA) { if (tmse) { GAME_TC_GEN(M, true); } else { GAME_TC_GEN(M, false); } }            \
     else if (tmse) { GAME_TC_EW(CGV, M, true); } else { GAME_TC_EW(CGV, M, false); }

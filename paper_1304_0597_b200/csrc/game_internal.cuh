@@ -42,25 +42,27 @@ __device__ __forceinline__ unsigned int sort_key(float f)
 
 // ---- term order of the TENSOR path's operands ---------------------------------------------------------------
 // A contraction does not care in which order its terms are stored as long as both operands agree, so E16 and C16
-// use an order that an in-kernel generator can stream: features in groups of 8, and inside a group one 8-wide
-// chunk (16 bytes of fp16 = one swizzle chunk) per term type, the 8 lanes of the chunk being the group's features:
-//     position = ((i / 8) * T + tau) * 8 + (i % 8),      T = terms per feature (2d+1 or d+1)
-// tau: Chebyshev T_0..T_d in order; trigonometric 1, cos x, sin x, cos 2x, sin 2x, ... so that (cos, sin) of one
-// multiple sit in adjacent chunks and one packed recurrence step yields both.  Features are padded to a multiple
-// of 8 (zero genes).  The tied families keep their natural order.  The ABI's order (L105) is untouched: only the
-// fp16 copies are permuted, by pop_to_f16_kernel and the expansion kernels.
+// use an order that an in-kernel generator can stream: features in groups of 8, one 8-wide chunk (16 bytes of fp16 =
+// one swizzle chunk) per (term type, group), the 8 lanes of the chunk being the group's features, TERM TYPE MAJOR:
+//     position = (tau * G + i / 8) * 8 + (i % 8),      G = ceil(F / 8) groups, tau = 0 .. T-1 (T = 2d+1 or d+1)
+// tau: Chebyshev T_0..T_d in order; trigonometric 1, cos x, sin x, cos 2x, sin 2x, ...  A k-block (8 chunks) is thus a
+// fixed run of consecutive term types for ALL groups, so generator threads that each own (pattern row, group) advance
+// their recurrences in step, one chunk per term type, with no per-chunk bookkeeping (round 1's group-major order had
+// 17 chunks per group straddling k-blocks: ~37 instructions per chunk in one in-order warp).  Features are padded to
+// a multiple of 8 (zero genes).  The tied families keep their natural order.  The ABI's order (L105) is untouched:
+// only the fp16 copies are permuted, by pop_to_f16_kernel / ga_step_kernel and the expansion kernels.
 __host__ __device__ inline bool tc_permuted(int family) { return family == GAME_TRIG || family == GAME_CHEB; }
 __host__ __device__ inline int tc_terms_per_feature(int family, int d) { return family == GAME_TRIG ? 2 * d + 1 : d + 1; }
 __host__ __device__ inline int tc_num_positions(int family, int d, int F, int K)
 {
     return tc_permuted(family) ? ((F + 7) / 8) * 8 * tc_terms_per_feature(family, d) : K;
 }
-// m = index inside the feature's block in the ABI's order [a_0, a_1..a_d, b_1..b_d]
-__host__ __device__ inline int tc_position(int family, int d, int i, int m)
+// m = index inside the feature's block in the ABI's order [a_0, a_1..a_d, b_1..b_d]; F = number of features
+__host__ __device__ inline int tc_position(int family, int d, int F, int i, int m)
 {
-    const int T = tc_terms_per_feature(family, d);
+    const int G = (F + 7) >> 3;
     const int tau = family == GAME_TRIG ? (m == 0 ? 0 : (m <= d ? 2 * m - 1 : 2 * (m - d))) : m;
-    return ((i >> 3) * T + tau) * 8 + (i & 7);
+    return (tau * G + (i >> 3)) * 8 + (i & 7);
 }
 
 // ---- programmatic dependent launch (PDL) -----------------------------------------------------------------------
@@ -75,7 +77,7 @@ __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.lau
 // ga_step_kernel while it builds the next generation (one launch and one pass over the genes less per generation).
 struct C16Sink {
     __half *ptr;         // nullptr: no copy wanted
-    int Kpad, family, d, split;
+    int Kpad, family, d, F, split;
     float scale;         // 1, or 0.5 for the tanh logistic (exact)
 };
 // gene k (ABI order) of chromosome p -> its fp16 position(s): round to nearest even.  A gene outside the finite fp16
@@ -89,7 +91,7 @@ __device__ __forceinline__ void c16_store(const C16Sink &s, int p, int k, float 
     int pos = k;
     if (tc_permuted(s.family)) {              // ABI order k = i*B + m  ->  the tensor path's term order
         const int B = tc_terms_per_feature(s.family, s.d);
-        pos = tc_position(s.family, s.d, k / B, k % B);
+        pos = tc_position(s.family, s.d, s.F, k / B, k % B);
     }
     if (!s.split) {
         s.ptr[(long long)p * s.Kpad + pos] = __float2half_rn(v);
