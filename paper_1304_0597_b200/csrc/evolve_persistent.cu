@@ -56,7 +56,7 @@ __device__ __forceinline__ void grid_barrier(unsigned int *ctr, unsigned int &ta
         for (uint32_t spin = 1;; ++spin) {
             asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
             if ((int)(v - target) >= 0) break;
-            if ((spin & 0xFFFFu) == 0) mbar_timeout_check(t0);
+            if ((spin & 0xFFFFu) == 0) t0 = mbar_timeout_check(t0);
         }
         asm volatile("fence.acq_rel.gpu;" ::: "memory");
     }

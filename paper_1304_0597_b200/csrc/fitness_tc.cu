@@ -31,15 +31,32 @@ constexpr int WARP_TMA = 0, WARP_MMA = 1, WARP_EPI0 = 2;      // warp roles; the
 //   SRC_RES  the resident population tile of SRC_GEN, with the B halves streamed from E16 by TMA into the same ring
 //            (isolates what residency alone buys: a third of the L2 -> SM traffic of SRC_TMA at P = 256)
 constexpr int SRC_TMA = 0, SRC_GEN = 1, SRC_RES = 2;
-constexpr int GEN_WARPS = 8;            // generator threads: (pattern row of this CTA's 128-row B half, group set)
-constexpr int GEN_SETS = GEN_WARPS / 4;  // thread sets per row: set s owns feature groups s, s + GEN_SETS, ...
-constexpr int GEN_NQ = 2;               // feature groups (of 8) per thread at most: F <= 8 * GEN_SETS * GEN_NQ = 32
+constexpr int GEN_WARPS = 16;           // generator threads: (pattern row of this CTA's 128-row B half, feature group)
+constexpr int GEN_GROUPS = GEN_WARPS / 4; // feature groups (of 8) the generator covers: F <= 32
 constexpr int GEN_EW = 4;               // epilogue warps of the generator variant (the epilogue is far from binding there)
 constexpr int GEN_STAGES = 4;           // B k-block stages of the generator ring
 constexpr int GEN_B_BYTES = 128 * BKB * 2;
+constexpr int GEN_THREADS = 128 + 32 * GEN_EW + 32 * GEN_WARPS;      // warpgroups: {TMA, MMA, relay, idle}, epilogue, 2 x generators
+// setmaxnreg: a 768-thread CTA starts at 80 registers per thread; the first warpgroup and the generators hand some to the epilogue
+constexpr int GEN_REGS_LOW = 56, GEN_REGS_GEN = 72, GEN_REGS_EPI = 128;
+static_assert((GEN_STAGES & (GEN_STAGES - 1)) == 0, "ring slot = k-block count mod GEN_STAGES");
+static_assert(128 * GEN_REGS_LOW + 32 * GEN_WARPS * GEN_REGS_GEN + 32 * GEN_EW * GEN_REGS_EPI <= 80 * GEN_THREADS, "register pool of the CTA");
 constexpr int GEN_BAR0 = 2;             // named barriers 2.. : one per generator stage (0 = CTA, 1 = epilogue)
 constexpr int MAX_STAGES = 6;           // barrier slots are laid out for the deepest ring
 constexpr int TC_TAIL_BYTES = 256 /*barriers*/ + 3 * BN * 4 /*targets: [3][BN], or [team][2][BN]*/ + 2 * 4 * BM * 4 /*column-block error sums of two tiles*/;
+
+#ifdef GAME_TRACE
+// measurement build only (-DGAME_TRACE, never the shipped library): clock64 stamps of the hand-overs of CTA pair 0
+__device__ unsigned long long g_trace[8][8192];
+__device__ unsigned int g_trace_n[8];
+#define TRACE(role) do { if (trace_i < 8192) g_trace[role][trace_i++] = clock64(); } while (0)
+#define TRACE_DONE(role) do { g_trace_n[role] = trace_i; } while (0)
+#define TRACE_DECL unsigned int trace_i = 0
+#else
+#define TRACE(role) do { } while (0)
+#define TRACE_DONE(role) do { } while (0)
+#define TRACE_DECL do { } while (0)
+#endif
 
 template <int CG> struct Cfg {
     static constexpr int BNL = BN / CG;                 // pattern rows this CTA stages
@@ -51,162 +68,149 @@ template <int CG> struct Cfg {
 
 
 // ---- a1 inside the kernel: the generator warps of the SRC_GEN variant ---------------------------------------
-// 256 generator threads per CTA: thread (row, set) owns one pattern row of this CTA's half of the 256-pattern tile and up
-// to GEN_NQ of the row's feature groups (groups set, set + GEN_SETS).  It writes its groups' chunks, 16 bytes (8 fp16 = one
-// swizzle chunk) at a time, into the B ring exactly where a 128B-swizzled TMA box would have put them: chunk j of row r of
-// a k-block lives at r*128 + ((j ^ (r & 7)) << 4).  With the term-type-major order of game_internal.cuh's tc_position()
-// chunk c = tau * G + group, so a thread's chunks come in ascending k-block order as it steps its recurrences, eight
-// features (four packed pairs) per group and step:
-//   Chebyshev (G7, G9):  T_0 = 1, T_1 = x, T_{m+1} = 2x T_m - T_{m-1}
-//   trigonometric (eq. 8-9):  1, cos x, sin x, then cos / sin (m+1)x = 2 cos x . cos / sin mx - cos / sin (m-1)x
+// 512 generator threads per CTA: thread (row, g) owns feature group g (eight features, four packed pairs) of one pattern
+// row of this CTA's half of the 256-pattern tile.  It writes the group's chunks, 16 bytes (8 fp16 = one swizzle chunk) at
+// a time, into the B ring exactly where a 128B-swizzled TMA box would have put them: chunk j of row r of a k-block lives at
+// r*128 + ((j ^ (r & 7)) << 4).  With the term-type-major order of game_internal.cuh's tc_position() chunk c = tau * G + g,
+// so the thread's chunks lie G <= 4 apart: they come in ascending k-block order as it steps its recurrences, every thread
+// owns a chunk of every k-block, and all generator threads move from stage to stage together, one step at a time.
+//   Chebyshev (G7, G9):  T_{-1} = x, T_0 = 1, T_{m+1} = 2x T_m - T_{m-1}
+//   trigonometric (eq. 8-9):  the constant term is cos 0x; cos / sin mx = 2 cos x . cos / sin (m-1)x - cos / sin (m-2)x
+//   started from cos(-x), cos 0x and sin(-x), sin 0x -- no special cases inside the loops
 // in fp32 (packed FFMA2; the recurrences' error grows like m^2 eps / 2: 3e-5 at m = 32, far below fp16's 2^-11), rounded
-// once to fp16.  Rows beyond N generate zeros (their start value is 0), matching the zero padding of the materialised E16.
-// A stage is published by the async-proxy fence + a (non-blocking) arrival on the stage's named barrier; the otherwise
-// idle TMA warp completes that barrier and performs the one mbarrier arrival per CTA and stage.
-__device__ __forceinline__ uint32_t pack_half2(float lo, float hi)
+// once to fp16.  The new value of a recurrence overwrites the older one in place (ping-pong, no register moves).  Rows
+// beyond N generate zeros (their start values are 0), matching the zero padding of the materialised E16.
+// A stage is published by the async-proxy fence + a (non-blocking) arrival on the stage's named barrier; the relay warp
+// completes that barrier and performs the one mbarrier arrival per CTA and stage.
+__device__ __forceinline__ uint32_t pack_half2(float2 v)
 {
-    __half2 h = __floats2half2_rn(lo, hi);
+    __half2 h = __floats2half2_rn(v.x, v.y);
     return *reinterpret_cast<uint32_t *>(&h);
 }
+__device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
 
 template <int FAMILY>
 __device__ __forceinline__ void generate_expansion(const float *__restrict__ X, int F, int d, long long N, int k_blocks,
                                                    int pair, int n_pairs, int total_tiles, int cta_rank, int gt,
-                                                   uint8_t *bring, uint32_t bar0)
+                                                   uint32_t bring, uint32_t bar0)
 {
-    const int set = gt >> 7, row = gt & 127;           // set is warp-uniform
+    const int g = gt >> 7, row = gt & 127;             // g is warp-uniform
+    int G = (F + 7) >> 3;
+    if (g >= G) return;                                // fewer feature groups than generator warpgroups
     const int T = tc_terms_per_feature(FAMILY, d);
-    const int G = (F + 7) >> 3;
+    int bar_count = 128 * G + 32;                      // the active generator warps + the relay warp
     const int nchunks = k_blocks * 8;
-    const int nq = G > set ? (G - set + GEN_SETS - 1) / GEN_SETS : 0;      // groups this thread owns: 0 .. GEN_NQ
-    uint8_t *my_row = bring + row * 128;
-    const int sw16 = (row & 7) << 4;
+    // this row of ring slot 0, with the row's swizzle term folded in: chunk j lives at (row address) ^ (j << 4)
+    uint32_t my_row = (bring + (uint32_t)row * 128u) ^ ((uint32_t)(row & 7) << 4);
+    uint32_t empty0 = bar0 + 8u * MAX_STAGES;
+    // (opaque to the compiler from here on: it would otherwise re-derive them from special registers at every use)
+    asm volatile("" : "+r"(my_row), "+r"(empty0), "+r"(G), "+r"(bar_count));
     const bool vec = (F & 3) == 0;
-    int s = 0; uint32_t ph = 0;                        // ring slot being written and its phase
-    int cur_kb = 0;                                    // which k-block of the tile that slot holds
-    uint8_t *dst = my_row;
-    mbar_wait<true>(bar0 + 8u * MAX_STAGES, 1);        // stage 0 starts free
+    uint32_t it = 0;                                   // k-blocks published so far: ring slot it % 4, phase (it / 4) & 1
+    int c_end = 8;                                     // first chunk of the NEXT k-block of the tile
+    uint32_t dst = my_row;
+    mbar_wait(empty0, 1);                              // stage 0 starts free
+    const bool tr = pair == 0 && gt == 0; (void)tr;
+    TRACE_DECL;
 
-    auto next_stage = [&]() {                          // publish the stage being written, move on to the next k-block
+    auto advance = [&]() {                             // publish the stage being written, move on to the next k-block
+        if (tr) TRACE(cta_rank);
         fence_proxy_async();                           // generic-proxy stores -> visible to the tensor core's async proxy
-        __threadfence_block();
-        asm volatile("bar.arrive %0, %1;" ::"r"(GEN_BAR0 + s), "n"(32 * GEN_WARPS + 32) : "memory");
-        if (++s == GEN_STAGES) { s = 0; ph ^= 1; }
+        asm volatile("bar.arrive %0, %1;" ::"r"(GEN_BAR0 + (it & (GEN_STAGES - 1))), "r"(bar_count) : "memory");
+        ++it;
+        const uint32_t s = it & (GEN_STAGES - 1);
         dst = my_row + s * GEN_B_BYTES;
-        mbar_wait<true>(bar0 + 8u * (MAX_STAGES + s), ph ^ 1);      // the MMAs that read this slot last have retired
-        ++cur_kb;
+        if (tr) TRACE(cta_rank);
+        mbar_wait_lean(empty0 + 8u * s, ((it / GEN_STAGES) & 1u) ^ 1u);     // the MMAs that read this slot last have retired
+        if (tr) TRACE(cta_rank);
     };
     auto put = [&](int c, const float2 (&v)[4]) {      // chunk c of this thread's row
-        const int kb = c >> 3;
-        while (cur_kb < kb) next_stage();
-        *reinterpret_cast<uint4 *>(dst + (((c & 7) << 4) ^ sw16)) =
-            make_uint4(pack_half2(v[0].x, v[0].y), pack_half2(v[1].x, v[1].y), pack_half2(v[2].x, v[2].y), pack_half2(v[3].x, v[3].y));
+        if (c >= c_end) { advance(); c_end += 8; }
+        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};"
+                     ::"r"(dst ^ (((uint32_t)c << 4) & 0x70u)), "r"(pack_half2(v[0])), "r"(pack_half2(v[1])),
+                       "r"(pack_half2(v[2])), "r"(pack_half2(v[3])) : "memory");
     };
-    auto load_x = [&](int tile, float (&x)[GEN_NQ][8]) {        // this thread's features of its pattern (0 outside)
+    auto load_x = [&](int tile, float (&x)[8]) {       // this thread's features of its pattern (0 outside)
         const long long n = (long long)tile * BN + cta_rank * 128 + row;
 #pragma unroll
-        for (int q = 0; q < GEN_NQ; ++q) {
+        for (int j = 0; j < 8; ++j) x[j] = 0.f;
+        if (tile >= total_tiles || n >= N) return;
+        const float *xr = X + n * F + g * 8;
+        if (vec) {
 #pragma unroll
-            for (int j = 0; j < 8; ++j) x[q][j] = 0.f;
-            if (q >= nq || tile >= total_tiles || n >= N) continue;
-            const int i0 = (set + q * GEN_SETS) * 8;
-            const float *xr = X + n * F + i0;
-            if (vec) {
+            for (int h = 0; h < 2; ++h)
+                if (g * 8 + 4 * h < F) {
+                    const float4 v = __ldg(reinterpret_cast<const float4 *>(xr) + h);
+                    x[4 * h] = v.x; x[4 * h + 1] = v.y; x[4 * h + 2] = v.z; x[4 * h + 3] = v.w;
+                }
+        } else {
 #pragma unroll
-                for (int h = 0; h < 2; ++h)
-                    if (i0 + 4 * h < F) {
-                        const float4 v = __ldg(reinterpret_cast<const float4 *>(xr) + h);
-                        x[q][4 * h] = v.x; x[q][4 * h + 1] = v.y; x[q][4 * h + 2] = v.z; x[q][4 * h + 3] = v.w;
-                    }
-            } else {
-#pragma unroll
-                for (int j = 0; j < 8; ++j) if (i0 + j < F) x[q][j] = __ldg(xr + j);
-            }
+            for (int j = 0; j < 8; ++j) if (g * 8 + j < F) x[j] = __ldg(xr + j);
         }
     };
 
-    float xn[GEN_NQ][8];
+    float xn[8];
     load_x(pair, xn);
     for (int tile = pair; tile < total_tiles; tile += n_pairs) {
         const long long n = (long long)tile * BN + cta_rank * 128 + row;
         const float one = n < N ? 1.f : 0.f;
         const float2 one2 = make_float2(one, one);
-        float2 x[GEN_NQ][4];
-#pragma unroll
-        for (int q = 0; q < GEN_NQ; ++q)
-#pragma unroll
-            for (int j = 0; j < 4; ++j) x[q][j] = make_float2(xn[q][2 * j], xn[q][2 * j + 1]);
-        load_x(tile + n_pairs, xn);                    // the next tile's features travel while this one is generated
-        const int c0 = set;                            // chunk of (tau, q): tau * G + set + q * GEN_SETS
-        float2 ones[4] = {one2, one2, one2, one2};
-#pragma unroll
-        for (int q = 0; q < GEN_NQ; ++q) if (q < nq) put(c0 + q * GEN_SETS, ones);                 // tau = 0: the constant term
+        int c = g;                                     // chunk of (tau, g): tau * G + g
         if (FAMILY == GAME_CHEB) {
-            float2 tm1[GEN_NQ][4], t0[GEN_NQ][4], x2[GEN_NQ][4];
+            float2 ta[4], tb[4], x2[4];                // T_tau and T_{tau-1} (alternating), 2x
 #pragma unroll
-            for (int q = 0; q < GEN_NQ; ++q) {
-#pragma unroll
-                for (int j = 0; j < 4; ++j) { tm1[q][j] = one2; t0[q][j] = __fmul2_rn(x[q][j], one2); x2[q][j] = __fadd2_rn(x[q][j], x[q][j]); }
-                if (q < nq) put(G + c0 + q * GEN_SETS, t0[q]);                                    // T_1 (degree >= 1 always)
+            for (int j = 0; j < 4; ++j) {
+                const float2 x = make_float2(xn[2 * j], xn[2 * j + 1]);
+                ta[j] = one2; tb[j] = __fmul2_rn(x, one2); x2[j] = __fadd2_rn(x, x);
             }
-            for (int m = 2; m <= d; ++m) {
+            load_x(tile + n_pairs, xn);                // the next tile's features travel while this one is generated
+            for (int tau = 0; tau <= d; tau += 2) {
+                put(c, ta); c += G;
 #pragma unroll
-                for (int q = 0; q < GEN_NQ; ++q) {
-                    if (q >= nq) continue;
+                for (int j = 0; j < 4; ++j) tb[j] = __ffma2_rn(x2[j], ta[j], neg2(tb[j]));
+                if (tau + 1 <= d) {
+                    put(c, tb); c += G;
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        const float2 t1 = __ffma2_rn(x2[q][j], t0[q][j], make_float2(-tm1[q][j].x, -tm1[q][j].y));
-                        tm1[q][j] = t0[q][j]; t0[q][j] = t1;
-                    }
-                    put(m * G + c0 + q * GEN_SETS, t0[q]);
+                    for (int j = 0; j < 4; ++j) ta[j] = __ffma2_rn(x2[j], tb[j], neg2(ta[j]));
                 }
             }
         } else {
-            float2 C2[GEN_NQ][4], c[GEN_NQ][4], cm[GEN_NQ][4], sn[GEN_NQ][4], sm[GEN_NQ][4];
+            float2 C2[4], ca[4], cb[4], sa[4], sb[4];  // 2 cos x; cos (m-1)x / (m-2)x and sin (m-1)x / (m-2)x (alternating)
 #pragma unroll
-            for (int q = 0; q < GEN_NQ; ++q) {
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    float2 Cv, Sv;
-                    __sincosf(x[q][j].x, &Sv.x, &Cv.x);                // |x| <= pi is checked at load for this variant
-                    __sincosf(x[q][j].y, &Sv.y, &Cv.y);
-                    C2[q][j] = __fadd2_rn(Cv, Cv);
-                    cm[q][j] = one2; c[q][j] = __fmul2_rn(Cv, one2);
-                    sm[q][j] = make_float2(0.f, 0.f); sn[q][j] = __fmul2_rn(Sv, one2);
-                }
+            for (int j = 0; j < 4; ++j) {
+                float2 Cv, Sv;
+                __sincosf(xn[2 * j], &Sv.x, &Cv.x);                    // |x| <= pi is checked at load for this variant
+                __sincosf(xn[2 * j + 1], &Sv.y, &Cv.y);
+                C2[j] = __fadd2_rn(Cv, Cv);
+                ca[j] = one2; cb[j] = __fmul2_rn(Cv, one2);                       // cos 0x, cos(-x)
+                sa[j] = make_float2(0.f, 0.f); sb[j] = neg2(__fmul2_rn(Sv, one2)); // sin 0x, sin(-x)
             }
+            load_x(tile + n_pairs, xn);
+            put(c, ca); c += G;                        // tau = 0: the constant term
+            for (int m = 1; m <= d; m += 2) {
 #pragma unroll
-            for (int q = 0; q < GEN_NQ; ++q) if (q < nq) put(G + c0 + q * GEN_SETS, c[q]);          // cos x
+                for (int j = 0; j < 4; ++j) cb[j] = __ffma2_rn(C2[j], ca[j], neg2(cb[j]));
+                put(c, cb); c += G;                    // tau = 2m - 1: cos mx
 #pragma unroll
-            for (int q = 0; q < GEN_NQ; ++q) if (q < nq) put(2 * G + c0 + q * GEN_SETS, sn[q]);     // sin x
-            for (int m = 2; m <= d; ++m) {
+                for (int j = 0; j < 4; ++j) sb[j] = __ffma2_rn(C2[j], sa[j], neg2(sb[j]));
+                put(c, sb); c += G;                    // tau = 2m: sin mx
+                if (m + 1 <= d) {
 #pragma unroll
-                for (int q = 0; q < GEN_NQ; ++q) {
-                    if (q >= nq) continue;
+                    for (int j = 0; j < 4; ++j) ca[j] = __ffma2_rn(C2[j], cb[j], neg2(ca[j]));
+                    put(c, ca); c += G;
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        const float2 c1 = __ffma2_rn(C2[q][j], c[q][j], make_float2(-cm[q][j].x, -cm[q][j].y));
-                        cm[q][j] = c[q][j]; c[q][j] = c1;
-                    }
-                    put((2 * m - 1) * G + c0 + q * GEN_SETS, c[q]);
-                }
-#pragma unroll
-                for (int q = 0; q < GEN_NQ; ++q) {
-                    if (q >= nq) continue;
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        const float2 s1 = __ffma2_rn(C2[q][j], sn[q][j], make_float2(-sm[q][j].x, -sm[q][j].y));
-                        sm[q][j] = sn[q][j]; sn[q][j] = s1;
-                    }
-                    put(2 * m * G + c0 + q * GEN_SETS, sn[q]);
+                    for (int j = 0; j < 4; ++j) sa[j] = __ffma2_rn(C2[j], sb[j], neg2(sa[j]));
+                    put(c, sa); c += G;
                 }
             }
         }
-        float2 zeros[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
-        for (int c = T * G + set; c < nchunks; c += GEN_SETS) put(c, zeros);          // K padded up to whole k-blocks
-        while (cur_kb < k_blocks) next_stage();            // publish what is left of the tile; on to the next tile's first stage
-        cur_kb = 0;
+        const float2 zeros[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+        for (; c < nchunks; c += G) put(c, zeros);     // K padded up to whole k-blocks (c = T * G + g here)
+        advance();                                     // publish the tile's last k-block; on to the next tile's first stage
+        c_end = 8;
     }
+    (void)T;
+    if (tr) TRACE_DONE(cta_rank);
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------
@@ -215,7 +219,7 @@ __device__ __forceinline__ void generate_expansion(const float *__restrict__ X, 
 // SHARE: see epilogue_chunk.  k_last: UMMA k-steps (of 16 terms) that hold real terms in the LAST k-block -- the
 // padding steps beyond them would multiply zeros (config 3: K = 112 = 7 steps, not 8) and are not issued.
 template <int CG, int ACT, bool TMSE, int EW, int SRC, int FAMILY, bool TEAMS, int BNT = BN, int SHARE = 0>
-__global__ void __launch_bounds__(64 + 32 * EW + (SRC == SRC_GEN ? 32 * GEN_WARPS : 0), 1)
+__global__ void __launch_bounds__(SRC == SRC_GEN ? GEN_THREADS : 64 + 32 * EW, 1)
 fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmE,
                   int n_tiles, int m_blocks, int k_blocks, long long N, const float *__restrict__ tgt, float R,
                   float *__restrict__ partial, int Ppad, const DevState *state,
@@ -230,7 +234,10 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     constexpr int STAGE_BYTES_K = A_BYTES + B_BYTES_K;
     constexpr int NSTAGES = RESIDENT_A ? GEN_STAGES : (STAGE_BYTES_K <= 32768 ? 6 : 4);
     static_assert(BNT != BN || (STAGE_BYTES_K == C::STAGE_BYTES && NSTAGES == (RESIDENT_A ? GEN_STAGES : C::STAGES)), "Cfg<CG> describes the full-size tile");
-    constexpr int WARP_GEN0 = WARP_EPI0 + EW;
+    // SRC_GEN: roles are laid out by warpgroup so that setmaxnreg can move registers between them
+    constexpr int EPI0 = SRC == SRC_GEN ? 4 : WARP_EPI0;
+    constexpr int WARP_GEN0 = EPI0 + EW, WARP_RELAY = 2;
+    static_assert(SRC != SRC_GEN || EW == 4, "generator variant: one epilogue warpgroup");
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t *gbase = smem_raw + (base - smem_u32(smem_raw));
@@ -253,6 +260,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     if (CG == 2) asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(cta_rank));
     const int pair = blockIdx.x / CG, n_pairs = gridDim.x / CG;
     const int total_tiles = n_tiles * m_blocks;
+    TRACE_DECL;
 
     if (threadIdx.x == 0) {
         // SRC_GEN: a B stage is full when the generator warps of BOTH CTAs have published their half
@@ -275,96 +283,114 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     pdl_wait();
     const bool stopped = state && state->stopped;      // uniform across the grid: the loop has stopped, nothing to do
 
-    if (stopped) {
-    } else if (warp == WARP_TMA) {
-        // ===== TMA producer =====
-        if (lane == 0 && RESIDENT_A) {
-            // the population tile is loaded ONCE and stays: block kb of this CTA's 128 chromosomes at base + kb * A_BYTES
-            if (cta_rank == 0) mbar_expect_tx(afull_bar, (uint32_t)(CG * k_blocks * A_BYTES));
-            for (int kb = 0; kb < k_blocks; ++kb)
-                tma_load_2d<CG>(base + kb * A_BYTES, &tmC, kb * BKB, (int)cta_rank * BM, afull_bar);
-        }
-        if (SRC == SRC_GEN) {
-            // relay: the generators never stall on the hand-over -- each thread makes its stores visible to the async
-            // proxy and arrives (non-blocking) on the stage's named barrier; this otherwise idle warp completes that
-            // barrier and performs the one mbarrier arrival per CTA and stage on the leader's barrier.  (Arriving on
-            // the mbarrier straight from the generator warps was measured slower: 0.322 vs 0.287 ms on config 4.)
-            int s = 0;
-            for (int tile = pair; tile < total_tiles; tile += n_pairs)
-                for (int kb = 0; kb < k_blocks; ++kb) {
-                    asm volatile("bar.sync %0, %1;" ::"r"(GEN_BAR0 + s), "n"(32 * GEN_WARPS + 32) : "memory");
-                    if (lane == 0) {
-                        if (cta_rank == 0) mbar_arrive(full_bar(s)); else mbar_arrive_cluster(full_bar(s), 0);
+    // SRC_GEN lays the roles out by warpgroup and moves registers between them (setmaxnreg, inside the role branches so
+    // that each one dominates its code): a 768-thread CTA starts with 80 registers per thread; the epilogue needs more
+    // (two 32-register accumulator chunks in flight), the first warpgroup (TMA, MMA, relay) and the generators fewer
+    if (SRC == SRC_GEN && warp >= WARP_GEN0) {
+        // ===== generator warps (a1 inside the kernel) =====
+        setmaxnreg_dec<GEN_REGS_GEN>();
+        if (!stopped)
+            generate_expansion<FAMILY>(X, F, degree, N, k_blocks, pair, n_pairs, total_tiles, (int)cta_rank,
+                                       threadIdx.x - 32 * WARP_GEN0, base + k_blocks * A_BYTES, bar0);
+    } else if (warp < EPI0) {
+        if (SRC == SRC_GEN) setmaxnreg_dec<GEN_REGS_LOW>();
+        if (stopped) {
+        } else if (warp == WARP_TMA) {
+            // ===== TMA producer =====
+            if (lane == 0 && RESIDENT_A) {
+                // the population tile is loaded ONCE and stays: block kb of this CTA's 128 chromosomes at base + kb * A_BYTES
+                if (cta_rank == 0) mbar_expect_tx(afull_bar, (uint32_t)(CG * k_blocks * A_BYTES));
+                for (int kb = 0; kb < k_blocks; ++kb)
+                    tma_load_2d<CG>(base + kb * A_BYTES, &tmC, kb * BKB, (int)cta_rank * BM, afull_bar);
+            }
+            if (SRC == SRC_GEN) {
+            } else if (SRC == SRC_RES) {
+                if (lane == 0) {                                  // stream this CTA's 128-pattern half of every B k-block
+                    int s = 0; uint32_t ph = 0;
+                    for (int tile = pair; tile < total_tiles; tile += n_pairs) {
+                        const int rowE = tile * k_blocks * BN + (int)cta_rank * 128;
+                        for (int kb = 0; kb < k_blocks; ++kb) {
+                            mbar_wait<SUSP>(empty_bar(s), ph ^ 1);
+                            if (cta_rank == 0) mbar_expect_tx(full_bar(s), CG * GEN_B_BYTES);
+                            tma_load_2d<CG>(base + k_blocks * A_BYTES + s * GEN_B_BYTES, &tmE, 0, rowE + kb * BN, full_bar(s));
+                            if (++s == NSTAGES) { s = 0; ph ^= 1; }
+                        }
                     }
-                    if (++s == GEN_STAGES) s = 0;
                 }
-        } else if (SRC == SRC_RES) {
-            if (lane == 0) {                                  // stream this CTA's 128-pattern half of every B k-block
+            } else if (lane == 0) {
                 int s = 0; uint32_t ph = 0;
                 for (int tile = pair; tile < total_tiles; tile += n_pairs) {
-                    const int rowE = tile * k_blocks * BN + (int)cta_rank * 128;
+                    const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
+                    const int rowC = (m_blk * CG + (int)cta_rank) * BM;
+                    // E16 is tile-blocked [n/256][kb][256][64]: this tile's (and this CTA's) rows inside the 256-row block
+                    const int n_first = n_tile * BNT + (int)cta_rank * (BNT / CG);
+                    const int rowE = (n_first >> 8) * k_blocks * BN + (n_first & 255);
                     for (int kb = 0; kb < k_blocks; ++kb) {
                         mbar_wait<SUSP>(empty_bar(s), ph ^ 1);
-                        if (cta_rank == 0) mbar_expect_tx(full_bar(s), CG * GEN_B_BYTES);
-                        tma_load_2d<CG>(base + k_blocks * A_BYTES + s * GEN_B_BYTES, &tmE, 0, rowE + kb * BN, full_bar(s));
+                        const uint32_t sa = base + s * STAGE_BYTES_K, sb = sa + A_BYTES;
+                        if (CG == 1 || cta_rank == 0) mbar_expect_tx(full_bar(s), CG * STAGE_BYTES_K);
+                        tma_load_2d<CG>(sa, &tmC, kb * BKB, rowC, full_bar(s));
+                        tma_load_2d<CG>(sb, &tmE, 0, rowE + kb * BN, full_bar(s));
                         if (++s == NSTAGES) { s = 0; ph ^= 1; }
                     }
                 }
             }
-        } else if (lane == 0) {
-            int s = 0; uint32_t ph = 0;
-            for (int tile = pair; tile < total_tiles; tile += n_pairs) {
-                const int n_tile = tile / m_blocks, m_blk = tile % m_blocks;
-                const int rowC = (m_blk * CG + (int)cta_rank) * BM;
-                // E16 is tile-blocked [n/256][kb][256][64]: this tile's (and this CTA's) rows inside the 256-row block
-                const int n_first = n_tile * BNT + (int)cta_rank * (BNT / CG);
-                const int rowE = (n_first >> 8) * k_blocks * BN + (n_first & 255);
-                for (int kb = 0; kb < k_blocks; ++kb) {
-                    mbar_wait<SUSP>(empty_bar(s), ph ^ 1);
-                    const uint32_t sa = base + s * STAGE_BYTES_K, sb = sa + A_BYTES;
-                    if (CG == 1 || cta_rank == 0) mbar_expect_tx(full_bar(s), CG * STAGE_BYTES_K);
-                    tma_load_2d<CG>(sa, &tmC, kb * BKB, rowC, full_bar(s));
-                    tma_load_2d<CG>(sb, &tmE, 0, rowE + kb * BN, full_bar(s));
-                    if (++s == NSTAGES) { s = 0; ph ^= 1; }
-                }
-            }
-        }
-    } else if (warp == WARP_MMA) {
-        // ===== MMA issuer (one thread; leader CTA only when paired) =====
-        if (lane == 0 && cta_rank == 0) {
-            constexpr uint32_t idesc = make_idesc(BM * CG, BNT);
-            int s = 0; uint32_t ph = 0;
-            int acc = 0; uint32_t aph = 0;
-            if (RESIDENT_A) mbar_wait<SUSP>(afull_bar, 0);          // resident population tile of both CTAs
-            for (int tile = pair; tile < total_tiles; tile += n_pairs) {
-                mbar_wait<SUSP>(tempty_bar(acc), aph ^ 1);          // epilogue has drained this accumulator
-                tc_fence_after();
-                const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BNT);
-                for (int kb = 0; kb < k_blocks; ++kb) {
-                    mbar_wait<SUSP>(full_bar(s), ph);               // operands have landed (SRC_GEN: were generated)
+        } else if (warp == WARP_MMA) {
+            // ===== MMA issuer (one thread; leader CTA only when paired) =====
+            if (lane == 0 && cta_rank == 0) {
+                constexpr uint32_t idesc = make_idesc(BM * CG, BNT);
+                int s = 0; uint32_t ph = 0;
+                int acc = 0; uint32_t aph = 0;
+                if (RESIDENT_A) mbar_wait<SUSP>(afull_bar, 0);          // resident population tile of both CTAs
+                for (int tile = pair; tile < total_tiles; tile += n_pairs) {
+                    mbar_wait<SUSP>(tempty_bar(acc), aph ^ 1);          // epilogue has drained this accumulator
                     tc_fence_after();
-                    const uint32_t sa = RESIDENT_A ? base + kb * A_BYTES : base + s * STAGE_BYTES_K;
-                    const uint32_t sb = RESIDENT_A ? base + k_blocks * A_BYTES + s * GEN_B_BYTES : sa + A_BYTES;
-                    const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sb);
-                    const int nk = kb + 1 == k_blocks ? k_last : BKB / UMMA_K;
-#pragma unroll
-                    for (int k = 0; k < BKB / UMMA_K; ++k) {
-                        // advance 16 fp16 = 32 bytes inside the swizzle row: +2 in 16-byte units
-                        if (k < nk) umma_f16<CG>(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
+                    const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BNT);
+                    for (int kb = 0; kb < k_blocks; ++kb) {
+                        if (pair == 0) TRACE(4);
+                        mbar_wait<SUSP>(full_bar(s), ph);               // operands have landed (SRC_GEN: were generated)
+                        if (pair == 0) TRACE(4);
+                        tc_fence_after();
+                        const uint32_t sa = RESIDENT_A ? base + kb * A_BYTES : base + s * STAGE_BYTES_K;
+                        const uint32_t sb = RESIDENT_A ? base + k_blocks * A_BYTES + s * GEN_B_BYTES : sa + A_BYTES;
+                        const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sb);
+                        const int nk = kb + 1 == k_blocks ? k_last : BKB / UMMA_K;
+    #pragma unroll
+                        for (int k = 0; k < BKB / UMMA_K; ++k) {
+                            // advance 16 fp16 = 32 bytes inside the swizzle row: +2 in 16-byte units
+                            if (k < nk) umma_f16<CG>(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
+                        }
+                        umma_commit<CG>(empty_bar(s));            // stage reusable when these MMAs retire
+                        if (pair == 0) TRACE(4);
+                        if (++s == NSTAGES) { s = 0; ph ^= 1; }
                     }
-                    umma_commit<CG>(empty_bar(s));            // stage reusable when these MMAs retire
-                    if (++s == NSTAGES) { s = 0; ph ^= 1; }
+                    umma_commit<CG>(tfull_bar(acc));              // accumulator complete
+                    if (++acc == 2) { acc = 0; aph ^= 1; }
                 }
-                umma_commit<CG>(tfull_bar(acc));              // accumulator complete
-                if (++acc == 2) { acc = 0; aph ^= 1; }
+                if (pair == 0) TRACE_DONE(4);
             }
+        } else if (SRC == SRC_GEN && warp == WARP_RELAY) {
+            // ===== relay: the generators never stall on the hand-over -- each thread makes its stores visible to the async
+            // proxy and arrives (non-blocking) on the stage's named barrier; this warp completes that barrier and performs
+            // the one mbarrier arrival per CTA and stage on the leader's barrier =====
+            const int G = (F + 7) >> 3;
+            const int bar_count = 128 * (G < GEN_GROUPS ? G : GEN_GROUPS) + 32;
+            int s = 0;
+            for (int tile = pair; tile < total_tiles; tile += n_pairs)
+                for (int kb = 0; kb < k_blocks; ++kb) {
+                    asm volatile("bar.sync %0, %1;" ::"r"(GEN_BAR0 + s), "r"(bar_count) : "memory");
+                    if (lane == 0) {
+                        if (pair == 0) TRACE(2 + cta_rank);
+                        if (cta_rank == 0) mbar_arrive(full_bar(s)); else mbar_arrive_cluster(full_bar(s), 0);
+                    }
+                    if (++s == GEN_STAGES) s = 0;
+                }
+            if (lane == 0 && pair == 0) TRACE_DONE(2 + cta_rank);
         }
-    } else if (SRC == SRC_GEN && warp >= WARP_GEN0) {
-        // ===== generator warps (a1 inside the kernel) =====
-        generate_expansion<FAMILY>(X, F, degree, N, k_blocks, pair, n_pairs, total_tiles, (int)cta_rank,
-                                   threadIdx.x - 32 * WARP_GEN0, gbase + k_blocks * A_BYTES, bar0);
     } else {
-        if (TEAMS) {
+        if (SRC == SRC_GEN) setmaxnreg_inc<GEN_REGS_EPI>();
+        if (stopped) {
+        } else if (TEAMS) {
             // ===== epilogue warps: two independent teams of four =====
             // Warp w may touch TMEM lanes 32*(w%4).., so four warps cover a tile's 128 chromosomes.  Team g (warps 4g..4g+3)
             // owns accumulator g and takes every other tile of this CTA's sequence: a thread walks ALL 256 pattern columns of
@@ -378,7 +404,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             // residual exactly zero (their expansion rows are zero, so z = 0): no masked code path.
             static_assert(!TEAMS || EW == 8, "two teams of four warps");
             constexpr int NCH = BNT / 32;               // 32-column chunks per tile: 8 (4 for half-size tiles)
-            const int ew = warp - WARP_EPI0;
+            const int ew = warp - EPI0;
             const int team = ew >> 2;
             const int quarter = warp & 3;               // TMEM lane quarter this warp may touch
             const int tt = (ew & 3) * 32 + lane;        // thread index inside the team, 0..127
@@ -442,10 +468,10 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             constexpr int NCB = EW / 4;                 // column blocks per tile
             constexpr int CBW = BN / NCB;               // columns per block: 128 or 64
             constexpr int NCH = CBW / 32;               // 32-column chunks per tile and warp: 4 or 2 (even)
-            const int ew = warp - WARP_EPI0;
+            const int ew = warp - EPI0;
             const int quarter = warp & 3;               // TMEM lane quarter this warp may touch
             const int cb = ew >> 2;                     // which column block of the 256-column tile
-            const int et = threadIdx.x - 32 * WARP_EPI0;
+            const int et = threadIdx.x - 32 * EPI0;
             // One continuous stream of 32-column chunks: the TMEM load of the next chunk -- the next TILE's first chunk
             // included -- is in flight while the current one is evaluated.  Targets are staged one tile ahead in a ring
             // of three buffers: the buffer written during tile i was last read in tile i-2, and the one barrier per tile
@@ -675,7 +701,7 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     if (pairs > total) pairs = (int)total;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)(pairs * CG));
-    cfg.blockDim = dim3(64 + 32 * EW + (SRC == SRC_GEN ? 32 * GEN_WARPS : 0));
+    cfg.blockDim = dim3(SRC == SRC_GEN ? GEN_THREADS : 64 + 32 * EW);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[2];
@@ -703,7 +729,7 @@ int tensor_expansion(const game_ctx *ctx, int P)
 {
     const int Ppad = ((P + 255) / 256) * 256;
     const int k_blocks = ctx->Kpad / BKB;
-    const bool can = tc_permuted(ctx->family) && Ppad == 256 && ctx->X != nullptr && ctx->F <= 8 * GEN_SETS * GEN_NQ &&
+    const bool can = tc_permuted(ctx->family) && Ppad == 256 && ctx->X != nullptr && ctx->F <= 8 * GEN_GROUPS &&
                      k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES <= 227 * 1024 &&
                      (ctx->family != GAME_TRIG || ctx->x_maxabs <= 3.14159f);
     if (ctx->expand_mode == GAME_EXPAND_REGENERATED) return can ? GAME_EXPAND_REGENERATED : -1;
@@ -807,3 +833,15 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
 }
 
 }  // namespace game
+
+#ifdef GAME_TRACE
+extern "C" int game_trace_read(unsigned long long *buf, unsigned int *n)
+{
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(buf, game::g_trace, sizeof(game::g_trace));
+    cudaMemcpyFromSymbol(n, game::g_trace_n, sizeof(game::g_trace_n));
+    unsigned int zero[8] = {0};
+    cudaMemcpyToSymbol(game::g_trace_n, zero, sizeof(zero));
+    return 0;
+}
+#endif

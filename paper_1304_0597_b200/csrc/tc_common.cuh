@@ -45,12 +45,14 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t rank)
 // wall-clock time (globaltimer, looked at every 2^16 probes), not a probe count, so a debugger, time-slicing or a
 // profiler replay that stalls the kernel for a while cannot trip it.
 constexpr unsigned long long MBAR_TIMEOUT_NS = 20ull * 1000 * 1000 * 1000;
-static __device__ __noinline__ void mbar_timeout_check(unsigned long long &t0)
+// (t0 travels by value: a reference would pin it to a stack slot and put a local store into every wait loop)
+static __device__ __noinline__ unsigned long long mbar_timeout_check(unsigned long long t0)
 {
     unsigned long long now;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
-    if (t0 == 0) t0 = now;
-    else if (now - t0 > MBAR_TIMEOUT_NS) __trap();
+    if (t0 == 0) return now;
+    if (now - t0 > MBAR_TIMEOUT_NS) __trap();
+    return t0;
 }
 template <bool SUSPEND = false>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
@@ -64,8 +66,18 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         else
             asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                          : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-        if ((spin & 0xFFFFu) == 0xFFFFu) mbar_timeout_check(t0);
+        if ((spin & 0xFFFFu) == 0xFFFFu) t0 = mbar_timeout_check(t0);
     }
+}
+// the same wait with the probing loop out of line: one try_wait on the fast path (for waits that mostly succeed at once
+// and sit in code that is inlined many times)
+static __device__ __noinline__ void mbar_wait_slow(uint32_t bar, uint32_t parity) { mbar_wait<false>(bar, parity); }
+__device__ __forceinline__ void mbar_wait_lean(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (!ok) mbar_wait_slow(bar, parity);
 }
 // non-blocking: has the phase with this parity completed?
 __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity)
@@ -75,6 +87,9 @@ __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity)
                  : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
+// setmaxnreg for the calling warpgroup (all four warps must execute it together)
+template <int REGS> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS)); }
+template <int REGS> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS)); }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // all state spaces: orders this thread's generic-proxy accesses (global stores included) with async-proxy (TMA) ones
