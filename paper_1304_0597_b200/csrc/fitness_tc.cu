@@ -336,8 +336,11 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                 }
             }
         } else if (warp == WARP_MMA) {
-            // ===== MMA issuer (one thread; leader CTA only when paired) =====
-            if (lane == 0 && cta_rank == 0) {
+            // ===== MMA issuer (leader CTA only when paired) =====
+            // The whole warp walks the loop, so the ring position, the phases and the descriptors are warp-uniform values
+            // (kept in uniform registers); one elected lane issues the MMAs and their commits.  (Running the loop in a
+            // lane-0 branch instead made every tcgen05.mma cost ~25 instructions of vector -> uniform register traffic.)
+            if (cta_rank == 0) {
                 constexpr uint32_t idesc = make_idesc(BM * CG, BNT);
                 int s = 0; uint32_t ph = 0;
                 int acc = 0; uint32_t aph = 0;
@@ -347,27 +350,31 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                     tc_fence_after();
                     const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BNT);
                     for (int kb = 0; kb < k_blocks; ++kb) {
-                        if (pair == 0) TRACE(4);
+                        if (pair == 0 && lane == 0) TRACE(4);
                         mbar_wait<SUSP>(full_bar(s), ph);               // operands have landed (SRC_GEN: were generated)
-                        if (pair == 0) TRACE(4);
+                        if (pair == 0 && lane == 0) TRACE(4);
                         tc_fence_after();
                         const uint32_t sa = RESIDENT_A ? base + kb * A_BYTES : base + s * STAGE_BYTES_K;
                         const uint32_t sb = RESIDENT_A ? base + k_blocks * A_BYTES + s * GEN_B_BYTES : sa + A_BYTES;
                         const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sb);
-                        const int nk = kb + 1 == k_blocks ? k_last : BKB / UMMA_K;
+                        const bool last = kb + 1 == k_blocks;
+                        const int nk = last ? k_last : BKB / UMMA_K;
+                        if (elect_one()) {
     #pragma unroll
-                        for (int k = 0; k < BKB / UMMA_K; ++k) {
-                            // advance 16 fp16 = 32 bytes inside the swizzle row: +2 in 16-byte units
-                            if (k < nk) umma_f16<CG>(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
+                            for (int k = 0; k < BKB / UMMA_K; ++k) {
+                                // advance 16 fp16 = 32 bytes inside the swizzle row: +2 in 16-byte units
+                                if (k < nk) umma_f16<CG>(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
+                            }
+                            umma_commit<CG>(empty_bar(s));            // stage reusable when these MMAs retire
+                            if (last) umma_commit<CG>(tfull_bar(acc));  // accumulator complete
                         }
-                        umma_commit<CG>(empty_bar(s));            // stage reusable when these MMAs retire
-                        if (pair == 0) TRACE(4);
+                        __syncwarp();
+                        if (pair == 0 && lane == 0) TRACE(4);
                         if (++s == NSTAGES) { s = 0; ph ^= 1; }
                     }
-                    umma_commit<CG>(tfull_bar(acc));              // accumulator complete
                     if (++acc == 2) { acc = 0; aph ^= 1; }
                 }
-                if (pair == 0) TRACE_DONE(4);
+                if (pair == 0 && lane == 0) TRACE_DONE(4);
             }
         } else if (SRC == SRC_GEN && warp == WARP_RELAY) {
             // ===== relay: the generators never stall on the hand-over -- each thread makes its stores visible to the async
