@@ -33,14 +33,16 @@ constexpr int WARP_TMA = 0, WARP_MMA = 1, WARP_EPI0 = 2;      // warp roles; the
 constexpr int SRC_TMA = 0, SRC_GEN = 1, SRC_RES = 2;
 constexpr int GEN_WARPS = 16;           // generator threads: (pattern row of this CTA's 128-row B half, feature group)
 constexpr int GEN_GROUPS = GEN_WARPS / 4; // feature groups (of 8) the generator covers: F <= 32
-constexpr int GEN_EW = 4;               // epilogue warps of the generator variant (the epilogue is far from binding there)
+constexpr int GEN_EW = 8;               // epilogue warps of the generator variant (the epilogue is far from binding there)
 constexpr int GEN_STAGES = 4;           // B k-block stages of the generator ring
 constexpr int GEN_B_BYTES = 128 * BKB * 2;
 constexpr int GEN_THREADS = 128 + 32 * GEN_EW + 32 * GEN_WARPS;      // warpgroups: {TMA, MMA, relay, idle}, epilogue, 2 x generators
 // setmaxnreg: a 768-thread CTA starts at 80 registers per thread; the first warpgroup and the generators hand some to the epilogue
-constexpr int GEN_REGS_LOW = 56, GEN_REGS_GEN = 72, GEN_REGS_EPI = 128;
+// (two epilogue warpgroups on 896 threads -- 40 / 104 / 64 registers -- were measured slower: 0.269 vs 0.257 ms on config 4)
+constexpr int GEN_REGS_START = 72, GEN_REGS_LOW = 40, GEN_REGS_GEN = 72, GEN_REGS_EPI = 88;
 static_assert((GEN_STAGES & (GEN_STAGES - 1)) == 0, "ring slot = k-block count mod GEN_STAGES");
-static_assert(128 * GEN_REGS_LOW + 32 * GEN_WARPS * GEN_REGS_GEN + 32 * GEN_EW * GEN_REGS_EPI <= 80 * GEN_THREADS, "register pool of the CTA");
+static_assert(128 * GEN_REGS_LOW + 32 * GEN_WARPS * GEN_REGS_GEN + 32 * GEN_EW * GEN_REGS_EPI <= GEN_REGS_START * GEN_THREADS, "register pool of the CTA");
+static_assert(GEN_REGS_START * GEN_THREADS <= 65536, "register file");
 constexpr int GEN_BAR0 = 2;             // named barriers 2.. : one per generator stage (0 = CTA, 1 = epilogue)
 constexpr int MAX_STAGES = 6;           // barrier slots are laid out for the deepest ring
 constexpr int TC_TAIL_BYTES = 256 /*barriers*/ + 3 * BN * 4 /*targets: [3][BN], or [team][2][BN]*/ + 2 * 4 * BM * 4 /*column-block error sums of two tiles*/;
@@ -126,6 +128,9 @@ __device__ __forceinline__ void generate_expansion(const float *__restrict__ X, 
     };
     auto put = [&](int c, const float2 (&v)[4]) {      // chunk c of this thread's row
         if (c >= c_end) { advance(); c_end += 8; }
+#ifdef PROBE_NOSTORE
+        if (c < 0)
+#endif
         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};"
                      ::"r"(dst ^ (((uint32_t)c << 4) & 0x70u)), "r"(pack_half2(v[0])), "r"(pack_half2(v[1])),
                        "r"(pack_half2(v[2])), "r"(pack_half2(v[3])) : "memory");
@@ -237,7 +242,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     // SRC_GEN: roles are laid out by warpgroup so that setmaxnreg can move registers between them
     constexpr int EPI0 = SRC == SRC_GEN ? 4 : WARP_EPI0;
     constexpr int WARP_GEN0 = EPI0 + EW, WARP_RELAY = 2;
-    static_assert(SRC != SRC_GEN || EW == 4, "generator variant: one epilogue warpgroup");
+    static_assert(SRC != SRC_GEN || EW == GEN_EW, "generator variant: whole epilogue warpgroups");
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t *gbase = smem_raw + (base - smem_u32(smem_raw));
@@ -288,7 +293,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     // (two 32-register accumulator chunks in flight), the first warpgroup (TMA, MMA, relay) and the generators fewer
     if (SRC == SRC_GEN && warp >= WARP_GEN0) {
         // ===== generator warps (a1 inside the kernel) =====
-        setmaxnreg_dec<GEN_REGS_GEN>();
+        if (GEN_REGS_GEN < GEN_REGS_START) setmaxnreg_dec<GEN_REGS_GEN>();
         if (!stopped)
             generate_expansion<FAMILY>(X, F, degree, N, k_blocks, pair, n_pairs, total_tiles, (int)cta_rank,
                                        threadIdx.x - 32 * WARP_GEN0, base + k_blocks * A_BYTES, bar0);
@@ -346,11 +351,15 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                 int acc = 0; uint32_t aph = 0;
                 if (RESIDENT_A) mbar_wait<SUSP>(afull_bar, 0);          // resident population tile of both CTAs
                 for (int tile = pair; tile < total_tiles; tile += n_pairs) {
+                    if (pair == 0 && lane == 0) TRACE(4);
                     mbar_wait<SUSP>(tempty_bar(acc), aph ^ 1);          // epilogue has drained this accumulator
                     tc_fence_after();
                     const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BNT);
                     for (int kb = 0; kb < k_blocks; ++kb) {
                         if (pair == 0 && lane == 0) TRACE(4);
+#ifdef PROBE_NOFULLWAIT
+                        if (SRC != SRC_GEN)
+#endif
                         mbar_wait<SUSP>(full_bar(s), ph);               // operands have landed (SRC_GEN: were generated)
                         if (pair == 0 && lane == 0) TRACE(4);
                         tc_fence_after();
@@ -547,6 +556,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                             if (CG == 1) mbar_arrive(tempty_bar(acc));
                             else mbar_arrive_cluster(tempty_bar(acc), 0);
                         }
+                        if (pair == 0 && cta_rank == 0 && ew == 0 && lane == 0) TRACE(6);
 #pragma unroll
                         for (int u = 0; u < TPT; ++u) {
                             if (has_next && et + u * 32 * EW < BN) tgt_s[tbn * BN + et + u * 32 * EW] = t_next[u] - tbias;
@@ -555,7 +565,9 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                         epi_barrier();
                         flush(sb ^ 1);
                         if (has_next) {                   // uniform over the CTA's epilogue warps
+                            if (pair == 0 && cta_rank == 0 && ew == 0 && lane == 0) TRACE(6);
                             mbar_wait<SUSP>(tfull_bar(acc ^ 1), acc ? aph ^ 1 : aph);
+                            if (pair == 0 && cta_rank == 0 && ew == 0 && lane == 0) TRACE(6);
                             tc_fence_after();
                             tmem_ld32(lane_addr + (uint32_t)((acc ^ 1) * BN), nxt);
                         }
@@ -572,6 +584,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                 epi_barrier();
                 flush(sb ^ 1);
             }
+            if (pair == 0 && cta_rank == 0 && ew == 0 && lane == 0) TRACE_DONE(6);
         }
     }
 
