@@ -265,6 +265,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     if (CG == 2) asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(cta_rank));
     const int pair = blockIdx.x / CG, n_pairs = gridDim.x / CG;
     const int total_tiles = n_tiles * m_blocks;
+    const int my_tiles = pair < total_tiles ? (total_tiles - pair + n_pairs - 1) / n_pairs : 0;     // this CTA (pair) takes tiles pair, pair + n_pairs, ...
     TRACE_DECL;
 
     if (threadIdx.x == 0) {
@@ -350,7 +351,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                 int s = 0; uint32_t ph = 0;
                 int acc = 0; uint32_t aph = 0;
                 if (RESIDENT_A) mbar_wait<SUSP>(afull_bar, 0);          // resident population tile of both CTAs
-                for (int tile = pair; tile < total_tiles; tile += n_pairs) {
+                for (int t = 0; t < my_tiles; ++t) {
                     if (pair == 0 && lane == 0) TRACE(4);
                     mbar_wait<SUSP>(tempty_bar(acc), aph ^ 1);          // epilogue has drained this accumulator
                     tc_fence_after();
@@ -392,7 +393,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
             const int G = (F + 7) >> 3;
             const int bar_count = 128 * (G < GEN_GROUPS ? G : GEN_GROUPS) + 32;
             int s = 0;
-            for (int tile = pair; tile < total_tiles; tile += n_pairs)
+            for (int t = 0; t < my_tiles; ++t)
                 for (int kb = 0; kb < k_blocks; ++kb) {
                     asm volatile("bar.sync %0, %1;" ::"r"(GEN_BAR0 + s), "r"(bar_count) : "memory");
                     if (lane == 0) {
