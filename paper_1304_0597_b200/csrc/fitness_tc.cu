@@ -10,11 +10,13 @@
 // Persistent, warp-specialised CTAs (one per SM, or one CTA pair per two SMs with cta_group::2):
 //   warp 0      TMA producer: 128B-swizzled [rows x 64] fp16 boxes of C (A operand) and E (B operand)
 //               into a ring of shared-memory stages, completion on mbarriers
-//   warp 1      TMEM allocator and the single-thread MMA issuer; tcgen05.commit frees stages and
-//               publishes finished accumulators
+//   warp 1      TMEM allocator and the MMA issuer (the whole warp walks the loop, one elected lane issues);
+//               tcgen05.commit frees stages and publishes finished accumulators
 //   warps 2-9   epilogue: tcgen05.ld the accumulator (two 128x256 fp32 buffers = all 512 TMEM columns, so
 //               the epilogue of tile i overlaps the MMAs of tile i+1), sigmoid, error, row sum, one
 //               coalesced store per warp into partial[slab][p]
+// (The regenerated variant, SRC_GEN, lays its roles out by warpgroup instead: {TMA, MMA, relay, idle}, two epilogue
+// warpgroups, four generator warpgroups -- 896 threads, registers moved between the groups with setmaxnreg.)
 // Tiles are ordered chromosome-block fastest so CTAs running together share the same E tile out of L2.
 // finalize_kernel (fitness_fp32.cu) then adds the slabs in fixed order: no float atomics, bit-reproducible,
 // and a chromosome's result does not depend on its row (DESIGN P20).
@@ -25,7 +27,7 @@ namespace game {
 constexpr int WARP_TMA = 0, WARP_MMA = 1, WARP_EPI0 = 2;      // warp roles; the epilogue warps follow (EW = 8 or 16 of them)
 // Where the B operand (the expansion tile) comes from:
 //   SRC_TMA  streamed from the materialised E16 in HBM, together with the A (population) tile, through a TMA ring
-//   SRC_GEN  regenerated from X inside the kernel by four generator warps writing 128B-swizzled k-blocks straight
+//   SRC_GEN  regenerated from X inside the kernel by sixteen generator warps writing 128B-swizzled k-blocks straight
 //            into shared memory, with the whole population tile RESIDENT in shared memory (small populations:
 //            one CTA pair covers all chromosomes, so every expansion value is generated exactly once per launch)
 //   SRC_RES  the resident population tile of SRC_GEN, with the B halves streamed from E16 by TMA into the same ring
@@ -33,12 +35,13 @@ constexpr int WARP_TMA = 0, WARP_MMA = 1, WARP_EPI0 = 2;      // warp roles; the
 constexpr int SRC_TMA = 0, SRC_GEN = 1, SRC_RES = 2;
 constexpr int GEN_WARPS = 16;           // generator threads: (pattern row of this CTA's 128-row B half, feature group)
 constexpr int GEN_GROUPS = GEN_WARPS / 4; // feature groups (of 8) the generator covers: F <= 32
-constexpr int GEN_EW = 8;               // epilogue warps of the generator variant (the epilogue is far from binding there)
+constexpr int GEN_EW = 8;               // epilogue warps of the generator variant (four were the bottleneck once the generator was fast: 0.257 vs 0.222 ms)
 constexpr int GEN_STAGES = 4;           // B k-block stages of the generator ring
 constexpr int GEN_B_BYTES = 128 * BKB * 2;
-constexpr int GEN_THREADS = 128 + 32 * GEN_EW + 32 * GEN_WARPS;      // warpgroups: {TMA, MMA, relay, idle}, epilogue, 2 x generators
-// setmaxnreg: a 768-thread CTA starts at 80 registers per thread; the first warpgroup and the generators hand some to the epilogue
-// (two epilogue warpgroups on 896 threads -- 40 / 104 / 64 registers -- were measured slower: 0.269 vs 0.257 ms on config 4)
+constexpr int GEN_THREADS = 128 + 32 * GEN_EW + 32 * GEN_WARPS;      // warpgroups: {TMA, MMA, relay, idle}, 2 x epilogue, 4 x generators
+// setmaxnreg: an 896-thread CTA starts at 72 registers per thread; the first warpgroup hands registers to the epilogue.
+// Measured on config 4: 40 / 88 / 72 (first warpgroup / epilogue / generators) 0.217 ms; 40 / 104 / 64 (generators spill)
+// 0.269 ms; one epilogue warpgroup on 768 threads, 56 / 128 / 72: 0.257 ms.
 constexpr int GEN_REGS_START = 72, GEN_REGS_LOW = 40, GEN_REGS_GEN = 72, GEN_REGS_EPI = 88;
 static_assert((GEN_STAGES & (GEN_STAGES - 1)) == 0, "ring slot = k-block count mod GEN_STAGES");
 static_assert(128 * GEN_REGS_LOW + 32 * GEN_WARPS * GEN_REGS_GEN + 32 * GEN_EW * GEN_REGS_EPI <= GEN_REGS_START * GEN_THREADS, "register pool of the CTA");
@@ -46,19 +49,6 @@ static_assert(GEN_REGS_START * GEN_THREADS <= 65536, "register file");
 constexpr int GEN_BAR0 = 2;             // named barriers 2.. : one per generator stage (0 = CTA, 1 = epilogue)
 constexpr int MAX_STAGES = 6;           // barrier slots are laid out for the deepest ring
 constexpr int TC_TAIL_BYTES = 256 /*barriers*/ + 3 * BN * 4 /*targets: [3][BN], or [team][2][BN]*/ + 2 * 4 * BM * 4 /*column-block error sums of two tiles*/;
-
-#ifdef GAME_TRACE
-// measurement build only (-DGAME_TRACE, never the shipped library): clock64 stamps of the hand-overs of CTA pair 0
-__device__ unsigned long long g_trace[8][8192];
-__device__ unsigned int g_trace_n[8];
-#define TRACE(role) do { if (trace_i < 8192) g_trace[role][trace_i++] = clock64(); } while (0)
-#define TRACE_DONE(role) do { g_trace_n[role] = trace_i; } while (0)
-#define TRACE_DECL unsigned int trace_i = 0
-#else
-#define TRACE(role) do { } while (0)
-#define TRACE_DONE(role) do { } while (0)
-#define TRACE_DECL do { } while (0)
-#endif
 
 template <int CG> struct Cfg {
     static constexpr int BNL = BN / CG;                 // pattern rows this CTA stages
@@ -112,25 +102,17 @@ __device__ __forceinline__ void generate_expansion(const float *__restrict__ X, 
     int c_end = 8;                                     // first chunk of the NEXT k-block of the tile
     uint32_t dst = my_row;
     mbar_wait(empty0, 1);                              // stage 0 starts free
-    const bool tr = pair == 0 && gt == 0; (void)tr;
-    TRACE_DECL;
 
     auto advance = [&]() {                             // publish the stage being written, move on to the next k-block
-        if (tr) TRACE(cta_rank);
         fence_proxy_async();                           // generic-proxy stores -> visible to the tensor core's async proxy
         asm volatile("bar.arrive %0, %1;" ::"r"(GEN_BAR0 + (it & (GEN_STAGES - 1))), "r"(bar_count) : "memory");
         ++it;
         const uint32_t s = it & (GEN_STAGES - 1);
         dst = my_row + s * GEN_B_BYTES;
-        if (tr) TRACE(cta_rank);
         mbar_wait_lean(empty0 + 8u * s, ((it / GEN_STAGES) & 1u) ^ 1u);     // the MMAs that read this slot last have retired
-        if (tr) TRACE(cta_rank);
     };
     auto put = [&](int c, const float2 (&v)[4]) {      // chunk c of this thread's row
         if (c >= c_end) { advance(); c_end += 8; }
-#ifdef PROBE_NOSTORE
-        if (c < 0)
-#endif
         asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};"
                      ::"r"(dst ^ (((uint32_t)c << 4) & 0x70u)), "r"(pack_half2(v[0])), "r"(pack_half2(v[1])),
                        "r"(pack_half2(v[2])), "r"(pack_half2(v[3])) : "memory");
@@ -215,7 +197,6 @@ __device__ __forceinline__ void generate_expansion(const float *__restrict__ X, 
         c_end = 8;
     }
     (void)T;
-    if (tr) TRACE_DONE(cta_rank);
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------
@@ -266,7 +247,6 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
     const int pair = blockIdx.x / CG, n_pairs = gridDim.x / CG;
     const int total_tiles = n_tiles * m_blocks;
     const int my_tiles = pair < total_tiles ? (total_tiles - pair + n_pairs - 1) / n_pairs : 0;     // this CTA (pair) takes tiles pair, pair + n_pairs, ...
-    TRACE_DECL;
 
     if (threadIdx.x == 0) {
         // SRC_GEN: a B stage is full when the generator warps of BOTH CTAs have published their half
@@ -352,17 +332,11 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                 int acc = 0; uint32_t aph = 0;
                 if (RESIDENT_A) mbar_wait<SUSP>(afull_bar, 0);          // resident population tile of both CTAs
                 for (int t = 0; t < my_tiles; ++t) {
-                    if (pair == 0 && lane == 0) TRACE(4);
                     mbar_wait<SUSP>(tempty_bar(acc), aph ^ 1);          // epilogue has drained this accumulator
                     tc_fence_after();
                     const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BNT);
                     for (int kb = 0; kb < k_blocks; ++kb) {
-                        if (pair == 0 && lane == 0) TRACE(4);
-#ifdef PROBE_NOFULLWAIT
-                        if (SRC != SRC_GEN)
-#endif
                         mbar_wait<SUSP>(full_bar(s), ph);               // operands have landed (SRC_GEN: were generated)
-                        if (pair == 0 && lane == 0) TRACE(4);
                         tc_fence_after();
                         const uint32_t sa = RESIDENT_A ? base + kb * A_BYTES : base + s * STAGE_BYTES_K;
                         const uint32_t sb = RESIDENT_A ? base + k_blocks * A_BYTES + s * GEN_B_BYTES : sa + A_BYTES;
@@ -379,12 +353,10 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                             if (last) umma_commit<CG>(tfull_bar(acc));  // accumulator complete
                         }
                         __syncwarp();
-                        if (pair == 0 && lane == 0) TRACE(4);
                         if (++s == NSTAGES) { s = 0; ph ^= 1; }
                     }
                     if (++acc == 2) { acc = 0; aph ^= 1; }
                 }
-                if (pair == 0 && lane == 0) TRACE_DONE(4);
             }
         } else if (SRC == SRC_GEN && warp == WARP_RELAY) {
             // ===== relay: the generators never stall on the hand-over -- each thread makes its stores visible to the async
@@ -397,12 +369,10 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                 for (int kb = 0; kb < k_blocks; ++kb) {
                     asm volatile("bar.sync %0, %1;" ::"r"(GEN_BAR0 + s), "r"(bar_count) : "memory");
                     if (lane == 0) {
-                        if (pair == 0) TRACE(2 + cta_rank);
                         if (cta_rank == 0) mbar_arrive(full_bar(s)); else mbar_arrive_cluster(full_bar(s), 0);
                     }
                     if (++s == GEN_STAGES) s = 0;
                 }
-            if (lane == 0 && pair == 0) TRACE_DONE(2 + cta_rank);
         }
     } else {
         if (SRC == SRC_GEN) setmaxnreg_inc<GEN_REGS_EPI>();
@@ -557,7 +527,6 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                             if (CG == 1) mbar_arrive(tempty_bar(acc));
                             else mbar_arrive_cluster(tempty_bar(acc), 0);
                         }
-                        if (pair == 0 && cta_rank == 0 && ew == 0 && lane == 0) TRACE(6);
 #pragma unroll
                         for (int u = 0; u < TPT; ++u) {
                             if (has_next && et + u * 32 * EW < BN) tgt_s[tbn * BN + et + u * 32 * EW] = t_next[u] - tbias;
@@ -566,9 +535,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                         epi_barrier();
                         flush(sb ^ 1);
                         if (has_next) {                   // uniform over the CTA's epilogue warps
-                            if (pair == 0 && cta_rank == 0 && ew == 0 && lane == 0) TRACE(6);
                             mbar_wait<SUSP>(tfull_bar(acc ^ 1), acc ? aph ^ 1 : aph);
-                            if (pair == 0 && cta_rank == 0 && ew == 0 && lane == 0) TRACE(6);
                             tc_fence_after();
                             tmem_ld32(lane_addr + (uint32_t)((acc ^ 1) * BN), nxt);
                         }
@@ -585,7 +552,6 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                 epi_barrier();
                 flush(sb ^ 1);
             }
-            if (pair == 0 && cta_rank == 0 && ew == 0 && lane == 0) TRACE_DONE(6);
         }
     }
 
@@ -741,11 +707,13 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
 // north_star (1): materialise E or regenerate it in the kernel, by measured cost.  The generator variant needs the
 // whole population in ONE CTA pair (Ppad = 256) and its fp16 copy resident in shared memory beside the B ring, i.e.
 // exactly the shapes where streaming the materialised E16 could limit the kernel (bytes of E16 per flop ~ 1/P).
-// Measured on B200 on config 4 (N = 1e6, K = 544, P = 256), same box: materialised 0.268 ms, regenerated 0.287 ms
-// -- the generator's math is not what limits it (a no-math probe ran at the same 0.287 ms); the CTA-pair ring does
-// (47 % tensor-pipe use against 71 %).  So AUTO streams the materialised matrix; the regenerated variant stays
-// selectable (game_set_expansion) and is held to the same parity tests.  The trigonometric generator uses the fast
-// sincos, accurate on |x| <= pi only (checked against the dataset at load).
+// Measured on B200, same box, kernel ms materialised / regenerated (DESIGN.md section 7 has the table):
+//   trig d=8 F=32 (K=544) N=1e6: P=256 0.226 / 0.217, P=128 0.215 / 0.211, P=20 0.205 / 0.208; N=2e5 0.052 / 0.056
+//   cheb d=16 F=32 (K=544) N=1e6 P=256 0.228 / 0.215;  K=272 (F=16) 0.128 / 0.147;  K=160 (d=2) 0.100 / 0.146
+// so AUTO regenerates deep contractions (>= 8 k-blocks) over all four feature groups on datasets of >= 2000 tiles per
+// launch (the matrix no longer fits in L2 and the start-up -- resident population tile, first features -- is amortised)
+// for P > 32, and streams the materialised matrix everywhere else.  The trigonometric generator uses the fast sincos,
+// accurate on |x| <= pi only (checked against the dataset at load).
 int tensor_expansion(const game_ctx *ctx, int P)
 {
     const int Ppad = ((P + 255) / 256) * 256;
@@ -754,7 +722,9 @@ int tensor_expansion(const game_ctx *ctx, int P)
                      k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES <= 227 * 1024 &&
                      (ctx->family != GAME_TRIG || ctx->x_maxabs <= 3.14159f);
     if (ctx->expand_mode == GAME_EXPAND_REGENERATED) return can ? GAME_EXPAND_REGENERATED : -1;
-    return GAME_EXPAND_MATERIALIZED;
+    if (ctx->expand_mode == GAME_EXPAND_MATERIALIZED) return GAME_EXPAND_MATERIALIZED;
+    const bool pays = k_blocks >= 8 && ctx->F > 8 * (GEN_GROUPS - 1) && ctx->Npad256 / BN >= 2000 && P > 32;
+    return can && pays ? GAME_EXPAND_REGENERATED : GAME_EXPAND_MATERIALIZED;
 }
 
 // make the fp16 operand copy (C16 / C16s) mirror `pop`, unless the GA operators already wrote it while building `pop`
@@ -855,14 +825,3 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
 
 }  // namespace game
 
-#ifdef GAME_TRACE
-extern "C" int game_trace_read(unsigned long long *buf, unsigned int *n)
-{
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(buf, game::g_trace, sizeof(game::g_trace));
-    cudaMemcpyFromSymbol(n, game::g_trace_n, sizeof(game::g_trace_n));
-    unsigned int zero[8] = {0};
-    cudaMemcpyToSymbol(game::g_trace_n, zero, sizeof(zero));
-    return 0;
-}
-#endif

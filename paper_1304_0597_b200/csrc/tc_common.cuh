@@ -71,10 +71,8 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 }
 // the same wait with the probing loop out of line: one try_wait on the fast path (for waits that mostly succeed at once
 // and sit in code that is inlined many times)
-#ifndef GEN_WAIT_SUSPEND
-#define GEN_WAIT_SUSPEND false
-#endif
-static __device__ __noinline__ void mbar_wait_slow(uint32_t bar, uint32_t parity) { mbar_wait<GEN_WAIT_SUSPEND>(bar, parity); }
+// (a suspend-time hint in the out-of-line loop changes nothing: 0.2565 vs 0.2566 ms on config 4)
+static __device__ __noinline__ void mbar_wait_slow(uint32_t bar, uint32_t parity) { mbar_wait<false>(bar, parity); }
 __device__ __forceinline__ void mbar_wait_lean(uint32_t bar, uint32_t parity)
 {
     uint32_t ok;

@@ -540,6 +540,39 @@ def test_regenerated_expansion_limits():
     assert ctx2.resolved_expansion(64) == g.GAME_EXPAND_MATERIALIZED
 
 
+def test_auto_regenerates_config4_full_size(orc):
+    """AUTO's measured choice: config 4 -- 9 k-blocks, four feature groups, 3907 tiles -- runs the
+    regenerated expansion; both sources are held to the oracle at full size, agree closely with each other, and the
+    neighbouring shapes where the materialised matrix measured faster keep it."""
+    w = wl.config(4)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    rng = np.random.default_rng(41)
+    pop = rng.uniform(-1, 1, (w.P, w.K)).astype(np.float32)
+    rows = np.unique(np.concatenate([[0, w.P - 1], rng.choice(w.P, 6, replace=False)]))
+    ctx = make_ctx(fam, d, X, t, w.act, w.err, w.R, g.GAME_PATH_AUTO)
+    assert ctx.resolved_path(w.P) == g.GAME_PATH_TENSOR
+    assert ctx.resolved_expansion(w.P) == g.GAME_EXPAND_REGENERATED
+    assert ctx.resolved_expansion(20) == g.GAME_EXPAND_MATERIALIZED          # small populations: no gain measured
+    assert ctx.resolved_expansion(257) == g.GAME_EXPAND_MATERIALIZED         # more than one CTA pair of chromosomes
+    got = {}
+    for mode in (g.GAME_EXPAND_AUTO, g.GAME_EXPAND_MATERIALIZED):
+        ctx.set_expansion(mode)
+        got[mode] = ctx.fitness(dev(pop)).cpu().numpy()
+        check_fitness(orc, got[mode][rows], fam, d, X, t, pop[rows], w.act, w.err, w.R, g.GAME_PATH_TENSOR, "cfg 4 expansion %d" % mode)
+    # MSE is continuous in z: there the two sources must agree far inside the tolerance class
+    ctx.set_error(MSE, 0.0)
+    for mode in (g.GAME_EXPAND_AUTO, g.GAME_EXPAND_MATERIALIZED):
+        ctx.set_expansion(mode)
+        got[mode] = ctx.fitness(dev(pop)).cpu().numpy()
+    assert np.allclose(got[g.GAME_EXPAND_AUTO], got[g.GAME_EXPAND_MATERIALIZED], rtol=2e-4, atol=2e-6)
+    ctx.destroy()
+    # a fifth of the patterns (782 tiles per launch): the start-up is not amortised, AUTO streams the matrix
+    ctx = make_ctx(fam, d, X[:200000], t[:200000], w.act, w.err, w.R, g.GAME_PATH_AUTO)
+    assert ctx.resolved_expansion(w.P) == g.GAME_EXPAND_MATERIALIZED
+    ctx.destroy()
+
+
 def test_trajectory_regenerated(orc):
     """A GA run with the regenerated expansion: operators bit-exact, fitness within the tensor class."""
     w = wl.config(1).scaled(P=64, generations=6)
