@@ -58,6 +58,7 @@ enum { GAME_EXPAND_AUTO = 0, GAME_EXPAND_MATERIALIZED = 1, GAME_EXPAND_REGENERAT
  *   GAME_TUNE_TEAMS        1/0  two-team epilogue (auto: contraction depth <= 256)
  *   GAME_TUNE_HALF_TILES   1/0  128-pattern tiles for sub-wave problems (auto: by shape)
  *   GAME_TUNE_PERSISTENT   1/0  one persistent cooperative kernel per game_evolve for sub-wave problems (auto: by shape)
+ *                          2 = the persistent kernel without its local-population form (every CTA holding the whole population)
  *   GAME_TUNE_RATIONAL_SHARE  0..8  of every 16 evaluation PAIRS of the tanh logistic, how many are evaluated on the FMA
  *                          pipe by a rational form with one shared reciprocal (team epilogue, single CTAs; 1, 2 round
  *                          up to 3; auto: the measured best) */

@@ -14,22 +14,39 @@
 //   phase C  a8-a11  elitism, tournament selection, crossover, mutation for the CTA's share of the children, from the same
 //                    Philox counters as ga_step_kernel; also writes the next generation's fp16 operand copy.
 //   -- grid barrier --
+// Small populations (one chromosome block, P K <= PERS_LOCAL_GENES: config 1, the paper's own shape) keep the WHOLE
+// population in every CTA's shared memory: each CTA applies the operators to all children itself (same counters, same
+// bits), writes the fp16 operand tile where a TMA box would have put it, and CTA 0 mirrors the result to global memory --
+// no population traffic, no population load in phase A and no second grid barrier (the tile sums alternate between two
+// buffers so that a CTA one phase ahead cannot overwrite what a slower one still reads).
 // The arithmetic of every phase is the launch path's, operation for operation (same MMA shapes and k order, the same
 // epilogue code, the same summation order, the same integer decisions), so a run through this kernel is bit-identical
 // to stepping the multi-launch path one generation at a time; tests/test_gpu_parity.py holds it to that.
 #include "ga_device.cuh"
 #include "tc_common.cuh"
 
+#ifdef PERS_TRACE
+__device__ long long g_ptrace[4096];
+#define PTRACE(slot) do { if (blockIdx.x == 0 && threadIdx.x == PTRACE_TID && e >= 100 && e < 228) g_ptrace[(e - 100) * 8 + (slot)] = clock64(); } while (0)
+extern "C" int game_ptrace_read(long long *buf) { cudaDeviceSynchronize(); return (int)cudaMemcpyFromSymbol(buf, g_ptrace, sizeof(g_ptrace)); }
+#ifndef PTRACE_TID
+#define PTRACE_TID 64
+#endif
+#else
+#define PTRACE(slot) do { } while (0)
+#endif
 namespace game {
 
-constexpr int PERS_THREADS = 256;       // warp 0 TMA producer, warp 1 MMA issuer, warps 2-5 epilogue; all 8 warps in phases B, C
+constexpr int PERS_THREADS = 512;       // warp 0 TMA producer, warp 1 MMA issuer, warps 2-5 epilogue; all 8 warps in phases B, C
 constexpr int PERS_TILE_N = 128;        // patterns per tile: the half-size tiles the launch path uses below one wave
 constexpr int PERS_KB_BYTES = 128 * BKB * 2;
 constexpr int PERS_LOCAL_RANK = 256;    // up to this many chromosomes every CTA ranks the whole population itself
 constexpr int PERS_MAX_P = 2048;        // sort keys of the whole population live in shared memory
+constexpr int PERS_LOCAL_GENES = 4096;  // local-population mode: every CTA rebuilds all P K genes itself (two Philox calls per gene)
 
 struct PersistArgs {
     int n_tiles, m_blocks, k_blocks, kb1, split, k_last, P, Ppad, generations, err;
+    int local;                          // local-population mode (see the header)
     long long N;
     const float *tgt;
     float R, stop_error;
@@ -87,6 +104,12 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
     unsigned long long *keys = reinterpret_cast<unsigned long long *>(tail + 128 + 512);        // [P]
     float *fit_s = reinterpret_cast<float *>(keys + P);                                         // [P]
     int *order_s = reinterpret_cast<int *>(fit_s + P);                                          // [P] (local rank only)
+    // local-population mode: the population twice (this generation's and the next one's genes) and a staging area of its own
+    // for the tile sums (the population tile, which serves as staging area otherwise, now lives across the phases)
+    const uint32_t local_off = (uint32_t)(128 + 512 + P * 16 + 15) & ~15u;                     // 16-byte aligned, behind order_s
+    float *pop_s0 = reinterpret_cast<float *>(tail + local_off);                                // [P K]
+    float *pop_s1 = pop_s0 + ((P * K + 3) & ~3);                                                // [P K]
+    float *stage_local = pop_s1 + ((P * K + 3) & ~3);                                           // [n_tiles][P4]
     __shared__ int sh[8];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, tid = threadIdx.x;
@@ -126,6 +149,41 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
         }
     }
 
+    // local-population mode: gene k of chromosome p goes to the CTA's fp32 copy and, as fp16 (c16_store's rounding and
+    // positions), to the operand tile at the 128B-swizzled address a TMA box of C16 / C16s would have filled; CTA 0 mirrors
+    // both to global memory, so the context's population and fp16 copy are what the launch path would have left
+    const C16Sink &sink = a.step.sink;
+    const int Bterms = tc_terms_per_feature(sink.family, sink.d);
+    struct GeneSlot { uint32_t blk_off, chunk; int pos; };       // where gene k lives: operand-tile block + in-row bytes, swizzle chunk, position
+    auto gene_slot = [&](int k) {
+        const int pos = tc_position(sink.family, sink.d, sink.F, k / Bterms, k % Bterms);
+        return GeneSlot{(uint32_t)(nres + (pos >> 6)) * PERS_KB_BYTES + ((uint32_t)pos & 7u) * 2u, ((uint32_t)pos & 63u) >> 3, pos};
+    };
+    auto store_gene = [&](const GeneSlot &g, float *pop_dst_s, float *pop_dst_g, int p, int k, float gene) {   // pop_dst_g: global mirror (or null)
+        pop_dst_s[p * K + k] = gene;
+        const float v = fabsf(gene) <= 65504.f ? gene * sink.scale : __int_as_float(0x7fc00000);
+        uint8_t *blk = gbase + g.blk_off + (uint32_t)p * 128u + ((g.chunk ^ ((uint32_t)p & 7u)) << 4);
+        const __half hi = __float2half_rn(v);
+        const __half lo = __float2half_rn(v - __half2float(hi));
+        *reinterpret_cast<__half *>(blk) = hi;
+        if (a.split) *reinterpret_cast<__half *>(blk + (size_t)kb1 * PERS_KB_BYTES) = lo;
+        if (pop_dst_g) {                                 // what c16_store would have written
+            pop_dst_g[(long long)p * K + k] = gene;
+            if (!a.split) sink.ptr[(long long)p * sink.Kpad + g.pos] = hi;
+            else { __half *row = sink.ptr + (long long)p * 3 * sink.Kpad; row[g.pos] = hi; row[sink.Kpad + g.pos] = lo; row[2 * sink.Kpad + g.pos] = hi; }
+        }
+    };
+    auto put_gene = [&](float *pop_dst_s, float *pop_dst_g, int p, int k, float gene) { store_gene(gene_slot(k), pop_dst_s, pop_dst_g, p, k, gene); };
+    if (a.local) {
+        uint4 *at = reinterpret_cast<uint4 *>(gbase + (size_t)nres * PERS_KB_BYTES);
+        for (int i = tid; i < nres * PERS_KB_BYTES / 16; i += PERS_THREADS) at[i] = make_uint4(0u, 0u, 0u, 0u);   // rows >= P, padding positions
+        __syncthreads();
+        for (int i = tid; i < P * K; i += PERS_THREADS) put_gene(pop_s0, nullptr, i / K, i % K, __ldcg(a.pop_a + i));   // (global memory already holds both)
+        fence_proxy_async();               // generic-proxy stores of the operand tile -> the tensor core's async-proxy reads
+        __syncthreads();
+    }
+    float *pop_cur_s = pop_s0, *pop_next_s = pop_s1;
+
     unsigned int bar_target = 0;
     uint32_t sph = 0;                                    // staging barrier phase
     int applied = 0, evals = 0, stopped = 0;
@@ -134,9 +192,12 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
     float *pop_next = a.pop_b;
 
     for (int e = 0;; ++e) {
+        // local mode has one grid barrier per generation: the tile sums alternate between two buffers (see the header)
+        float *partial_e = a.partial + (a.local && (e & 1) ? (long long)a.n_tiles * a.Ppad : 0);
+        PTRACE(0);
         // ================= phase A: this CTA's tile of the fused fitness =================
         if (warp == 0) {
-            if (lane == 0) {
+            if (lane == 0 && !a.local) {
                 fence_proxy_async_all();                 // the genes were written by other CTAs' generic stores (phase C)
                 mbar_expect_tx(afull_bar, (uint32_t)(nres * PERS_KB_BYTES));
                 for (int j = 0; j < nres; ++j)           // split: ranges 0 (hi) and 1 (lo); range 2 repeats range 0
@@ -146,12 +207,12 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
             if (lane == 0) {
                 constexpr uint32_t idesc = make_idesc(BM, PERS_TILE_N);
                 if (e == 0) mbar_wait(bfull_bar, 0);
-                mbar_wait(afull_bar, (uint32_t)(e & 1));
+                if (!a.local) mbar_wait(afull_bar, (uint32_t)(e & 1));      // (local mode: the tile was written before the CTA barrier)
                 tc_fence_after();
                 for (int kb = 0; kb < k_blocks; ++kb) {  // the launch path's k order, whatever block the data sits in
                     const int ja = kb < nres ? kb : kb - nres, jb = kb < kb1 ? kb : kb - kb1;
                     const uint64_t adesc = make_smem_desc(baseA + ja * PERS_KB_BYTES), bdesc = make_smem_desc(baseB + jb * PERS_KB_BYTES);
-                    const int nk = kb + 1 == k_blocks ? a.k_last : BKB / UMMA_K;
+                    const int nk = (kb + 1) % kb1 == 0 ? a.k_last : BKB / UMMA_K;     // the last block of each K range ends in padding
 #pragma unroll
                     for (int k = 0; k < BKB / UMMA_K; ++k)
                         if (k < nk) umma_f16<1>(tmem_base, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
@@ -177,10 +238,12 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
                 epilogue_chunk<ACT, TMSE>(cur, tgt_s + 32 * c, a.R, acc2);
             }
             tc_fence_before();                           // the next generation's MMAs overwrite the accumulator after the barrier
-            a.partial[(long long)n_tile * a.Ppad + m_blk * BM + quarter * 32 + lane] =
+            partial_e[(long long)n_tile * a.Ppad + m_blk * BM + quarter * 32 + lane] =
                 ((acc2[0].x + acc2[0].y) + (acc2[1].x + acc2[1].y)) + ((acc2[2].x + acc2[2].y) + (acc2[3].x + acc2[3].y));
         }
+        PTRACE(1);
         grid_barrier(a.gbar, bar_target);
+        PTRACE(2);
         ++evals;
 
         // ================= phase B: a5 tail, a6 rank, a7 stop test =================
@@ -188,9 +251,10 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
         // once (the population tile's area is idle between the phases and serves as the staging buffer) -- so the reduction
         // costs ONE L2 round trip instead of one per addend.
         {
-            float *stage = reinterpret_cast<float *>(gbase + nres * PERS_KB_BYTES);
+            float *stage = a.local ? stage_local : reinterpret_cast<float *>(gbase + nres * PERS_KB_BYTES);
+            const uint32_t stage_addr = a.local ? smem_u32(stage_local) : baseA;
             const int P4 = (P + 3) & ~3;
-            const int cp = min(P4, (nres * PERS_KB_BYTES / 4 / a.n_tiles) & ~3);      // chromosomes per pass (n_tiles <= 148: >= 24)
+            const int cp = a.local ? P4 : min(P4, (nres * PERS_KB_BYTES / 4 / a.n_tiles) & ~3);      // chromosomes per pass (n_tiles <= 148: >= 24)
             for (int p0 = 0; p0 < P; p0 += cp) {
                 const int np4 = min(cp, P4 - p0);                                     // a multiple of 4: 16-byte rows
                 if (a.n_tiles * np4 <= 8 * PERS_THREADS) {
@@ -199,7 +263,7 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
 #pragma unroll
                     for (int u = 0; u < 8; ++u) {
                         const int i = u * PERS_THREADS + tid, ch = i / np4, pp = i - ch * np4;
-                        v[u] = i < a.n_tiles * np4 ? __ldcg(a.partial + (long long)ch * a.Ppad + p0 + pp) : 0.f;
+                        v[u] = i < a.n_tiles * np4 ? __ldcg(partial_e + (long long)ch * a.Ppad + p0 + pp) : 0.f;
                     }
 #pragma unroll
                     for (int u = 0; u < 8; ++u)
@@ -210,7 +274,7 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
                         fence_proxy_async_all();       // other CTAs' generic stores -> this thread's async-proxy reads
                         mbar_expect_tx(sfull_bar, (uint32_t)(a.n_tiles * np4 * 4));
                         for (int ch = 0; ch < a.n_tiles; ++ch)
-                            bulk_load(baseA + (uint32_t)(ch * np4 * 4), a.partial + (long long)ch * a.Ppad + p0, (uint32_t)(np4 * 4), sfull_bar);
+                            bulk_load(stage_addr + (uint32_t)(ch * np4 * 4), partial_e + (long long)ch * a.Ppad + p0, (uint32_t)(np4 * 4), sfull_bar);
                     }
                     mbar_wait(sfull_bar, sph);
                     sph ^= 1;
@@ -268,6 +332,7 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
             grid_barrier(a.gbar, bar_target);
             best_p = __ldcg(&a.state->best_index);
         }
+        PTRACE(3);
         best_f = fit_s[best_p];                          // every CTA holds every fitness: the same bits everywhere
         if (a.stop_error >= 0.0f && best_f <= a.stop_error) stopped = 1;
         if (stopped || e == a.generations) break;
@@ -275,6 +340,69 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
         // ================= phase C: a8-a11 for this CTA's share of the elites and child pairs =================
         const uint32_t gen = a.step.gen + (uint32_t)e;
         const int n_items = a.step.e + a.step.npairs;
+        if (a.local) {
+            // every CTA builds the whole next population from its own copy.  Step 1: one thread per child pair and parent draws
+            // the pair's decisions (a9 tournament, a10 cut point); step 2: one (item, gene) per thread and turn, so a thread
+            // walks n_items K / 512 genes with two Philox calls each.  Nothing goes to global memory inside the loop: the final
+            // population is written out once, after the last evaluation.
+            int *dec_s = reinterpret_cast<int *>(stage_local);            // [3][npairs]: parents A, B, crossover word (staging area is idle)
+            const int npairs = a.step.npairs;
+            if (tid < 3 * npairs) {
+                const int q = tid % npairs, what = tid / npairs;
+                int mine;
+                if (what < 2) {                          // a9 tournament by rank (R3): t rank draws, the best wins
+                    uint32_t best = 0xFFFFFFFFu;
+                    W4 w{0, 0, 0, 0};
+                    for (int j = 0; j < a.step.tsize; ++j) {
+                        if ((j & 3) == 0) w = draw(a.step.seed, (uint32_t)(j >> 2), (uint32_t)(2 * q + what), gen, TAG_SELECT);
+                        const uint32_t word = (j & 3) == 0 ? w.x : (j & 3) == 1 ? w.y : (j & 3) == 2 ? w.z : w.w;
+                        best = min(best, idx_of(word, (uint32_t)P));
+                    }
+                    mine = order_s[(int)best];
+                } else {                                 // a10 decision (R5): bit 30 = apply, low bits = cut point
+                    W4 w = draw(a.step.seed, 0u, (uint32_t)q, gen, TAG_XOVER);
+                    const int doit = (K >= 2) && hit(w.x, a.step.pc);
+                    mine = (doit << 30) | (K >= 2 ? 1 + (int)idx_of(w.y, (uint32_t)(K - 1)) : 0);
+                }
+                dec_s[what * npairs + q] = mine;
+            }
+            __syncthreads();
+            // a thread keeps ONE gene index (its slot in the operand tile is computed once) and walks the items; genes beyond
+            // 128 per chromosome take further turns
+            const int kt = tid & 127;
+            for (int k = kt; k < K; k += 128) {
+              const GeneSlot gs = gene_slot(k);
+              float *const mirror = nullptr;
+              for (int item = tid >> 7; item < n_items; item += PERS_THREADS / 128) {
+                if (item < a.step.e) {                   // a8 elitism (L148, L291; DESIGN G17)
+                    const int src = a.step.elite_mode == GAME_ELITE_TOP_E ? order_s[item] : order_s[0];
+                    store_gene(gs, pop_next_s, mirror, item, k, pop_cur_s[src * K + k]);
+                    continue;
+                }
+                const int q = item - a.step.e;
+                const int sA = a.step.e + 2 * q, sB = sA + 1;
+                const int pa = dec_s[q], pb = dec_s[npairs + q], xo = dec_s[2 * npairs + q];
+                const int doit = xo >> 30, cut = xo & 0x3fffffff;
+                const float ga = pop_cur_s[pa * K + k], gb = pop_cur_s[pb * K + k];
+                const bool head = doit ? (k < cut) : true;
+                float cA = head ? ga : gb, cB = head ? gb : ga;      // A = pa[0:c] | pb[c:K], B = pb[0:c] | pa[c:K]
+                const W4 w = draw(a.step.seed, (uint32_t)k, (uint32_t)sA, gen, TAG_MUTATE);       // a11 (R6)
+                const W4 v = draw(a.step.seed, (uint32_t)k, (uint32_t)sB, gen, TAG_MUTATE);
+                if (hit(w.x, a.step.pm)) cA = upm1(w.y);
+                if (hit(v.x, a.step.pm)) cB = upm1(v.y);
+                store_gene(gs, pop_next_s, mirror, sA, k, cA);
+                if (sB < P) store_gene(gs, pop_next_s, mirror, sB, k, cB);
+              }
+            }
+            ++applied;
+            PTRACE(4);
+            fence_proxy_async();                         // the operand tile just written is read by the tensor core next
+            __syncthreads();
+            PTRACE(5);
+            { float *t = pop_cur_s; pop_cur_s = pop_next_s; pop_next_s = t; }
+            const float *t = pop_cur; pop_cur = pop_next; pop_next = const_cast<float *>(t);
+            continue;
+        }
         // one WARP per item, so the items of a CTA (and their dependent order -> parent -> gene loads) are all in flight at once
         for (int item = blockIdx.x + warp * gridDim.x; item < n_items; item += gridDim.x * (PERS_THREADS / 32)) {
             auto rank_to_index = [&](int r) { return local_rank ? order_s[r] : __ldcg(a.order + r); };
@@ -326,11 +454,23 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
             }
         }
         ++applied;
+        PTRACE(4);
         fence_proxy_async_all();                         // the fp16 genes just stored are read by TMA (async proxy) next
         grid_barrier(a.gbar, bar_target);
+        PTRACE(5);
         const float *t = pop_cur; pop_cur = pop_next; pop_next = const_cast<float *>(t);
     }
 
+    if (a.local) {
+        // the population the loop ended on (this CTA's copy is everyone's) goes to the buffer the launch path would have left
+        // it in, with its fp16 copy; the CTAs share the writing
+        float *out = const_cast<float *>(pop_cur);
+        for (int i = blockIdx.x * PERS_THREADS + tid; i < P * K; i += gridDim.x * PERS_THREADS) {
+            const float gene = pop_cur_s[i];
+            out[i] = gene;
+            c16_store(sink, i / K, i % K, gene);
+        }
+    }
     if (blockIdx.x == 0 && tid == 0) {
         a.state->stopped = stopped;
         a.state->stop_request = stopped;
@@ -345,10 +485,22 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
 }
 
 
+// local-population mode (see the header): one chromosome block and few enough genes for every CTA to rebuild them all.
+// GAME_TUNE_PERSISTENT = 2 keeps the shared-population form, for measurement.
+static bool persistent_local(const game_ctx *c, int P)
+{
+    return c->tune[GAME_TUNE_PERSISTENT] != 2 && P <= BM && (long long)P * c->K <= PERS_LOCAL_GENES;
+}
+
 static size_t persistent_smem_bytes(const game_ctx *c, int path, int P)
 {
     const int kb1 = c->Kpad / BKB, nres = path == GAME_PATH_TENSOR_SPLIT ? 2 * kb1 : kb1;
-    return (size_t)2 * nres * PERS_KB_BYTES + 1024 + 128 + 512 + (size_t)P * 16 + 64;
+    size_t bytes = (size_t)2 * nres * PERS_KB_BYTES + 1024 + 128 + 512 + (size_t)P * 16 + 64;
+    if (persistent_local(c, P)) {
+        const size_t n_tiles = (size_t)((c->N + PERS_TILE_N - 1) / PERS_TILE_N);
+        bytes += 16 + 2 * (((size_t)P * c->K + 3) & ~(size_t)3) * 4 + (n_tiles < 2 ? 2 : n_tiles) * ((P + 3) & ~3) * 4;   // (the staging area also holds phase C's 3 P / 2 decisions)
+    }
+    return bytes;
 }
 
 // can game_evolve run this population / dataset through the persistent kernel?
@@ -405,9 +557,18 @@ int launch_evolve_persistent(game_ctx *c, const game_ga_params *gp, unsigned lon
     a.k_blocks = (split ? 3 : 1) * c->Kpad / BKB;
     a.kb1 = c->Kpad / BKB; a.split = split ? 1 : 0;
     const int npos = tc_num_positions(c->family, c->degree, c->F, c->K);
-    a.k_last = split ? BKB / UMMA_K : (npos - (c->Kpad - BKB) + UMMA_K - 1) / UMMA_K;
+    a.k_last = (npos - (c->Kpad - BKB) + UMMA_K - 1) / UMMA_K;      // real k-steps in the last k-block of a K range (split: three ranges)
     a.P = P; a.Ppad = ((P + 255) / 256) * 256; a.generations = generations; a.err = c->err;
     a.N = c->N; a.tgt = c->t; a.R = c->R; a.stop_error = gp->stop_error;
+    a.local = persistent_local(c, P) ? 1 : 0;
+    if (a.local) {                              // two buffers of tile sums (one grid barrier per generation)
+        const size_t need = (size_t)2 * a.n_tiles * a.Ppad;
+        if (need > c->partial_cap) {
+            if (c->partial) { cudaFree(c->partial); c->partial = nullptr; c->partial_cap = 0; }
+            GAME_CUDA(c, cudaMalloc(&c->partial, need * sizeof(float)));
+            c->partial_cap = need;
+        }
+    }
     a.partial = c->partial; a.fit = c->fit; a.order = c->order;
     a.pop_a = c->pop; a.pop_b = c->pop_next;
     a.state = c->state; a.gbar = c->gbar;

@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(SRC == SRC_GEN ? GEN_THREADS : 64 + 32 * EW, 1
 fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmE,
                   int n_tiles, int m_blocks, int k_blocks, long long N, const float *__restrict__ tgt, float R,
                   float *__restrict__ partial, int Ppad, const DevState *state,
-                  const float *__restrict__ X, int F, int degree, int k_last)
+                  const float *__restrict__ X, int F, int degree, int k_last, int kb_range)
 {
     using C = Cfg<CG>;
     static_assert(SRC == SRC_TMA || CG == 2, "the generator variant runs as CTA pairs");
@@ -342,7 +342,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                         const uint32_t sb = RESIDENT_A ? base + k_blocks * A_BYTES + s * GEN_B_BYTES : sa + A_BYTES;
                         const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sb);
                         const bool last = kb + 1 == k_blocks;
-                        const int nk = last ? k_last : BKB / UMMA_K;
+                        const int nk = (kb + 1) % kb_range == 0 ? k_last : BKB / UMMA_K;      // padding steps would multiply zeros
                         if (elect_one()) {
     #pragma unroll
                             for (int k = 0; k < BKB / UMMA_K; ++k) {
@@ -674,10 +674,11 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     using C = Cfg<CG>;
     auto kern = fitness_tc_kernel<CG, ACT, TMSE, EW, SRC, FAMILY, TEAMS, BNT, SHARE>;
     const int k_blocks = (split ? 3 : 1) * ctx->Kpad / BKB;
-    // real terms in the last k-block, in UMMA k-steps of 16 (the split form's three K ranges each end in the same padding,
-    // so only the one-pass form trims; the generator variant writes whole k-blocks and is left alone too)
+    // real terms in the last k-block of a K range, in UMMA k-steps of 16 (the split form has three ranges that end in the same
+    // padding; the generator variant writes whole k-blocks and is left alone)
     const int npos = tc_num_positions(ctx->family, ctx->degree, ctx->F, ctx->K);
-    const int k_last = (split || SRC == SRC_GEN) ? BKB / UMMA_K : (npos - (ctx->Kpad - BKB) + UMMA_K - 1) / UMMA_K;
+    const int k_last = SRC == SRC_GEN ? BKB / UMMA_K : (npos - (ctx->Kpad - BKB) + UMMA_K - 1) / UMMA_K;
+    const int kb_range = ctx->Kpad / BKB;                    // k-blocks per K range
     const CUtensorMap *maps_E = (const CUtensorMap *)(split ? ctx->tmap_Es : ctx->tmap_E);
     const int smem = SRC != SRC_TMA ? k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES
                    : BNT == BN    ? C::SMEM
@@ -700,7 +701,7 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     KernelTimer timer(ctx);
     GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, maps_E[BNT / CG == 128 ? 1 : 0], n_tiles,
                                       m_blocks, k_blocks, ctx->N, (const float *)ctx->t, ctx->R, ctx->partial, Ppad, state,
-                                      (const float *)ctx->X, ctx->F, ctx->degree, k_last));
+                                      (const float *)ctx->X, ctx->F, ctx->degree, k_last, kb_range));
     return GAME_OK;
 }
 

@@ -322,7 +322,7 @@ int game_set_tuning(game_ctx *c, int knob, int value)
 {
     if (!c) return GAME_ERR_INVALID_ARG;
     if (knob < 0 || knob >= GAME_TUNE_COUNT_) return fail(c, GAME_ERR_INVALID_ARG, "game_set_tuning: unknown knob");
-    static const int lo[GAME_TUNE_COUNT_] = {0, 1, 0, 0, 0, 0, 0, 0}, hi[GAME_TUNE_COUNT_] = {1, 2, 2, 1, 1, 1, 1, 8};
+    static const int lo[GAME_TUNE_COUNT_] = {0, 1, 0, 0, 0, 0, 0, 0}, hi[GAME_TUNE_COUNT_] = {1, 2, 2, 1, 1, 1, 2, 8};
     if (value != -1 && (value < lo[knob] || value > hi[knob] || (knob == GAME_TUNE_SIGMOID && value == 1)))
         return fail(c, GAME_ERR_INVALID_ARG, "game_set_tuning: value out of range for this knob");
     c->tune[knob] = value;
