@@ -36,6 +36,7 @@ extern "C" int game_ptrace_read(long long *buf) { cudaDeviceSynchronize(); retur
 #define PTRACE(slot) do { } while (0)
 #endif
 namespace game {
+constexpr int PERS_TMEM_COLS = 128;
 
 constexpr int PERS_THREADS = 512;       // warp 0 TMA producer, warp 1 MMA issuer, warps 2-5 epilogue; all 8 warps in phases B, C
 constexpr int PERS_TILE_N = 128;        // patterns per tile: the half-size tiles the launch path uses below one wave
@@ -125,7 +126,7 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmC) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmE) : "memory");
     }
-    if (warp == 1) tmem_alloc<1>(tmem_slot, 128);
+    if (warp == 1) tmem_alloc<1>(tmem_slot, PERS_TMEM_COLS);
     // the tile's targets, staged once: t - tbias, and for a padding pattern the value that makes its residual exactly zero
     // (its expansion row is zero, so z = 0) -- the launch path's rule (fitness_tc_kernel, team epilogue)
     constexpr float tbias = ACT == MODE_SIG_TANH32 ? 0.5f : 0.f;
@@ -204,20 +205,22 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
                     tma_load_2d<1>(baseA + j * PERS_KB_BYTES, &tmC, j * BKB, m_blk * BM, afull_bar);
             }
         } else if (warp == 1) {
-            if (lane == 0) {
-                constexpr uint32_t idesc = make_idesc(BM, PERS_TILE_N);
-                if (e == 0) mbar_wait(bfull_bar, 0);
-                if (!a.local) mbar_wait(afull_bar, (uint32_t)(e & 1));      // (local mode: the tile was written before the CTA barrier)
-                tc_fence_after();
-                for (int kb = 0; kb < k_blocks; ++kb) {  // the launch path's k order, whatever block the data sits in
-                    const int ja = kb < nres ? kb : kb - nres, jb = kb < kb1 ? kb : kb - kb1;
-                    const uint64_t adesc = make_smem_desc(baseA + ja * PERS_KB_BYTES), bdesc = make_smem_desc(baseB + jb * PERS_KB_BYTES);
-                    const int nk = (kb + 1) % kb1 == 0 ? a.k_last : BKB / UMMA_K;     // the last block of each K range ends in padding
+            // the whole warp walks the loop (descriptors stay warp-uniform), one elected lane issues -- see fitness_tc.cu
+            constexpr uint32_t idesc = make_idesc(BM, PERS_TILE_N);
+            if (e == 0) mbar_wait(bfull_bar, 0);
+            if (!a.local) mbar_wait(afull_bar, (uint32_t)(e & 1));      // (local mode: the tile was written before the CTA barrier)
+            tc_fence_after();
+            for (int kb = 0; kb < k_blocks; ++kb) {      // the launch path's k order, whatever block the data sits in
+                const int ja = kb < nres ? kb : kb - nres, jb = kb < kb1 ? kb : kb - kb1;
+                const uint64_t adesc = make_smem_desc(baseA + ja * PERS_KB_BYTES), bdesc = make_smem_desc(baseB + jb * PERS_KB_BYTES);
+                const int nk = (kb + 1) % kb1 == 0 ? a.k_last : BKB / UMMA_K;     // the last block of each K range ends in padding
+                if (elect_one()) {
 #pragma unroll
                     for (int k = 0; k < BKB / UMMA_K; ++k)
                         if (k < nk) umma_f16<1>(tmem_base, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (kb | k) != 0);
+                    if (kb + 1 == k_blocks) umma_commit<1>(tfull_bar);
                 }
-                umma_commit<1>(tfull_bar);
+                __syncwarp();
             }
         } else if (warp < 6) {
             // one thread per chromosome walks the tile's 128 pattern columns in four 32-column chunks, the TMEM load of the
@@ -403,53 +406,64 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
             const float *t = pop_cur; pop_cur = pop_next; pop_next = const_cast<float *>(t);
             continue;
         }
-        // one WARP per item, so the items of a CTA (and their dependent order -> parent -> gene loads) are all in flight at once
-        for (int item = blockIdx.x + warp * gridDim.x; item < n_items; item += gridDim.x * (PERS_THREADS / 32)) {
+        // This CTA's share of the items (item = blockIdx.x + j gridDim.x), in two steps like the local form.  Step 1: one thread
+        // per item and decision (elite source; the pair's two parents by a9 tournament; its a10 cut point), so the dependent
+        // rank -> index loads of all of them are in flight at once.  Step 2: one (item, gene) per thread and turn: the parents'
+        // genes, two Philox calls, the children and their fp16 copies -- a gene per thread instead of a warp per pair.
+        {
+            const int nj = blockIdx.x < n_items ? (n_items - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+            int *dec_s = reinterpret_cast<int *>(gbase + nres * PERS_KB_BYTES);          // [3][nj] (the population tile's area is idle)
             auto rank_to_index = [&](int r) { return local_rank ? order_s[r] : __ldcg(a.order + r); };
-            if (item < a.step.e) {                       // a8 elitism (L148, L291; DESIGN G17)
-                const int src = a.step.elite_mode == GAME_ELITE_TOP_E ? rank_to_index(item) : rank_to_index(0);
-                for (int k = lane; k < K; k += 32) {
-                    const float v = __ldcg(pop_cur + (long long)src * K + k);
-                    pop_next[(long long)item * K + k] = v;
-                    if (a.step.sink.ptr) c16_store(a.step.sink, item, k, v);
+            for (int u = tid; u < 3 * nj; u += PERS_THREADS) {
+                const int j = u % nj, what = u / nj, item = blockIdx.x + j * gridDim.x;
+                int mine = 0;
+                if (item < a.step.e) {                   // a8 elitism (L148, L291; DESIGN G17)
+                    if (what == 0) mine = a.step.elite_mode == GAME_ELITE_TOP_E ? rank_to_index(item) : rank_to_index(0);
+                } else if (what < 2) {                   // a9 tournament by rank (R3): t rank draws, the best wins
+                    const int q = item - a.step.e;
+                    uint32_t best = 0xFFFFFFFFu;
+                    W4 w{0, 0, 0, 0};
+                    for (int i = 0; i < a.step.tsize; ++i) {
+                        if ((i & 3) == 0) w = draw(a.step.seed, (uint32_t)(i >> 2), (uint32_t)(2 * q + what), gen, TAG_SELECT);
+                        const uint32_t word = (i & 3) == 0 ? w.x : (i & 3) == 1 ? w.y : (i & 3) == 2 ? w.z : w.w;
+                        best = min(best, idx_of(word, (uint32_t)P));
+                    }
+                    mine = rank_to_index((int)best);
+                } else {                                 // a10 decision (R5): bit 30 = apply, low bits = cut point
+                    W4 w = draw(a.step.seed, 0u, (uint32_t)(item - a.step.e), gen, TAG_XOVER);
+                    const int doit = (K >= 2) && hit(w.x, a.step.pc);
+                    mine = (doit << 30) | (K >= 2 ? 1 + (int)idx_of(w.y, (uint32_t)(K - 1)) : 0);
                 }
-                continue;
+                dec_s[what * nj + j] = mine;
             }
-            const int q = item - a.step.e;
-            const int sA = a.step.e + 2 * q, sB = sA + 1;
-            int mine = 0;
-            if (lane < 2) {                              // a9 tournament by rank (R3): t rank draws, the best wins
-                uint32_t best = 0xFFFFFFFFu;
-                W4 w{0, 0, 0, 0};
-                for (int j = 0; j < a.step.tsize; ++j) {
-                    if ((j & 3) == 0) w = draw(a.step.seed, (uint32_t)(j >> 2), (uint32_t)(2 * q + lane), gen, TAG_SELECT);
-                    const uint32_t word = (j & 3) == 0 ? w.x : (j & 3) == 1 ? w.y : (j & 3) == 2 ? w.z : w.w;
-                    best = min(best, idx_of(word, (uint32_t)P));
-                }
-                mine = rank_to_index((int)best);
-            } else if (lane == 2) {                      // a10 decision (R5): bit 31 = apply, low bits = cut point
-                W4 w = draw(a.step.seed, 0u, (uint32_t)q, gen, TAG_XOVER);
-                const int doit = (K >= 2) && hit(w.x, a.step.pc);
-                mine = (doit << 30) | (K >= 2 ? 1 + (int)idx_of(w.y, (uint32_t)(K - 1)) : 0);
-            }
-            const int pa = __shfl_sync(0xffffffffu, mine, 0), pb = __shfl_sync(0xffffffffu, mine, 1);
-            const int xo = __shfl_sync(0xffffffffu, mine, 2);
-            const int doit = xo >> 30, cut = xo & 0x3fffffff;
-            const float *ra = pop_cur + (long long)pa * K, *rb = pop_cur + (long long)pb * K;
-            for (int k = lane; k < K; k += 32) {
-                const float ga = __ldcg(ra + k), gb = __ldcg(rb + k);
-                const bool head = doit ? (k < cut) : true;
-                float cA = head ? ga : gb;               // A = pa[0:c] | pb[c:K]
-                float cB = head ? gb : ga;               // B = pb[0:c] | pa[c:K]
-                W4 w = draw(a.step.seed, (uint32_t)k, (uint32_t)sA, gen, TAG_MUTATE);       // a11 (R6)
-                if (hit(w.x, a.step.pm)) cA = upm1(w.y);
-                pop_next[(long long)sA * K + k] = cA;
-                if (a.step.sink.ptr) c16_store(a.step.sink, sA, k, cA);
-                if (sB < P) {
-                    W4 v = draw(a.step.seed, (uint32_t)k, (uint32_t)sB, gen, TAG_MUTATE);
+            __syncthreads();
+            for (int k = tid & 127; k < K; k += 128) {
+                for (int j = tid >> 7; j < nj; j += PERS_THREADS / 128) {
+                    const int item = blockIdx.x + j * gridDim.x;
+                    if (item < a.step.e) {
+                        const float v = __ldcg(pop_cur + (long long)dec_s[j] * K + k);
+                        pop_next[(long long)item * K + k] = v;
+                        if (a.step.sink.ptr) c16_store(a.step.sink, item, k, v);
+                        continue;
+                    }
+                    const int q = item - a.step.e;
+                    const int sA = a.step.e + 2 * q, sB = sA + 1;
+                    const int pa = dec_s[j], pb = dec_s[nj + j], xo = dec_s[2 * nj + j];
+                    const int doit = xo >> 30, cut = xo & 0x3fffffff;
+                    const float ga = __ldcg(pop_cur + (long long)pa * K + k), gb = __ldcg(pop_cur + (long long)pb * K + k);
+                    const bool head = doit ? (k < cut) : true;
+                    float cA = head ? ga : gb;           // A = pa[0:c] | pb[c:K]
+                    float cB = head ? gb : ga;           // B = pb[0:c] | pa[c:K]
+                    const W4 w = draw(a.step.seed, (uint32_t)k, (uint32_t)sA, gen, TAG_MUTATE);       // a11 (R6)
+                    const W4 v = draw(a.step.seed, (uint32_t)k, (uint32_t)sB, gen, TAG_MUTATE);
+                    if (hit(w.x, a.step.pm)) cA = upm1(w.y);
                     if (hit(v.x, a.step.pm)) cB = upm1(v.y);
-                    pop_next[(long long)sB * K + k] = cB;
-                    if (a.step.sink.ptr) c16_store(a.step.sink, sB, k, cB);
+                    pop_next[(long long)sA * K + k] = cA;
+                    if (a.step.sink.ptr) c16_store(a.step.sink, sA, k, cA);
+                    if (sB < P) {
+                        pop_next[(long long)sB * K + k] = cB;
+                        if (a.step.sink.ptr) c16_store(a.step.sink, sB, k, cB);
+                    }
                 }
             }
         }
@@ -481,7 +495,7 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 1) { __syncwarp(); tc_fence_after(); tmem_dealloc<1>(tmem_base, 128); }
+    if (warp == 1) { __syncwarp(); tc_fence_after(); tmem_dealloc<1>(tmem_base, PERS_TMEM_COLS); }
 }
 
 
