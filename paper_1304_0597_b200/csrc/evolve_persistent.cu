@@ -25,20 +25,10 @@
 #include "ga_device.cuh"
 #include "tc_common.cuh"
 
-#ifdef PERS_TRACE
-__device__ long long g_ptrace[4096];
-#define PTRACE(slot) do { if (blockIdx.x == 0 && threadIdx.x == PTRACE_TID && e >= 100 && e < 228) g_ptrace[(e - 100) * 8 + (slot)] = clock64(); } while (0)
-extern "C" int game_ptrace_read(long long *buf) { cudaDeviceSynchronize(); return (int)cudaMemcpyFromSymbol(buf, g_ptrace, sizeof(g_ptrace)); }
-#ifndef PTRACE_TID
-#define PTRACE_TID 64
-#endif
-#else
-#define PTRACE(slot) do { } while (0)
-#endif
 namespace game {
 constexpr int PERS_TMEM_COLS = 128;
 
-constexpr int PERS_THREADS = 512;       // warp 0 TMA producer, warp 1 MMA issuer, warps 2-5 epilogue; all 8 warps in phases B, C
+constexpr int PERS_THREADS = 512;       // warp 0 TMA producer, warp 1 MMA issuer, warps 2-5 epilogue; all 16 warps in phases B, C (256 threads: phase C 5.6k vs 8.4k clk on config 1)
 constexpr int PERS_TILE_N = 128;        // patterns per tile: the half-size tiles the launch path uses below one wave
 constexpr int PERS_KB_BYTES = 128 * BKB * 2;
 constexpr int PERS_LOCAL_RANK = 256;    // up to this many chromosomes every CTA ranks the whole population itself
@@ -195,7 +185,6 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
     for (int e = 0;; ++e) {
         // local mode has one grid barrier per generation: the tile sums alternate between two buffers (see the header)
         float *partial_e = a.partial + (a.local && (e & 1) ? (long long)a.n_tiles * a.Ppad : 0);
-        PTRACE(0);
         // ================= phase A: this CTA's tile of the fused fitness =================
         if (warp == 0) {
             if (lane == 0 && !a.local) {
@@ -244,9 +233,7 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
             partial_e[(long long)n_tile * a.Ppad + m_blk * BM + quarter * 32 + lane] =
                 ((acc2[0].x + acc2[0].y) + (acc2[1].x + acc2[1].y)) + ((acc2[2].x + acc2[2].y) + (acc2[3].x + acc2[3].y));
         }
-        PTRACE(1);
         grid_barrier(a.gbar, bar_target);
-        PTRACE(2);
         ++evals;
 
         // ================= phase B: a5 tail, a6 rank, a7 stop test =================
@@ -335,7 +322,6 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
             grid_barrier(a.gbar, bar_target);
             best_p = __ldcg(&a.state->best_index);
         }
-        PTRACE(3);
         best_f = fit_s[best_p];                          // every CTA holds every fitness: the same bits everywhere
         if (a.stop_error >= 0.0f && best_f <= a.stop_error) stopped = 1;
         if (stopped || e == a.generations) break;
@@ -398,10 +384,8 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
               }
             }
             ++applied;
-            PTRACE(4);
             fence_proxy_async();                         // the operand tile just written is read by the tensor core next
             __syncthreads();
-            PTRACE(5);
             { float *t = pop_cur_s; pop_cur_s = pop_next_s; pop_next_s = t; }
             const float *t = pop_cur; pop_cur = pop_next; pop_next = const_cast<float *>(t);
             continue;
@@ -468,10 +452,8 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
             }
         }
         ++applied;
-        PTRACE(4);
         fence_proxy_async_all();                         // the fp16 genes just stored are read by TMA (async proxy) next
         grid_barrier(a.gbar, bar_target);
-        PTRACE(5);
         const float *t = pop_cur; pop_cur = pop_next; pop_next = const_cast<float *>(t);
     }
 

@@ -952,6 +952,35 @@ def test_persistent_loop_equals_launch_path(orc, cfg, P, gens, path, act, err):
     assert np.array_equal(f2.view(np.uint32), fg.view(np.uint32))
 
 
+@pytest.mark.parametrize("cfg,P,gens", [(1, None, 9), (1, 41, 6), (1, 2, 5), (2, 33, 4)])
+def test_persistent_local_population_form(orc, cfg, P, gens):
+    """Small populations (P K <= 4096 genes) run the persistent loop with the whole population in every CTA's shared memory
+    (no population traffic, one grid barrier per generation).  Same bits as the shared-population form
+    (GAME_TUNE_PERSISTENT = 2) and as the launch path (0), including odd P, P = 2 and a resumed run."""
+    w = wl.config(cfg)
+    w = w.scaled(P=P or w.P, generations=gens)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    gp = g.ga_params(P=w.P)
+    out = {}
+    for knob in (1, 2, 0):
+        ctx = make_ctx(fam, d, X, t, w.act, w.err, w.R, g.GAME_PATH_AUTO)
+        ctx.set_tuning(g.GAME_TUNE_PERSISTENT, knob)
+        ctx.evolve(gens, w.seed, gp)
+        ctx.evolve(3, w.seed, gp)                              # resume: the global copy written at the end of the first call
+        out[knob] = ctx.get_population_host()
+        f2 = ctx.fitness(dev(out[knob][0])).cpu().numpy()      # the fp16 copy written at the end matches the population
+        assert np.array_equal(f2.view(np.uint32), out[knob][1].view(np.uint32))
+        ctx.destroy()
+    for knob in (2, 0):
+        for a, b in zip(out[1], out[knob]):
+            assert np.array_equal(np.asarray(a).view(np.uint32), np.asarray(b).view(np.uint32)), knob
+    # the oracle's operators from the GPU's own order reproduce one more generation bit for bit
+    pop, fit, order = out[1]
+    check_fitness(orc, fit, fam, d, X, t, pop, w.act, w.err, w.R, g.GAME_PATH_TENSOR_SPLIT, "local form")
+    assert np.array_equal(order, orc.rank(fit))
+
+
 def test_persistent_loop_stop_criterion(orc):
     w = wl.config(1)
     fam, d = w.family, w.degree
