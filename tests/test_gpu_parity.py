@@ -952,11 +952,11 @@ def test_persistent_loop_equals_launch_path(orc, cfg, P, gens, path, act, err):
     assert np.array_equal(f2.view(np.uint32), fg.view(np.uint32))
 
 
-@pytest.mark.parametrize("cfg,P,gens", [(1, None, 9), (1, 41, 6), (1, 2, 5), (2, 33, 4)])
+@pytest.mark.parametrize("cfg,P,gens", [(1, None, 9), (1, 41, 6), (1, 3, 5), (2, 33, 4)])
 def test_persistent_local_population_form(orc, cfg, P, gens):
     """Small populations (P K <= 4096 genes) run the persistent loop with the whole population in every CTA's shared memory
     (no population traffic, one grid barrier per generation).  Same bits as the shared-population form
-    (GAME_TUNE_PERSISTENT = 2) and as the launch path (0), including odd P, P = 2 and a resumed run."""
+    (GAME_TUNE_PERSISTENT = 2) and as the launch path (0), including odd P, P = 3 and a resumed run."""
     w = wl.config(cfg)
     w = w.scaled(P=P or w.P, generations=gens)
     fam, d = w.family, w.degree
