@@ -267,6 +267,8 @@ void game_destroy(game_ctx *c)
     dfree(c->gbar);
     free(c->tmap_E); free(c->tmap_C); free(c->tmap_Es);
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    for (cudaEvent_t e : c->copy_ev) if (e) cudaEventDestroy(e);
     delete c;
 }
 
@@ -372,10 +374,42 @@ int game_fitness_host(game_ctx *c, const float *pop, int P, float *out)
         c->stage_cap = P;
     }
     int *range = reinterpret_cast<int *>(c->stage_fit + P);
-    GAME_CUDA(c, cudaMemcpyAsync(c->stage_pop, pop, (size_t)P * c->K * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    GAME_CUDA(c, cudaMemsetAsync(range, 0, 2 * sizeof(int), c->stream));
-    int rc = launch_max_abs(c, c->stage_pop, (long long)P * c->K, range);
-    if (!rc) rc = run_fitness(c, c->stage_pop, P, c->stage_fit, nullptr);
+    // Large populations go up in four chunks on a copy stream, each chunk's kernels starting as soon as it has landed: the
+    // upload (27 MB at config 5, ~1.1 ms over PCIe) hides behind the evaluation of the chunks before it.  A chromosome's
+    // fitness does not depend on its row or on the rest of the population (DESIGN P20), so the chunks give the bits one call
+    // would; they are used only when a chunk takes the same path and launch configuration class as the whole population.
+    const int Pc = (((P + 3) / 4 + 255) / 256) * 256;
+    // (a chunk must also be well above one wave of tiles, or the tensor path would switch to its half-size tiles for it)
+    const bool chunked = P >= 4096 && Pc >= 1024 && resolve_path(c, Pc) == resolve_path(c, P) &&
+                         (c->Npad256 / 256) * (long long)(Pc / 128) >= 2LL * c->sm_count;
+    int rc = GAME_OK;
+    if (!chunked) {
+        GAME_CUDA(c, cudaMemcpyAsync(c->stage_pop, pop, (size_t)P * c->K * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+        GAME_CUDA(c, cudaMemsetAsync(range, 0, 2 * sizeof(int), c->stream));
+        rc = launch_max_abs(c, c->stage_pop, (long long)P * c->K, range);
+        if (!rc) rc = run_fitness(c, c->stage_pop, P, c->stage_fit, nullptr);
+    } else {
+        if (!c->copy_stream) {
+            GAME_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+            for (cudaEvent_t &e : c->copy_ev) GAME_CUDA(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        }
+        GAME_CUDA(c, cudaEventRecord(c->copy_ev[0], c->stream));            // earlier work on the context's stream may still read the staging area
+        GAME_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->copy_ev[0], 0));
+        int nch = 0;
+        for (int p0 = 0; p0 < P; p0 += Pc, ++nch) {
+            const int n = P - p0 < Pc ? P - p0 : Pc;
+            GAME_CUDA(c, cudaMemcpyAsync(c->stage_pop + (size_t)p0 * c->K, pop + (size_t)p0 * c->K, (size_t)n * c->K * sizeof(float),
+                                         cudaMemcpyHostToDevice, c->copy_stream));
+            GAME_CUDA(c, cudaEventRecord(c->copy_ev[1 + nch], c->copy_stream));
+        }
+        GAME_CUDA(c, cudaMemsetAsync(range, 0, 2 * sizeof(int), c->stream));
+        for (int i = 0; i < nch && !rc; ++i) {
+            const int p0 = i * Pc, n = P - p0 < Pc ? P - p0 : Pc;
+            GAME_CUDA(c, cudaStreamWaitEvent(c->stream, c->copy_ev[1 + i], 0));
+            rc = launch_max_abs(c, c->stage_pop + (size_t)p0 * c->K, (long long)n * c->K, range);
+            if (!rc) rc = run_fitness(c, c->stage_pop + (size_t)p0 * c->K, n, c->stage_fit + p0, nullptr);
+        }
+    }
     if (rc) return rc;
     int hr[2] = {0, 0};
     GAME_CUDA(c, cudaMemcpyAsync(out, c->stage_fit, (size_t)P * sizeof(float), cudaMemcpyDeviceToHost, c->stream));

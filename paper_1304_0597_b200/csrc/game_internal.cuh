@@ -164,6 +164,8 @@ struct game_ctx {
     float c16_scale = 0.f;
     float *stage_pop = nullptr, *stage_fit = nullptr;   // device staging for *_host calls
     size_t stage_cap = 0;
+    cudaStream_t copy_stream = nullptr;                 // game_fitness_host on large populations: uploads run here, a chunk ahead of the kernels
+    cudaEvent_t copy_ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // [0] entry (context stream), [1..4] chunk uploaded
     void *tmap_E = nullptr, *tmap_C = nullptr;          // host copies of CUtensorMap (TENSOR path)
     void *tmap_Es = nullptr;                            // the same for E16s
 

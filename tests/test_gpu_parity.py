@@ -197,6 +197,33 @@ def test_fitness_host_matches_device(orc):
     check_fitness(orc, a, fam, d, X, t, pop, SIGMOID, TMSE, 0.49, ctx.resolved_path(P))
 
 
+@pytest.mark.parametrize("cfg,N,P", [(3, 20000, 4096), (5, 6000, 5000), (2, None, 4100)])
+def test_fitness_host_chunked_upload(orc, cfg, N, P):
+    """game_fitness_host uploads populations of >= 4096 chromosomes in four chunks on a copy stream, a chunk ahead of the
+    kernels; a chromosome's fitness does not depend on its row (P20), so the result equals the device call bit for bit --
+    also with a ragged last chunk, pinned or pageable host memory, and twice in a row (the staging area is reused).  Small
+    datasets (config 2: a chunk would fall below one wave of tiles and change the tile shape) go up in one piece."""
+    w = wl.config(cfg)
+    w = w.scaled(N=N or w.N, P=P)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    pop = wl.uniform_population(P, w.K, cfg)
+    ctx = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    b = ctx.fitness(dev(pop)).cpu().numpy()
+    pinned = torch.from_numpy(pop).pin_memory().numpy()
+    for src in (pop, pinned, pinned):
+        a = ctx.fitness_host(src)
+        assert np.array_equal(a.view(np.uint32), b.view(np.uint32))
+    rows = np.array([0, 1023, 1024, P // 2, P - 1])
+    check_fitness(orc, b[rows], fam, d, X, t, pop[rows], w.act, w.err, w.R, ctx.resolved_path(P), "host chunks")
+    # a gene outside the fp16 range in the LAST chunk is still reported
+    bad = pop.copy(); bad[P - 1, 0] = 1e6
+    if ctx.resolved_path(P) != g.GAME_PATH_FP32:
+        with pytest.raises(g.GameError) as e:
+            ctx.fitness_host(bad)
+        assert e.value.code == 5
+
+
 def test_planted_and_replication(orc):
     # P8 / P10 on the GPU: the planted chromosome scores ~0; replicated rows leave the error unchanged
     fam, d, F, N = TRIG, 4, 11, 2100
