@@ -380,7 +380,8 @@ int game_fitness_host(game_ctx *c, const float *pop, int P, float *out)
     // would; they are used only when a chunk takes the same path and launch configuration class as the whole population.
     const int Pc = (((P + 3) / 4 + 255) / 256) * 256;
     // (a chunk must also be well above one wave of tiles, or the tensor path would switch to its half-size tiles for it)
-    const bool chunked = P >= 4096 && Pc >= 1024 && resolve_path(c, Pc) == resolve_path(c, P) &&
+    // ... and the upload must be worth hiding: four times the launches cost more than 1.8 MB take (config 3: 0.235 vs 0.220 ms per call)
+    const bool chunked = P >= 4096 && Pc >= 1024 && (size_t)P * c->K * sizeof(float) >= ((size_t)8 << 20) && resolve_path(c, Pc) == resolve_path(c, P) &&
                          (c->Npad256 / 256) * (long long)(Pc / 128) >= 2LL * c->sm_count;
     int rc = GAME_OK;
     if (!chunked) {
