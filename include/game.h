@@ -119,10 +119,12 @@ int game_resolved_path(const game_ctx *ctx, int P);
  *   GAME_EXPAND_MATERIALIZED  streams the fp16 expansion matrix built once by game_load (L254's hoisting);
  *   GAME_EXPAND_REGENERATED   recomputes each 256-pattern tile of it from X inside the kernel, straight into shared
  *                             memory, with the population's fp16 copy resident there.  Available for the per-feature
- *                             families when P <= 256 and K (padded to 64 per 8 features) <= 576, and for the
+ *                             families when P <= 256, F <= 32 and K (padded to 64 per 8 features) <= 576, and for the
  *                             trigonometric family only when max|X| <= pi; otherwise the fitness call fails with
  *                             GAME_ERR_UNSUPPORTED;
- *   GAME_EXPAND_AUTO          (default) the faster of the two as measured on B200.
+ *   GAME_EXPAND_AUTO          (default) the faster of the two as measured on B200: regenerated
+ *                             where it is available AND the contraction has >= 8 k-blocks of 64 terms, more than 24
+ *                             features, the launch >= 2000 tiles of 256 patterns and P > 32; materialised otherwise.
  * game_resolved_expansion: which of the two a TENSOR-path fitness call on P chromosomes will use, or -1 if the
  * requested one is unavailable. */
 int game_set_expansion(game_ctx *ctx, int mode);
