@@ -544,6 +544,9 @@ int launch_evolve_persistent(game_ctx *c, const game_ga_params *gp, unsigned lon
     if (split) {
         int rcs = tensor_prepare_split(c);
         if (rcs) return rcs;
+    } else {
+        int rce = tensor_ensure_E16(c);
+        if (rce) return rce;
     }
     if (!c->gbar) GAME_CUDA(c, cudaMalloc(&c->gbar, sizeof(unsigned int)));
     GAME_CUDA(c, cudaMemsetAsync(c->gbar, 0, sizeof(unsigned int), c->stream));

@@ -649,6 +649,17 @@ int tensor_prepare(game_ctx *ctx)
     return GAME_OK;
 }
 
+// the materialised fp16 expansion and its tensor maps, where game_load left them for the first call that needs them
+int tensor_ensure_E16(game_ctx *ctx)
+{
+    if (ctx->E16) return GAME_OK;
+    const size_t n16 = (size_t)ctx->Npad256 * ctx->Kpad;
+    GAME_CUDA(ctx, cudaMalloc(&ctx->E16, n16 * sizeof(__half)));
+    GAME_CUDA(ctx, cudaMemsetAsync(ctx->E16, 0, n16 * sizeof(__half), ctx->stream));
+    int rc = launch_expand_fp16(ctx, nullptr);
+    return rc ? rc : tensor_prepare(ctx);
+}
+
 // TENSOR_SPLIT path: the [hi | hi | lo] expansion and its tensor maps, built on the first call that needs them
 int tensor_prepare_split(game_ctx *ctx)
 {
@@ -680,7 +691,8 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     const int npos = tc_num_positions(ctx->family, ctx->degree, ctx->F, ctx->K);
     const int k_last = (npos - (ctx->Kpad - BKB) + UMMA_K - 1) / UMMA_K;
     const int kb_range = ctx->Kpad / BKB;                    // k-blocks per K range
-    const CUtensorMap *maps_E = (const CUtensorMap *)(split ? ctx->tmap_Es : ctx->tmap_E);
+    // (the generator variant takes no expansion map: the population's stands in for the unused argument)
+    const CUtensorMap *maps_E = (const CUtensorMap *)(SRC == SRC_GEN ? ctx->tmap_C : split ? ctx->tmap_Es : ctx->tmap_E);
     const int smem = SRC != SRC_TMA ? k_blocks * A_BYTES + GEN_STAGES * GEN_B_BYTES + 1024 + TC_TAIL_BYTES
                    : BNT == BN    ? C::SMEM
                                   : 6 * (A_BYTES + BNT * BKB * 2) + 1024 + TC_TAIL_BYTES;
@@ -700,7 +712,7 @@ static int launch_variant(game_ctx *ctx, int n_tiles, int m_blocks, int Ppad, co
     attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = pdl_enabled(ctx) ? 2 : 1;
     KernelTimer timer(ctx);
-    GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, maps_E[BNT / CG == 128 ? 1 : 0], n_tiles,
+    GAME_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *(const CUtensorMap *)ctx->tmap_C, maps_E[SRC == SRC_GEN ? 0 : BNT / CG == 128 ? 1 : 0], n_tiles,
                                       m_blocks, k_blocks, ctx->N, (const float *)ctx->t, ctx->R, ctx->partial, Ppad, state,
                                       (const float *)ctx->X, ctx->F, ctx->degree, k_last, kb_range));
     return GAME_OK;
@@ -758,6 +770,10 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     const int Kp = (split ? 3 : 1) * ctx->Kpad;              // contraction depth the kernel sees
     const int expansion = split ? GAME_EXPAND_MATERIALIZED : tensor_expansion(ctx, P);
     if (expansion < 0) return fail(ctx, GAME_ERR_UNSUPPORTED, "regenerated expansion unavailable for this shape (needs P <= 256, K <= 576 after padding, trig: max|X| <= pi)");
+    if (!split && expansion != GAME_EXPAND_REGENERATED) {
+        int rce = tensor_ensure_E16(ctx);
+        if (rce) return rce;
+    }
     // Small populations (one CTA pair covers all chromosomes): keep the fp16 population tile RESIDENT in shared memory and
     // stream only the expansion (SRC_RES) -- a third of SRC_TMA's L2 -> SM traffic.  Config 4, same box: 0.229 vs 0.263 ms,
     // identical bits; the kernel then runs at 5.1 TB/s of HBM reads (78 % of the measured peak).

@@ -188,19 +188,30 @@ static int load_common(game_ctx *c, const float *X, const float *targets, long l
         c->N = N;                                 // the expansion launchers read it; withdrawn again on failure
         int rc = launch_check_finite(c, c->X, N * c->F, c->t, N, flag);
         if (rc) return rc;
-        // the fp16 tile-blocked expansion of the tensor paths (also measures max|E|); the fp32 term-major one (ET) is
-        // built on first use by the FFMA kernels / game_predict / game_classify (ensure_ET)
-        size_t n16 = (size_t)c->Npad256 * c->Kpad;
-        GAME_CUDA(c, cudaMalloc(&c->E16, n16 * sizeof(__half)));
-        GAME_CUDA(c, cudaMemsetAsync(c->E16, 0, n16 * sizeof(__half), c->stream));
-        rc = launch_expand_fp16(c, reinterpret_cast<float *>(flag + 1));
-        if (rc) return rc;
+        // The fp16 tile-blocked expansion of the tensor paths (E16) also measures max|E|, which decides whether those paths are
+        // offered.  Where that maximum is known without looking -- |cos|, |sin| <= 1 always; |T_m(x)| <= 1 for |x| <= 1 -- E16 is
+        // built on FIRST USE instead (tensor_ensure_E16): a run whose fitness calls all regenerate the expansion in the kernel
+        // (config 4, and every chunk of the out-of-core driver at such shapes) never pays for the matrix or its 2 N Kpad bytes.
+        // The fp32 term-major expansion (ET) is built on first use by the FFMA kernels / game_predict / game_classify (ensure_ET).
         GAME_CUDA(c, cudaMemcpyAsync(h, flag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
         GAME_CUDA(c, cudaStreamSynchronize(c->stream));
         if (h[0]) return fail(c, GAME_ERR_NONFINITE_INPUT, "game_load: X or targets contain NaN/Inf");
+        memcpy(&c->x_maxabs, &h[2], sizeof(float));
+        const bool bounded = c->family == GAME_TRIG || (c->family == GAME_CHEB && c->x_maxabs <= 1.0f);
+        if (!bounded) {
+            size_t n16 = (size_t)c->Npad256 * c->Kpad;
+            GAME_CUDA(c, cudaMalloc(&c->E16, n16 * sizeof(__half)));
+            GAME_CUDA(c, cudaMemsetAsync(c->E16, 0, n16 * sizeof(__half), c->stream));
+            rc = launch_expand_fp16(c, reinterpret_cast<float *>(flag + 1));
+            if (rc) return rc;
+            GAME_CUDA(c, cudaMemcpyAsync(h, flag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+            GAME_CUDA(c, cudaStreamSynchronize(c->stream));
+        } else {
+            const float one = 1.0f;
+            memcpy(&h[1], &one, sizeof(float));
+        }
         float mx;
         memcpy(&mx, &h[1], sizeof(float));
-        memcpy(&c->x_maxabs, &h[2], sizeof(float));
         // fp16 rounding is relative: sums over features (tied families) of magnitude ~F would carry an absolute
         // error ~F*2^-11 into z, outside the 1e-3 class, so the tensor path is offered for |E| <= 2 only
         // ... and the tile-blocked expansion is addressed with 32-bit TMA row coordinates (the split form has 3x the rows)
@@ -209,8 +220,8 @@ static int load_common(game_ctx *c, const float *X, const float *targets, long l
         // the split form keeps ~22 bits of every value whatever its magnitude (hi + lo), so it only needs the values well
         // inside fp16's range and above its subnormals' grain: |E| <= 1024 (e.g. Chebyshev terms of unnormalised features)
         c->split_ok = mx <= 1024.0f && rows_ok && tc_permuted(c->family);
-        if (c->tensor_ok) return tensor_prepare(c);
-        dfree(c->E16);
+        if (c->tensor_ok && c->E16) return tensor_prepare(c);
+        if (!c->tensor_ok) dfree(c->E16);
         return GAME_OK;
     };
     const int rc = body();

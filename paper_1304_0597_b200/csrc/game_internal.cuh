@@ -268,6 +268,7 @@ int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scra
 // fitness_tc.cu
 bool tensor_path_built();
 int tensor_prepare(game_ctx *ctx);                               // tensor maps etc. after load
+int tensor_ensure_E16(game_ctx *ctx);                            // build the materialised fp16 expansion if game_load deferred it
 int tensor_expansion(const game_ctx *ctx, int P);                // GAME_EXPAND_MATERIALIZED / _REGENERATED, or -1
 int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, const DevState *state, PartialInfo *defer,
                           bool split = false);
