@@ -600,6 +600,40 @@ def test_auto_regenerates_config4_full_size(orc):
     ctx.destroy()
 
 
+def test_expansion_matrix_is_built_on_first_use(orc):
+    """game_load defers the fp16 expansion matrix when max|E| is known without measuring (trig; Chebyshev on [-1, 1]):
+    a context whose fitness calls regenerate the expansion in the kernel never allocates its 2 N Kpad bytes; the first
+    call that streams the matrix builds it, with the same result as before."""
+    import torch
+    N, F, d, P = 300000, 32, 8, 64
+    rng = np.random.default_rng(77)
+    X = rng.uniform(-1, 1, (N, F)).astype(np.float32)
+    t = rng.integers(0, 2, N).astype(np.float32)
+    e16_bytes = ((N + 255) // 256) * 256 * 576 * 2
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    ctx = make_ctx(TRIG, d, X, t, SIGMOID, MSE, 0.0, g.GAME_PATH_TENSOR)
+    pop = rng.uniform(-1, 1, (P, ctx.num_terms())).astype(np.float32)
+    ctx.set_expansion(g.GAME_EXPAND_REGENERATED)
+    a = ctx.fitness(dev(pop)).cpu().numpy()
+    torch.cuda.synchronize()
+    used_regen = free0 - torch.cuda.mem_get_info()[0]
+    assert used_regen < e16_bytes // 2, (used_regen, e16_bytes)
+    ctx.set_expansion(g.GAME_EXPAND_MATERIALIZED)
+    b = ctx.fitness(dev(pop)).cpu().numpy()
+    torch.cuda.synchronize()
+    used_mat = free0 - torch.cuda.mem_get_info()[0]
+    assert used_mat >= e16_bytes, (used_mat, e16_bytes)
+    assert np.allclose(a, b, rtol=2e-4, atol=2e-6)
+    rows = np.array([0, 17, P - 1])
+    check_fitness(orc, b[rows], TRIG, d, X, t, pop[rows], SIGMOID, MSE, 0.0, g.GAME_PATH_TENSOR, "deferred E16")
+    ctx.destroy()
+    # Chebyshev features outside [-1, 1]: the maximum has to be measured, so the matrix is built at load (and the path decided)
+    ctx = make_ctx(CHEB, 3, (X[:4096, :8] * 1.5).astype(np.float32), t[:4096], path=g.GAME_PATH_AUTO)
+    assert ctx.resolved_path(P) in (g.GAME_PATH_TENSOR_SPLIT, g.GAME_PATH_FP32)          # max|T_3(1.5)| = 9 > 2: no one-pass fp16 path
+    ctx.destroy()
+
+
 def test_trajectory_regenerated(orc):
     """A GA run with the regenerated expansion: operators bit-exact, fitness within the tensor class."""
     w = wl.config(1).scaled(P=64, generations=6)
