@@ -391,7 +391,7 @@ def run_ours(args, w):
         e2e_value, _ = replicas.job_throughput(float(hi - lo) * w.P * e2e_steps, world, e0.elapsed_time(e1), "cuda")
         e2e = {"value": e2e_value, "unit": UNIT,
                "h2d_bytes_per_step": int(wr.P * wr.K * 4), "d2h_bytes_per_step": int(wr.P * 4),
-               "what": "game_fitness_host: population from pinned host memory in (>= 4096 chromosomes: four chunks on a copy stream, a chunk ahead of the kernels), fitness back out, per step; "
+               "what": "game_fitness_host: population from pinned host memory in (large populations: two or four chunks on a copy stream, a chunk ahead of the kernels), fitness back out, per step; "
                        "dataset resident (game_load_host took %.1f ms once, incl. H2D of X and the expansion)" % load_ms}
 
     if rank != 0:

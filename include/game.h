@@ -149,7 +149,7 @@ int game_load_host(game_ctx *ctx, const float *X, const float *targets, long lon
  *   out[p] = mean_n e  (RMSE: sqrt).
  * pop is P x K row-major fp32, out is P fp32.  Asynchronous.  The N x P matrix z never reaches HBM.
  * game_fitness: DEV pointers.  game_fitness_host: HOST pointers; copies pop in, runs, copies out back
- * and synchronises the stream before returning.  Populations of >= 4096 chromosomes and >= 8 MB on large datasets go up in four
+ * and synchronises the stream before returning.  Populations of >= 2048 chromosomes on large datasets go up in two (>= 1 MB) or four (>= 8 MB)
  * chunks on a copy stream of the context's own (ordered after the work already on the context's stream), each chunk's
  * kernels starting when it has landed -- pass pinned memory for the upload to overlap; the result is bit-identical to
  * one call (a chromosome's fitness does not depend on its row or on the rest of the population). */

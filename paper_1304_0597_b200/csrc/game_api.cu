@@ -385,14 +385,17 @@ int game_fitness_host(game_ctx *c, const float *pop, int P, float *out)
         c->stage_cap = P;
     }
     int *range = reinterpret_cast<int *>(c->stage_fit + P);
-    // Large populations go up in four chunks on a copy stream, each chunk's kernels starting as soon as it has landed: the
+    // Large populations go up in chunks on a copy stream, each chunk's kernels starting as soon as it has landed: the
     // upload (27 MB at config 5, ~1.1 ms over PCIe) hides behind the evaluation of the chunks before it.  A chromosome's
     // fitness does not depend on its row or on the rest of the population (DESIGN P20), so the chunks give the bits one call
     // would; they are used only when a chunk takes the same path and launch configuration class as the whole population.
-    const int Pc = (((P + 3) / 4 + 255) / 256) * 256;
+    // How many chunks: every chunk repeats the small launches of a call, so a 1.8 MB population (config 3) goes up in two
+    // (242 us per call against 270 in one piece; four measured slower than one there), 8 MB and more in four.
+    const size_t pop_bytes = (size_t)P * c->K * sizeof(float);
+    const int want = pop_bytes >= ((size_t)8 << 20) ? 4 : pop_bytes >= ((size_t)1 << 20) ? 2 : 1;
+    const int Pc = (((P + want - 1) / want + 255) / 256) * 256;
     // (a chunk must also be well above one wave of tiles, or the tensor path would switch to its half-size tiles for it)
-    // ... and the upload must be worth hiding: four times the launches cost more than 1.8 MB take (config 3: 0.235 vs 0.220 ms per call)
-    const bool chunked = P >= 4096 && Pc >= 1024 && (size_t)P * c->K * sizeof(float) >= ((size_t)8 << 20) && resolve_path(c, Pc) == resolve_path(c, P) &&
+    const bool chunked = want > 1 && P >= 2048 && Pc >= 1024 && resolve_path(c, Pc) == resolve_path(c, P) &&
                          (c->Npad256 / 256) * (long long)(Pc / 128) >= 2LL * c->sm_count;
     int rc = GAME_OK;
     if (!chunked) {

@@ -197,9 +197,9 @@ def test_fitness_host_matches_device(orc):
     check_fitness(orc, a, fam, d, X, t, pop, SIGMOID, TMSE, 0.49, ctx.resolved_path(P))
 
 
-@pytest.mark.parametrize("cfg,N,P", [(3, 20000, 20000), (5, 6000, 5000), (2, None, 4100)])
+@pytest.mark.parametrize("cfg,N,P", [(3, 20000, 20000), (3, 30000, 4096), (5, 6000, 5000), (2, None, 4100)])
 def test_fitness_host_chunked_upload(orc, cfg, N, P):
-    """game_fitness_host uploads populations of >= 4096 chromosomes and >= 8 MB in four chunks on a copy stream, a chunk ahead of the
+    """game_fitness_host uploads populations of >= 2048 chromosomes in two (>= 1 MB) or four (>= 8 MB) chunks on a copy stream, a chunk ahead of the
     kernels; a chromosome's fitness does not depend on its row (P20), so the result equals the device call bit for bit --
     also with a ragged last chunk, pinned or pageable host memory, and twice in a row (the staging area is reused).  Small
     datasets (config 2: a chunk would fall below one wave of tiles and change the tile shape) go up in one piece."""
