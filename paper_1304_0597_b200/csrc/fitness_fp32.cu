@@ -183,6 +183,47 @@ post_small_kernel(const float *__restrict__ partial, int n_chunks, int Ppad, int
     }
 }
 
+// The same tail for small populations over MANY slabs (config 4: 256 chromosomes x 3907 tiles): the slab axis is totalled by
+// finalize_split_kernel's FIN_SPLIT CTAs, and this single CTA adds those totals in finalize_merge_kernel's order, ranks and
+// tests -- one launch instead of three (merge, rank count, rank scatter) in every generation.
+__global__ void __launch_bounds__(256, 1)
+post_merge_small_kernel(const double *__restrict__ fin2, int Ppad, int P, long long N, int err,
+                        float *__restrict__ fit, int *__restrict__ order, DevState *state, float stop_error)
+{
+    pdl_wait();
+    pdl_trigger();
+    if (state->stopped) return;
+    __shared__ unsigned long long keys[256];
+    const int p = threadIdx.x;
+    unsigned long long mine = ~0ull;
+    float f = 0.f;
+    if (p < P) {
+        double tot = 0.0;
+        for (int y = 0; y < FIN_SPLIT; ++y) tot += fin2[(long long)y * Ppad + p];
+        double v = tot / (double)N;
+        if (err == GAME_ERR_RMSE) v = sqrt(v);
+        f = (float)v;
+        fit[p] = f;
+        mine = ((unsigned long long)sort_key(f) << 32) | (unsigned)p;
+    }
+    keys[p] = mine;
+    __syncthreads();
+    if (p >= P) return;
+    int cnt = 0;
+#pragma unroll 8
+    for (int q = 0; q < P; ++q) cnt += keys[q] < mine;
+    order[cnt] = p;
+    if (cnt == 0) {
+        state->best_error = f;
+        state->best_index = p;
+        state->evals_done += 1;
+        if (stop_error >= 0.0f && f <= stop_error) state->stop_request = 1;
+    }
+}
+
+__global__ void finalize_split_kernel(const float *__restrict__ partial, int n_chunks, int Ppad, int P, double *__restrict__ fin2,
+                                      const DevState *state);
+
 int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scratch, int *order, DevState *state,
                 float stop_error)
 {
@@ -190,6 +231,14 @@ int launch_post(game_ctx *ctx, PartialInfo pi, int P, float *fit, int *rank_scra
         GAME_CUDA(ctx, launch_pdl(post_small_kernel, dim3(1), dim3(256), 0, ctx, ctx->partial, pi.n_chunks, pi.Ppad, P, ctx->N,
                                   ctx->err, fit, order, state, stop_error));
         ++ctx->launches;
+        return GAME_OK;
+    }
+    if (P <= 256 && pi.n_chunks >= 1024) {            // the two-pass reduction's first pass, then merge + rank + stop test in one CTA
+        GAME_CUDA(ctx, launch_pdl(finalize_split_kernel, dim3((P + 31) / 32, FIN_SPLIT), dim3(32, 32), 0, ctx, ctx->partial, pi.n_chunks, pi.Ppad, P,
+                                  ctx->fin2, (const DevState *)state));
+        GAME_CUDA(ctx, launch_pdl(post_merge_small_kernel, dim3(1), dim3(256), 0, ctx, (const double *)ctx->fin2, pi.Ppad, P, ctx->N, ctx->err,
+                                  fit, order, state, stop_error));
+        ctx->launches += 2;
         return GAME_OK;
     }
     // (a fused multi-CTA finalize + rank kernel for mid-size populations was measured on config 2: 22.7 vs 19.7 us per
