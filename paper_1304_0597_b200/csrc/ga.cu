@@ -41,6 +41,9 @@ int launch_init_population(game_ctx *ctx, int mode, unsigned long long seed, int
 }
 
 // ---- a6: rank by counting.  key = (error, index) ascending, NaN as +inf, -0 as +0 (DESIGN G20) --------
+// (Measured and dropped: ONE launch with all P keys in every CTA's shared memory and eight lanes per chromosome -- the tail of a
+// generation grew from 30 to 45 us on config 3 (P = 4096) and from 100 to 121 us on config 5: 128-256 CTAs each staging
+// every key cost more than the launch they saved.)
 constexpr int RANK_T = 128, RANK_Q = 256;   // chromosomes per CTA x keys per CTA: (P/128) x (P/256) CTAs
 
 __global__ void rank_count_kernel(const float *__restrict__ fit, int P, int *__restrict__ rank, const DevState *state)
