@@ -587,6 +587,11 @@ def test_auto_regenerates_config4_full_size(orc):
         ctx.set_expansion(mode)
         got[mode] = ctx.fitness(dev(pop)).cpu().numpy()
         check_fitness(orc, got[mode][rows], fam, d, X, t, pop[rows], w.act, w.err, w.R, g.GAME_PATH_TENSOR, "cfg 4 expansion %d" % mode)
+    # the generator's stores race with nothing: repeated launches give the same bits
+    ctx.set_expansion(g.GAME_EXPAND_AUTO)
+    for _ in range(6):
+        again = ctx.fitness(dev(pop)).cpu().numpy()
+        assert np.array_equal(again.view(np.uint32), got[g.GAME_EXPAND_AUTO].view(np.uint32))
     # MSE is continuous in z: there the two sources must agree far inside the tolerance class
     ctx.set_error(MSE, 0.0)
     for mode in (g.GAME_EXPAND_AUTO, g.GAME_EXPAND_MATERIALIZED):
