@@ -392,7 +392,7 @@ def run_ours(args, w):
         e2e = {"value": e2e_value, "unit": UNIT,
                "h2d_bytes_per_step": int(wr.P * wr.K * 4), "d2h_bytes_per_step": int(wr.P * 4),
                "what": "game_fitness_host: population from pinned host memory in (large populations: two or four chunks on a copy stream, a chunk ahead of the kernels), fitness back out, per step; "
-                       "dataset resident (game_load_host took %.1f ms once, incl. H2D of X and the expansion)" % load_ms}
+                       "dataset resident (game_load_host took %.1f ms once: H2D of X and the targets, finite check; the fp16 expansion matrix, where a path streams it, is built on the first call that needs it -- during warm-up)" % load_ms}
 
     if rank != 0:
         return
