@@ -242,6 +242,37 @@ int game_init_population(game_ctx *ctx, int init_mode, unsigned long long seed, 
  * compare the device generator with an independent implementation word for word. */
 int game_philox(game_ctx *ctx, unsigned long long seed, const unsigned int *ctr, int n, unsigned int *out);
 
+/* game_rank without any device-memory allocation (a6: the "sort by fitness" of the training loop, L217-L220; same key
+ * and tie rule as game_rank, DESIGN G20).
+ *
+ * For callers that cannot allocate on the GPU: game_rank takes its P ints of counting scratch from the driver's
+ * stream-ordered allocator on every call, which is not an option in a process whose device memory is wholly owned by
+ * another component (a framework's caching allocator, a serving engine that reserved all of HBM at start-up), in a
+ * latency-critical loop that must stay off the driver's allocation path, or in a service that forbids driver
+ * allocations after set-up so that running out of memory can only happen at start.  This entry point needs no context
+ * and calls no cudaMalloc / cudaFree / allocating library routine: its scratch is an array of
+ * GAME_RANK_STATIC_MAX_P ints (256 KiB) built into the library image.  Every GPU that loads libgame_b200.so holds that
+ * array until the process exits, used or not; hence the modest limit.
+ *
+ *   fit    DEV  P fp32 errors (lower is better; NaN ranks last, -0 == +0, equal errors by ascending index)
+ *   order  DEV  P int32, written: order[0] = index of the best chromosome ... order[P-1] = the worst
+ *   cuda_stream  a cudaStream_t of the CURRENT device (0 = legacy default stream); the work is enqueued on it and
+ *          the call returns without waiting.  fit and order stay the caller's and must live until the stream has
+ *          passed this call.
+ * Runs on the device that is current in the calling thread.  The FIRST call on each device also looks up the device
+ * address of the built-in array (once per device; a cheap host-side query, no allocation): make that first call
+ * during set-up, before any stream capture is begun.
+ * 1 <= P <= GAME_RANK_STATIC_MAX_P, else GAME_ERR_INVALID_ARG (use game_rank for larger populations); NULL pointers
+ * likewise; CUDA failures give GAME_ERR_CUDA.  game_rank_static_error() returns the text of the calling thread's last
+ * failure (HOST string owned by the library, "" after a success).
+ * All calls on one GPU share the one array and find in it what the previous call left: each call clears the part it
+ * uses first, on its stream.  Calls that can OVERLAP on the same GPU -- different streams with no ordering between
+ * them, or several threads -- race on that array and give wrong orders: keep them on one stream or order them with
+ * events. */
+#define GAME_RANK_STATIC_MAX_P 65536
+int game_rank_static(const float *fit, int P, int *order, void *cuda_stream);
+const char *game_rank_static_error(void);
+
 /* Number of kernels this context has launched since creation (bench.py reports it). */
 long long game_launch_count(const game_ctx *ctx);
 

@@ -36,7 +36,9 @@ SYMBOLS = [
     "game_set_population", "game_set_generation", "game_evolve", "game_get_population",
     "game_get_population_host", "game_rank", "game_ga_step", "game_init_population", "game_philox",
     "game_launch_count", "game_set_kernel_timing", "game_get_kernel_timing", "game_microbench",
+    "game_rank_static", "game_rank_static_error",
 ]
+GAME_RANK_STATIC_MAX_P = 65536
 
 
 class game_ga_params(C.Structure):
@@ -115,6 +117,9 @@ def load_library():
         L.game_set_kernel_timing.argtypes = [vp, i]
         L.game_get_kernel_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(ll)]
         L.game_microbench.argtypes = [vp, i, i, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.game_rank_static.argtypes = [vp, i, vp, vp]
+        L.game_rank_static_error.restype = C.c_char_p
+        L.game_rank_static_error.argtypes = []
         _lib = L
     return _lib
 
@@ -143,6 +148,26 @@ def ga_params(P, tournament_size=3, elitism=2, elite_mode=GAME_ELITE_COPIES_OF_B
               p_mutation=0.05, stop_error=-1.0):
     return game_ga_params(P, tournament_size, elitism, elite_mode, selection, init_mode,
                           p_crossover, p_mutation, stop_error)
+
+
+def rank_static(fit, order=None, stream=None):
+    """``game_rank_static``: rank P errors (CUDA float32 tensor) into ``order`` (int32, order[0] = best) without allocating
+    device memory inside the library -- for hosts whose GPU memory belongs to another allocator or that must stay off the
+    driver's allocation path.  Pass a preallocated ``order`` to keep this wrapper from allocating either (it only makes
+    one when none is given).  P <= GAME_RANK_STATIC_MAX_P; the library's one scratch array is shared, so calls that
+    could overlap on the GPU must be ordered by the caller.  Enqueued on ``stream`` (default: torch's current stream)."""
+    import torch
+    L = load_library()
+    if not torch.cuda.is_available():
+        raise RuntimeError("libgame_b200 needs a CUDA device; there is no CPU fallback")
+    if order is None:
+        order = torch.empty(fit.shape[0], dtype=torch.int32, device=fit.device)
+    s = stream if stream is not None else torch.cuda.current_stream(fit.device)
+    with torch.cuda.device(fit.device):
+        rc = L.game_rank_static(_dev(fit, torch.float32), fit.shape[0], _dev(order, torch.int32), C.c_void_p(s.cuda_stream))
+    if rc:
+        raise GameError(rc, L.game_rank_static_error().decode())
+    return order
 
 
 class Game:
