@@ -4,6 +4,9 @@
         fl32(f_max - f_min)) * 2^24) + 1, every step one IEEE fp32 operation.
   P16b  oracle_init_gene, GAME_INIT_NORMAL_PM1 (DESIGN G13 / R2): S = sum of the top 24 bits of the 12 Philox words of
         counters (k, p, j, TAG_INIT), j = 0..2; gene = clamp(fl32(fl32(S - 6 (2^24 - 1)) * fl32(2^-24 / 3)), -1, 1).
+  P18b  oracle_ga_step (DESIGN R3 / R5 / R6, G15-G19): the tournament ranks, parents, crossover flag and cut, mutation
+        mask and values and the elite copies of whole small generations (VERDICT r2 finding (i): which word and which
+        counter feeds which decision was pinned only statistically).
 
 The expected values are derived here in exact rational arithmetic (fractions.Fraction) with an integer implementation
 of round-to-nearest-even to 24 significant bits -- no numpy/C float operation of the kind the oracle uses -- and the
@@ -158,6 +161,77 @@ def test_p16b_init_normal_gene_by_hand(orc, aten_words):
         v = np.float32(orc.lib().oracle_init_gene(2, ctypes.c_uint64(seed), p, k))
         assert Fraction(float(u)) == Fraction((w >> 8) - 2**23, 2**23)
         assert Fraction(float(v)) == Fraction(w >> 8, 2**24)
+
+
+# ---- P18b: one whole generation of operator decisions from ATen's Philox words (R3, R5, R6) ----------------------
+def ga_step_by_hand(words, seed, g, P, K, t, e, elite_mode, pc, pm, order, pop):
+    """DESIGN R3 / R5 / R6 and G15-G19 written out with Python integers; `words(seed, c0, c1, c2, c3)` -> [w0..w3].
+    Returns (next population as Fractions, parents, do-flags, cuts)."""
+    TAG_SELECT, TAG_XOVER, TAG_MUTATE = 1, 2, 3
+
+    def thr_hit(w, p):                                   # R0: hit = p >= 1 or w < floor(p 2^32), p the fp32 parameter
+        pf = Fraction(float(np.float32(p)))
+        return pf >= 1 or w < (pf * 2**32).numerator // (pf * 2**32).denominator
+
+    def upm1(w):
+        return Fraction((w >> 8) - 2**23, 2**23)
+
+    rows = [[Fraction(float(v)) for v in r] for r in pop]
+    nxt = [None] * P
+    for j in range(e):                                   # a8 (G17): e copies of the best, or the best e
+        nxt[j] = list(rows[order[j] if elite_mode == 1 else order[0]])
+    npairs = (P - e + 1) // 2
+    parents, dos, cuts = [], [], []
+    for q in range(npairs):
+        pa_pb = []
+        for s in (0, 1):                                 # a9 (R3): t draws, draw j = word j mod 4 of counter (j div 4, 2q+s, g, 1)
+            ranks = []
+            for j in range(t):
+                w = words(seed, j // 4, 2 * q + s, g, TAG_SELECT)[j % 4]
+                ranks.append((w * P) >> 32)
+            pa_pb.append(int(order[min(ranks)]))
+        w = words(seed, 0, q, g, TAG_XOVER)              # a10 (R5)
+        do = 1 if (K >= 2 and thr_hit(w[0], pc)) else 0
+        cut = 1 + ((w[1] * (K - 1)) >> 32) if K >= 2 else 0
+        a, b = rows[pa_pb[0]], rows[pa_pb[1]]
+        A = a[:cut] + b[cut:] if do else list(a)
+        B = b[:cut] + a[cut:] if do else list(b)
+        for child, slot in ((A, e + 2 * q), (B, e + 2 * q + 1)):
+            if slot >= P:                                # G19: an odd remainder drops the last B
+                continue
+            for k in range(K):                           # a11 (R6): counter (k, slot, g, 3)
+                w = words(seed, k, slot, g, TAG_MUTATE)
+                if thr_hit(w[0], pm):
+                    child[k] = upm1(w[1])
+            nxt[slot] = child
+        parents.append(pa_pb); dos.append(do); cuts.append(cut)
+    return nxt, parents, dos, cuts
+
+
+@pytest.mark.parametrize("P,K,t,e,elite_mode,pc,pm", [
+    (9, 7, 5, 2, 0, 0.9, 0.2),          # the paper's t-class with a second Philox block (draw 4 = word 0 of counter c0 = 1); odd children
+    (12, 5, 5, 3, 1, 0.5, 0.5),         # TOP_E elites
+    (6, 2, 3, 0, 0, 1.0, 0.05),         # K = 2: the only cut is 1; p_c = 1 always hits
+    (7, 4, 9, 1, 0, 0.3, 1.0),          # three Philox blocks per tournament; every gene mutated
+])
+def test_p18b_ga_step_decisions_by_hand(orc, aten_words, P, K, t, e, elite_mode, pc, pm):
+    """Which Philox word and counter feeds which decision (VERDICT r2 finding (i)): parents, do-flag, cut, mutation mask and
+    values and the elite copies of whole generations, derived from ATen's words in integer arithmetic and compared EXACTLY
+    with oracle_ga_step -- a w0/w1 swap, a transposed counter or a shifted slot index changes them."""
+    rng = np.random.default_rng(180 + P)
+    for seed, g in ((1, 0), (0xABCDEF0123456789, 3999), (2**64 - 1, 2**31 + 5)):
+        pop = rng.uniform(-1, 1, (P, K)).astype(np.float32)
+        fit = rng.random(P).astype(np.float32)
+        order = rng.permutation(P).astype(np.int32)
+        gp = orc.GaParams(P=P, tournament_size=t, elitism=e, elite_mode=elite_mode, selection=0, init_mode=1,
+                          p_crossover=pc, p_mutation=pm, stop_error=-1.0)
+        nxt, par, do, cut = orc.ga_step(gp, seed, g, order, fit, pop, debug=True)
+        exp, eparents, edos, ecuts = ga_step_by_hand(aten_words, seed, g, P, K, t, e, elite_mode, pc, pm, order, pop)
+        assert par.tolist() == eparents
+        assert do.tolist() == edos
+        assert [c for c, d in zip(cut.tolist(), edos) if d] == [c for c, d in zip(ecuts, edos) if d]
+        for p in range(P):
+            assert [Fraction(float(v)) for v in nxt[p]] == exp[p], (seed, g, p)
 
 
 def test_fl32_helper_is_ieee():
