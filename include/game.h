@@ -175,7 +175,11 @@ int game_fitness_host(game_ctx *ctx, const float *pop, int P, float *out);
  *   (once the stop test has fired, later asynchronous calls leave the population unchanged), and game_sync collects them.
  * game_sync: synchronises the stream and closes a run of asynchronous game_advance calls: res (HOST, may be NULL) gets
  *   the generations applied since the run began, whether the stop test fired, and the best error / index of the last
- *   evaluation.  Every other call that needs the host-side generation counter does this implicitly. */
+ *   evaluation.  Every other call that needs the host-side generation counter does this implicitly.  With NO run open
+ *   (no asynchronous game_advance since the last collection) there is nothing to report: res is filled with zeros, and its
+ *   best_error / best_index then carry no information (they are not a perfect fit at row 0).
+ * An asynchronous run may mix evaluation-only calls (apply_operators == 0, e.g. to log the fitness) with stepping ones:
+ *   the operators' random draws are keyed on the number of steps APPLIED, so the trajectory is the one game_evolve gives. */
 int game_fitness_sums(game_ctx *ctx, const float *pop, int P, double *sums, int accumulate);
 int game_advance(game_ctx *ctx, const double *sums, long long N_total, unsigned long long seed, const game_ga_params *params,
                  int apply_operators, game_result *res);

@@ -521,6 +521,11 @@ static int launch_persistent_variant(game_ctx *c, const CUtensorMap &tmC, const 
 {
     auto kern = evolve_persistent_kernel<ACT, TMSE>;
     GAME_CUDA(c, ensure_smem_attr(c, (const void *)kern, smem));
+    // a cooperative grid must be co-resident: ask how many CTAs of THIS variant fit (a shared-memory carve-out or a
+    // partitioned GPU can leave fewer than one per SM) and let the caller take the launch-per-kernel path if not
+    int per_sm = 0;
+    GAME_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, PERS_THREADS, (size_t)smem));
+    if ((long long)per_sm * c->sm_count < grid) return PERSISTENT_UNAVAILABLE;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3(PERS_THREADS);
@@ -530,7 +535,12 @@ static int launch_persistent_variant(game_ctx *c, const CUtensorMap &tmC, const 
     attr[0].id = cudaLaunchAttributeCooperative;
     attr[0].val.cooperative = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    GAME_CUDA(c, cudaLaunchKernelEx(&cfg, kern, tmC, tmE, a));
+    cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tmC, tmE, a);
+    if (le == cudaErrorCooperativeLaunchTooLarge) {      // SMs taken by someone else (MPS / green-context partition, a resident kernel)
+        cudaGetLastError();
+        return PERSISTENT_UNAVAILABLE;
+    }
+    GAME_CUDA(c, le);
     ++c->launches;
     return GAME_OK;
 }

@@ -395,8 +395,18 @@ int game_fitness_host(game_ctx *c, const float *pop, int P, float *out)
     const int want = pop_bytes >= ((size_t)8 << 20) ? 4 : pop_bytes >= ((size_t)1 << 20) ? 2 : 1;
     const int Pc = (((P + want - 1) / want + 255) / 256) * 256;
     // (a chunk must also be well above one wave of tiles, or the tensor path would switch to its half-size tiles for it)
-    const bool chunked = want > 1 && P >= 2048 && Pc >= 1024 && resolve_path(c, Pc) == resolve_path(c, P) &&
-                         (c->Npad256 / 256) * (long long)(Pc / 128) >= 2LL * c->sm_count;
+    // The same must hold for the ragged LAST chunk (it can be as short as one row, which would run single CTAs, the resident
+    // tile or half tiles, and could resolve AUTO's expansion differently): a tail that fails the test is folded into the
+    // chunk before it.
+    auto same_class = [&](int n) {
+        return n >= 1024 && resolve_path(c, n) == resolve_path(c, P) &&
+               (c->Npad256 / 256) * (long long)(n / 128) >= 2LL * c->sm_count &&
+               (resolve_path(c, P) != GAME_PATH_TENSOR || tensor_expansion(c, n) == tensor_expansion(c, P));
+    };
+    int cstart[8], ccount[8], nch = 0;
+    for (int p0 = 0; p0 < P && nch < 8; p0 += Pc, ++nch) { cstart[nch] = p0; ccount[nch] = P - p0 < Pc ? P - p0 : Pc; }
+    if (nch >= 2 && !same_class(ccount[nch - 1])) { ccount[nch - 2] += ccount[nch - 1]; --nch; }
+    const bool chunked = want > 1 && P >= 2048 && nch >= 2 && same_class(Pc);
     int rc = GAME_OK;
     if (!chunked) {
         GAME_CUDA(c, cudaMemcpyAsync(c->stage_pop, pop, (size_t)P * c->K * sizeof(float), cudaMemcpyHostToDevice, c->stream));
@@ -410,16 +420,15 @@ int game_fitness_host(game_ctx *c, const float *pop, int P, float *out)
         }
         GAME_CUDA(c, cudaEventRecord(c->copy_ev[0], c->stream));            // earlier work on the context's stream may still read the staging area
         GAME_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->copy_ev[0], 0));
-        int nch = 0;
-        for (int p0 = 0; p0 < P; p0 += Pc, ++nch) {
-            const int n = P - p0 < Pc ? P - p0 : Pc;
+        for (int i = 0; i < nch; ++i) {
+            const int p0 = cstart[i], n = ccount[i];
             GAME_CUDA(c, cudaMemcpyAsync(c->stage_pop + (size_t)p0 * c->K, pop + (size_t)p0 * c->K, (size_t)n * c->K * sizeof(float),
                                          cudaMemcpyHostToDevice, c->copy_stream));
-            GAME_CUDA(c, cudaEventRecord(c->copy_ev[1 + nch], c->copy_stream));
+            GAME_CUDA(c, cudaEventRecord(c->copy_ev[1 + i], c->copy_stream));
         }
         GAME_CUDA(c, cudaMemsetAsync(range, 0, 2 * sizeof(int), c->stream));
         for (int i = 0; i < nch && !rc; ++i) {
-            const int p0 = i * Pc, n = P - p0 < Pc ? P - p0 : Pc;
+            const int p0 = cstart[i], n = ccount[i];
             GAME_CUDA(c, cudaStreamWaitEvent(c->stream, c->copy_ev[1 + i], 0));
             rc = launch_max_abs(c, c->stage_pop + (size_t)p0 * c->K, (long long)n * c->K, range);
             if (!rc) rc = run_fitness(c, c->stage_pop + (size_t)p0 * c->K, n, c->stage_fit + p0, nullptr);
@@ -470,6 +479,7 @@ int game_advance(game_ctx *c, const double *sums, long long N_total, unsigned lo
         // gen_base_open + evals_done - 1, as the game_evolve loop does)
         GAME_CUDA(c, cudaMemsetAsync(c->state, 0, sizeof(DevState), c->stream));
         c->gen_base_open = (unsigned int)c->generation;
+        c->noop_evals_open = 0;
         c->loop_open = true;
     }
     rc = launch_fit_from_sums(c, sums, P, N_total, c->fit, c->state);                              // a5 tail
@@ -477,9 +487,16 @@ int game_advance(game_ctx *c, const double *sums, long long N_total, unsigned lo
     if (rc) return rc;
     if (apply_operators) {                                                                          // a8-a11
         const int path = resolve_path(c, P, true);
+        // the operators also write the next fitness call's fp16 copy: size it for THIS population first (the sums may come
+        // from elsewhere, so no fitness call of this context need have seen P chromosomes yet)
+        if (c->N > 0) { rc = ensure_scratch(c, P); if (rc) return rc; }
         C16Sink sink = tensor_sink(c, path == GAME_PATH_TENSOR_SPLIT);
-        const bool with_sink = (path == GAME_PATH_TENSOR || path == GAME_PATH_TENSOR_SPLIT) && sink.ptr != nullptr && c->N > 0;
-        rc = launch_ga_step(c, gp, seed, c->gen_base_open, c->order, c->fit, c->pop, c->pop_next, c->state, c->rw,
+        const size_t need16 = (size_t)((P + 255) / 256) * 256 * (size_t)c->Kpad;
+        const bool sink_fits = sink.split ? c->c16s_cap >= 3 * need16 : c->c16_cap >= need16;
+        const bool with_sink = (path == GAME_PATH_TENSOR || path == GAME_PATH_TENSOR_SPLIT) && sink.ptr != nullptr && sink_fits && c->N > 0;
+        // generation key of the operators = gen_base + (evaluations done - 1) on the device; evaluation-only calls inside this
+        // run (apply_operators == 0) count as evaluations but apply nothing, so the base steps back by their number
+        rc = launch_ga_step(c, gp, seed, c->gen_base_open - c->noop_evals_open, c->order, c->fit, c->pop, c->pop_next, c->state, c->rw,
                             c->rprefix, with_sink ? &sink : nullptr);
         if (rc) return rc;
         float *tmp = c->pop; c->pop = c->pop_next; c->pop_next = tmp;
@@ -487,6 +504,7 @@ int game_advance(game_ctx *c, const double *sums, long long N_total, unsigned lo
         c->have_fit = false;       // (if the stop test fired the population did not move, but the host cannot know yet)
     } else {
         c->have_fit = true;
+        ++c->noop_evals_open;
     }
     if (!res) return GAME_OK;      // asynchronous: game_sync (or any call that needs the counters) collects later
     return close_loop(c, res);
@@ -531,7 +549,33 @@ int game_set_population(game_ctx *c, const float *pop, int P)
     if (!pop || P < 2) return fail(c, GAME_ERR_INVALID_ARG, "game_set_population: pop NULL or P < 2");
     DeviceGuard dg(c);
     GAME_CLOSE_LOOP(c);
-    int rc = ensure_population(c, P);
+    int rc;
+    if ((size_t)P > c->pop_cap && c->have_pop) {
+        // growing means reallocating, which frees the installed population: check the newcomer in a buffer of its own first,
+        // so that a rejected one (NaN / Inf genes, genes too large for the requested tensor path) leaves the old one in place
+        float *probe = nullptr;
+        const size_t n = (size_t)P * c->K;
+        GAME_CUDA(c, cudaMalloc(&probe, (n + 2) * sizeof(float)));
+        int *prange = reinterpret_cast<int *>(probe + n);
+        int hp[2] = {0, 0};
+        cudaError_t e = cudaMemcpyAsync(probe, pop, n * sizeof(float), cudaMemcpyDefault, c->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(prange, 0, 2 * sizeof(int), c->stream);
+        rc = e == cudaSuccess ? launch_max_abs(c, probe, (long long)n, prange) : cuda_fail(c, e, "game_set_population: staging copy");
+        if (!rc) {
+            e = cudaMemcpyAsync(hp, prange, sizeof(hp), cudaMemcpyDeviceToHost, c->stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+            if (e != cudaSuccess) rc = cuda_fail(c, e, "game_set_population: staging check");
+        }
+        cudaFree(probe);
+        if (rc) return rc;
+        float pmx;
+        memcpy(&pmx, &hp[1], sizeof(float));
+        if (hp[0]) return fail(c, GAME_ERR_NONFINITE_INPUT, "game_set_population: genes contain NaN/Inf");
+        if (pmx > 65504.0f && (c->path == GAME_PATH_TENSOR || c->path == GAME_PATH_TENSOR_SPLIT))
+            return fail(c, GAME_ERR_UNSUPPORTED, "game_set_population: |gene| > 65504 cannot be an fp16 operand of the requested tensor path; "
+                                                 "use GAME_PATH_FP32 or GAME_PATH_AUTO");
+    }
+    rc = ensure_population(c, P);
     if (rc) return rc;
     // gene range first (into the spare buffer): a rejected population leaves the installed one untouched
     int *range = reinterpret_cast<int *>(c->rank);          // P >= 2 ints, zero between uses (the rank kernels keep it so)
@@ -590,12 +634,18 @@ int game_evolve(game_ctx *c, int generations, unsigned long long seed, const gam
         // plus the final evaluation -- as ONE persistent cooperative kernel with grid barriers between the phases
         // (evolve_persistent.cu).  Bit-identical to the launch-per-kernel path below.
         const int path0 = resolve_path(c, P, true);
-        if (persistent_eligible(c, gp, path0)) {
+        const bool ran_persistent = persistent_eligible(c, gp, path0);
+        if (ran_persistent) {
             const bool split = path0 == GAME_PATH_TENSOR_SPLIT;
             rc = ensure_scratch(c, P);
             if (!rc) rc = tensor_refresh_c16(c, c->pop, P, split, nullptr);
             if (!rc) rc = launch_evolve_persistent(c, gp, seed, generations, path0);
-            if (rc) return rc;
+            if (rc > 0) return rc;
+        }
+        // (rc == PERSISTENT_UNAVAILABLE: the cooperative grid cannot be co-resident on this device right now; nothing ran, and
+        // the launch-per-kernel loop below gives the same bits)
+        if (ran_persistent && rc == GAME_OK) {
+            const bool split = path0 == GAME_PATH_TENSOR_SPLIT;
             GAME_CUDA(c, cudaMemcpyAsync(&h, c->state, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
             GAME_CUDA(c, cudaStreamSynchronize(c->stream));
             if (h.gens_run & 1) { float *tmp = c->pop; c->pop = c->pop_next; c->pop_next = tmp; }
@@ -611,6 +661,7 @@ int game_evolve(game_ctx *c, int generations, unsigned long long seed, const gam
             }
             return GAME_OK;
         }
+        rc = GAME_OK;
     }
     const bool can_stop = gp->stop_error >= 0.f;
     const unsigned int gen_base = (unsigned int)c->generation;      // the device adds its own evaluation counter

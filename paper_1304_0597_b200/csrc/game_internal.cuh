@@ -141,6 +141,7 @@ struct game_ctx {
     long long generation = 0;
     bool loop_open = false;                  // asynchronous game_advance calls pending: DevState counts since gen_base_open
     unsigned int gen_base_open = 0;
+    unsigned int noop_evals_open = 0;        // evaluation-only game_advance calls (apply_operators == 0) since the run opened
     float *pop = nullptr, *pop_next = nullptr, *fit = nullptr;
     int *order = nullptr, *rank = nullptr;
     unsigned int *rw = nullptr;              // roulette weights
@@ -278,6 +279,9 @@ int tensor_encode_population_map(game_ctx *ctx, bool split, int Ppad);          
 
 // evolve_persistent.cu: the whole loop as one cooperative kernel, for sub-wave problems
 bool persistent_eligible(const game_ctx *ctx, const game_ga_params *gp, int path);
+// returns GAME_OK, an error code (> 0), or PERSISTENT_UNAVAILABLE when the cooperative grid cannot be co-resident on the
+// device as it is now (nothing was launched: the caller runs the launch-per-kernel loop instead)
+constexpr int PERSISTENT_UNAVAILABLE = -1;
 int launch_evolve_persistent(game_ctx *ctx, const game_ga_params *gp, unsigned long long seed, int generations, int path);
 
 // ga.cu
