@@ -1,14 +1,15 @@
 #!/usr/bin/env python
 """bench.py -- GAME hot path on B200: chromosome x pattern fitness evaluations / second.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--repeats 5] [--config 5] [--impl ours|reference]
                   [--path auto|fp32|tensor|split] [--shard] [--no-cpu-baseline] [--peaks]
 
 A *step* is one generation of the whole hot path (fused fitness of every chromosome
 on every pattern, rank, stop test, elitism, selection, crossover, mutation) on the config's synthetic
 workload.  `game_evolve(K)` runs K such steps plus the final re-evaluation of the returned population
 (DESIGN G18); the timed region is exactly that call, so `value` counts (K+1)*N*P evaluations and
-`ms_per_step` = time / K (the final evaluation is charged to the steps).  Prints ONE JSON line.
+`ms_per_step` = time / K (the final evaluation is charged to the steps).  The region is timed --repeats times (default 5,
+SURVEY 8(d)) and the MEDIAN region is the headline; all regions are listed under `repeats`.  Prints ONE JSON line.
 The default workload is config 5, the largest (the one north_star quotes its roofline target on); --config picks the
 others.  At N > 1 every rank runs its own replica (weak scaling); --shard splits ONE problem's patterns over the ranks
 instead (one all-reduce of P doubles per generation, strong scaling).
@@ -44,18 +45,32 @@ def read_peaks():
     return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, sm_max_mhz=1965.0, source="fallback")
 
 
+KERNEL_SOURCES = {"tensor": ("fitness_tc.cu", "tc_common.cuh"), "fp32": ("fitness_fp32.cu",),
+                  "persistent": ("evolve_persistent.cu", "tc_common.cuh")}
+
+
+def kernel_source_hash(kind):
+    """sha256 (first 16 hex digits) of the CUDA source files the dominant kernel of this kind is compiled from."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES[kind]:
+        h.update(open(os.path.join(ROOT, "paper_1304_0597_b200", "csrc", name), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def ncu_traffic(w, path_name):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-    `ncu --set full` capture summarised in profiles/r02_traffic.csv / r01_traffic.csv (null when that config was not captured)."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the `ncu --set full` capture
+    summarised in profiles/r03_traffic.csv.  Every row carries the hash of the kernel sources it was captured on; a row
+    whose hash no longer matches the sources in this tree describes another kernel and is NOT reported (null), and
+    neither is a config that was not captured."""
     key = "%s/%s" % (w.name, path_name)
-    for name in ("r02_traffic.csv", "r01_traffic.csv"):          # the latest round's capture first
-        p = os.path.join(ROOT, "profiles", name)
-        if not os.path.exists(p):
-            continue
-        for line in open(p).read().splitlines()[1:]:
-            f = line.split(",")
-            if f[0] == key:
-                return float(f[1])
+    p = os.path.join(ROOT, "profiles", "r03_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    for line in open(p).read().splitlines()[1:]:
+        f = line.split(",")
+        if f[0] == key:
+            return float(f[1]) if len(f) >= 5 and kernel_source_hash(f[3]) == f[4] else None
     return None
 
 
@@ -103,13 +118,15 @@ class ClockSampler(threading.Thread):
                 pass
             time.sleep(0.01 if self.nv is not None else 0.1)
 
-    def summary(self):
-        if not self.samples:
+    def summary(self, lo=0, hi=None):
+        """Median / minimum clock, throttle reasons and peak power over samples[lo:hi] (default: all of them)."""
+        samples = self.samples[lo:hi]
+        if not samples:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["clock sampling unavailable"]}
-        sm = sorted(s[0] for s in self.samples)
-        reasons = [n for i, n in enumerate(self.NAMES) if any(s[3][i] for s in self.samples)]
-        return {"sm_mhz": sm[len(sm) // 2], "sm_min_mhz": sm[0], "sm_max_mhz": self.samples[0][1], "reasons": reasons,
-                "power_w_max": max(s[2] for s in self.samples), "samples": len(self.samples), "source": self.source}
+        sm = sorted(s[0] for s in samples)
+        reasons = [n for i, n in enumerate(self.NAMES) if any(s[3][i] for s in samples)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_min_mhz": sm[0], "sm_max_mhz": samples[0][1], "reasons": reasons,
+                "power_w_max": max(s[2] for s in samples), "samples": len(samples), "source": self.source}
 
 
 def workload_dict(w, path_name):
@@ -345,16 +362,29 @@ def run_ours(args, w):
         ctx.get_kernel_timing()
         sampler = ClockSampler(local)
         sampler.start()
-        barrier()
-        launches0 = ctx.launch_count()
-        e0.record(stream)
-        res = evolve(args.steps)                                # exactly K steps (+ the final re-evaluation)
-        e1.record(stream)
-        barrier()
+        # "median of 5 repeats".  The timed region -- exactly K steps between a barrier + synchronize on both
+        # sides -- is run `--repeats` times back to back in this one invocation (the evolution simply continues); the
+        # headline is the MEDIAN region, and every region's time, kernel time, clocks and power are printed beside it.
+        reps = []
+        for _ in range(max(args.repeats, 1)):
+            barrier()
+            s0 = len(sampler.samples)
+            launches0 = ctx.launch_count()
+            e0.record(stream)
+            res = evolve(args.steps)                            # exactly K steps (+ the final re-evaluation)
+            e1.record(stream)
+            barrier()
+            assert res.generations_run == args.steps
+            ms_r = e0.elapsed_time(e1)
+            k_ms, k_n = ctx.get_kernel_timing()
+            share = 1.0 / world if args.shard else 1.0         # sharded: the ranks split ONE job's evaluations
+            value_r, ms_max_r = replicas.job_throughput(float(w.N) * w.P * (args.steps + 1) * share, world, ms_r, "cuda")
+            reps.append(dict(ms=ms_r, ms_max=ms_max_r, value=value_r, kern_ms=k_ms, kern_n=k_n,
+                             launches=ctx.launch_count() - launches0, clocks=sampler.summary(s0, len(sampler.samples))))
         sampler.stop_flag = True
-        ms = e0.elapsed_time(e1)
-        launches = ctx.launch_count() - launches0
-        kern_ms, kern_n = ctx.get_kernel_timing()
+        med = sorted(reps, key=lambda r: r["ms_max"])[(len(reps) - 1) // 2]
+        ms, launches, kern_ms, kern_n = med["ms"], med["launches"], med["kern_ms"], med["kern_n"]
+        value, ms_max = med["value"], med["ms_max"]
         kern_pass_ms = ms
         if separate_pass:
             ctx.set_kernel_timing(True)
@@ -366,10 +396,6 @@ def run_ours(args, w):
             kern_ms, kern_n = ctx.get_kernel_timing()
         ctx.set_kernel_timing(False)
         sampler.join()
-        assert res.generations_run == args.steps
-
-        share = 1.0 / world if args.shard else 1.0             # sharded: the ranks split ONE job's evaluations
-        value, ms_max = replicas.job_throughput(float(w.N) * w.P * (args.steps + 1) * share, world, ms, "cuda")
 
         # e2e: the same metric through the C ABI with HOST buffers: population in, fitness out, every step
         pop_host, _, _ = ctx.get_population_host()
@@ -400,7 +426,8 @@ def run_ours(args, w):
     flops = 2.0 * (hi - lo) * w.K * w.P           # what ONE launch of this rank's kernel computes
     evals = float(hi - lo) * w.P
     avg_s = kern_ms * 1e-3 / max(kern_n, 1)
-    clocks = sampler.summary()
+    clocks = dict(med["clocks"])                 # the clock record of the region the headline comes from
+    clocks["all_repeats"] = sampler.summary()
     # Which tensor peak applies follows from THIS run's clock record: MEASURED_PEAKS.json holds a burst figure (best of 10
     # at full clock) and a sustained one (4 s back to back, power-capped to ~1357 MHz).  A timed region whose median SM
     # clock held >= 95 % of the maximum ran at burst clocks; anything else is compared with the sustained figure -- and if
@@ -464,6 +491,12 @@ def run_ours(args, w):
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms_max / args.steps, "generations_per_sec": args.steps / (ms_max * 1e-3),
+           "ms_per_step_min": min(r["ms_max"] for r in reps) / args.steps, "ms_per_step_max": max(r["ms_max"] for r in reps) / args.steps,
+           "timing": "median of %d timed regions of %d steps each, run back to back in this invocation" % (len(reps), args.steps),
+           "repeats": [{"ms_per_step": r["ms_max"] / args.steps, "value": r["value"],
+                        "kernel_ms_avg": (r["kern_ms"] / r["kern_n"]) if r["kern_n"] else None,
+                        "sm_mhz": r["clocks"].get("sm_mhz"), "sm_min_mhz": r["clocks"].get("sm_min_mhz"),
+                        "power_w_max": r["clocks"].get("power_w_max"), "reasons": r["clocks"].get("reasons")} for r in reps],
            "higher_is_better": True, "scaling": "strong" if args.shard else "weak", "vs_baseline": None,
            "dtype": {g.GAME_PATH_TENSOR: "f16 operands, f32 accumulate", g.GAME_PATH_TENSOR_SPLIT: "split f16 (hi+lo) operands, f32 accumulate",
                      g.GAME_PATH_FP32: "f32"}[path],
@@ -478,6 +511,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=400)
     ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--repeats", type=int, default=5, help="timed regions of --steps steps each; the headline is their median (SURVEY 8(d))")
     ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number (1-5); 5 = the largest, the one the north star's target is quoted on")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--path", default="auto", choices=["auto", "fp32", "tensor", "split"])

@@ -49,22 +49,6 @@ enum { GAME_ELITE_COPIES_OF_BEST = 0, GAME_ELITE_TOP_E = 1 };      /* L148; DESI
  * fp32-accumulate MMA (same 11-bit significand as TF32), 1e-3 class.  AUTO picks by problem shape. */
 enum { GAME_PATH_AUTO = 0, GAME_PATH_FP32 = 1, GAME_PATH_TENSOR = 2, GAME_PATH_TENSOR_SPLIT = 3 };
 enum { GAME_EXPAND_AUTO = 0, GAME_EXPAND_MATERIALIZED = 1, GAME_EXPAND_REGENERATED = 2 };
-/* Launch-configuration knobs of game_set_tuning: measurement aids, none changes what is computed beyond the stated
- * tolerance class.  value -1 restores the automatic choice.
- *   GAME_TUNE_PDL          1/0  programmatic dependent launch between the kernels of a generation (auto: 1)
- *   GAME_TUNE_CTA_GROUP    1/2  single CTAs or cta_group::2 pairs in the tensor kernel (auto: by shape)
- *   GAME_TUNE_SIGMOID      0 ex2+rcp logistic, 2 tanh.approx logistic (TENSOR path; auto: 2)
- *   GAME_TUNE_RESIDENT     1/0  resident population tile for P <= 256 (auto: 1)
- *   GAME_TUNE_TEAMS        1/0  two-team epilogue (auto: contraction depth <= 256)
- *   GAME_TUNE_HALF_TILES   1/0  128-pattern tiles for sub-wave problems (auto: by shape)
- *   GAME_TUNE_PERSISTENT   1/0  one persistent cooperative kernel per game_evolve for sub-wave problems (auto: by shape)
- *                          2 = the persistent kernel without its local-population form (every CTA holding the whole population)
- *   GAME_TUNE_RATIONAL_SHARE  0..8  of every 16 evaluation PAIRS of the tanh logistic, how many are evaluated on the FMA
- *                          pipe by a rational form with one shared reciprocal (team epilogue, single CTAs; 1, 2 round
- *                          up to 3; auto: the measured best) */
-enum { GAME_TUNE_PDL = 0, GAME_TUNE_CTA_GROUP = 1, GAME_TUNE_SIGMOID = 2, GAME_TUNE_RESIDENT = 3, GAME_TUNE_TEAMS = 4,
-       GAME_TUNE_HALF_TILES = 5, GAME_TUNE_PERSISTENT = 6, GAME_TUNE_RATIONAL_SHARE = 7, GAME_TUNE_COUNT_ = 8 };
-
 /* GA parameters (L275-L291).  Probabilities are per parent pair (crossover, DESIGN G15) and per gene
  * (mutation, DESIGN G16).  stop_error < 0 disables the error-threshold stop (L219, L287). */
 typedef struct {
@@ -129,8 +113,6 @@ int game_resolved_path(const game_ctx *ctx, int P);
  * requested one is unavailable. */
 int game_set_expansion(game_ctx *ctx, int mode);
 int game_resolved_expansion(const game_ctx *ctx, int P);
-/* Launch-configuration knob (GAME_TUNE_*), per context; unknown knobs / values give GAME_ERR_INVALID_ARG. */
-int game_set_tuning(game_ctx *ctx, int knob, int value);
 /* Pattern-sharded runs: the number of patterns of the WHOLE problem (all shards).  GAME_PATH_AUTO then picks the path from
  * it instead of this context's own N, so every shard evaluates in the same tolerance class.  0 = unset. */
 int game_set_global_patterns(game_ctx *ctx, long long N_total);
@@ -277,23 +259,8 @@ int game_philox(game_ctx *ctx, unsigned long long seed, const unsigned int *ctr,
 int game_rank_static(const float *fit, int P, int *order, void *cuda_stream);
 const char *game_rank_static_error(void);
 
-/* Number of kernels this context has launched since creation (bench.py reports it). */
-long long game_launch_count(const game_ctx *ctx);
-
-/* Measurement aid: while enabled, every launch of the dominant kernel (the fused contraction +
- * epilogue of game_fitness / game_evolve) is bracketed by CUDA events on the context's stream.
- * game_get_kernel_timing synchronises the stream, returns the summed duration in milliseconds and the
- * number of launches since the last call, and resets both.  HOST out pointers.  While enabled, game_evolve
- * issues its kernels one by one instead of replaying a captured CUDA graph (events cannot be timed inside one). */
-int game_set_kernel_timing(game_ctx *ctx, int enabled);
-int game_get_kernel_timing(game_ctx *ctx, double *total_ms, long long *launches);
-
-/* Measurement aid: register-only micro-benchmarks of the pipes the "alu" rooflines are quoted against, one
- * CTA per SM, timed with CUDA events on the context's stream; synchronises.  kind = GAME_PEAK_*; param = FMA instructions
- * per tanh for GAME_PEAK_TANH_MIX (0..8), ignored otherwise.  *ops_per_s (HOST) = fused multiply-adds (FFMA, FFMA2: count
- * both lanes) or special-function results per second over the whole GPU; *ms (HOST, may be NULL) = the timed launch. */
-enum { GAME_PEAK_FFMA = 0, GAME_PEAK_FFMA2 = 1, GAME_PEAK_TANH = 2, GAME_PEAK_EX2 = 3, GAME_PEAK_TANH_MIX = 4 };
-int game_microbench(game_ctx *ctx, int kind, int param, double *ops_per_s, double *ms);
+/* Measurement aids (kernel timing, launch counter, pipe micro-benchmarks, launch-configuration knobs) are NOT part of this
+ * API: they are declared in game_bench.h, which this header does not include. */
 
 #ifdef __cplusplus
 }

@@ -1,6 +1,7 @@
 """Thin ctypes binding over libgame_b200.so -- argument marshalling only.
 
-Every function has the name and meaning of the C entry point in ``include/game.h``; every step of
+Every function has the name and meaning of the C entry point in ``include/game.h`` (product API) or
+``include/game_bench.h`` (measurement aids); every step of
 the path runs in the library's CUDA kernels.  Device arrays are ``torch`` CUDA tensors (torch is used
 for device memory and streams only), host arrays are numpy.  There is no CPU fallback: if the
 library is missing or no CUDA device is present the calls raise.
@@ -26,7 +27,7 @@ GAME_EXPAND_AUTO, GAME_EXPAND_MATERIALIZED, GAME_EXPAND_REGENERATED = 0, 1, 2
 GAME_PEAK_FFMA, GAME_PEAK_FFMA2, GAME_PEAK_TANH, GAME_PEAK_EX2, GAME_PEAK_TANH_MIX = range(5)
 ERROR_NAMES = {1: "INVALID_ARG", 2: "NOT_LOADED", 3: "ALLOC", 4: "CUDA", 5: "UNSUPPORTED", 6: "NONFINITE_INPUT"}
 
-# every symbol include/game.h declares (tests check the library exports exactly these)
+# every symbol include/game.h and include/game_bench.h declare (tests check the library exports exactly these)
 SYMBOLS = [
     "game_create", "game_destroy", "game_num_terms", "game_generation", "game_last_error",
     "game_set_stream", "game_set_activation", "game_set_error", "game_set_path", "game_resolved_path",

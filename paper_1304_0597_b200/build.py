@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgame_b200.so")
 SOURCES = ["game_api.cu", "expand.cu", "fitness_fp32.cu", "fitness_tc.cu", "ga.cu", "peaks.cu", "evolve_persistent.cu", "rank_static.cu"]
-HEADERS = [os.path.join(CSRC, h) for h in ("game_internal.cuh", "tc_common.cuh", "ga_device.cuh")] + [os.path.join(HERE, "..", "include", "game.h")]
+HEADERS = [os.path.join(CSRC, h) for h in ("game_internal.cuh", "tc_common.cuh", "ga_device.cuh")] + [os.path.join(HERE, "..", "include", h) for h in ("game.h", "game_bench.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-cudart", "static"]
 

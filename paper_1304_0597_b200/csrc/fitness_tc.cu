@@ -801,19 +801,17 @@ int launch_fitness_tensor(game_ctx *ctx, const float *pop, int P, float *out, co
     // the split path is the 1e-5 tolerance class: its logistic is the ex2 + rcp form (2^-22), not tanh.approx (2^-11)
     const int mode = ctx->act == GAME_ACT_IDENTITY ? MODE_IDENTITY : (split ? MODE_SIG_EXACT : sigmoid_mode(ctx));
     // a share of the logistics on the FMA pipe (shallow contractions, where the special-function unit binds): pairs of 16
-    // per 32-column chunk; GAME_TUNE_RATIONAL_SHARE overrides (0 = none; 3..8 are built)
+    // per 32-column chunk; GAME_TUNE_RATIONAL_SHARE = 0 turns it off.  Only the measured best share (RATIONAL_SHARE_AUTO
+    // of every 16 pairs) is built: the sweep over 4..8 that found it lives in DESIGN.md section 7, not in the library.
     const int share_req = ctx->tune[GAME_TUNE_RATIONAL_SHARE];
-    const int share = (mode != MODE_SIG_TANH32 || !teams || cg != 1 || half_tiles) ? 0
-                    : share_req < 0 ? RATIONAL_SHARE_AUTO : share_req == 0 ? 0 : share_req < 3 ? 3 : share_req > 8 ? 8 : share_req;
+    const int share = (mode != MODE_SIG_TANH32 || !teams || cg != 1 || half_tiles || share_req == 0) ? 0 : RATIONAL_SHARE_AUTO;
     int rc = tensor_refresh_c16(ctx, pop, P, split, state);
     if (!rc) rc = tensor_encode_population_map(ctx, split, Ppad);
     if (rc) return rc;
 #define GAME_TC_SHARE(M, T, S) launch_variant<1, M, T, 8, SRC_TMA, GAME_TRIG, true, BN, (M == MODE_SIG_TANH32 ? S : 0)>(ctx, n_tiles, m_blocks, Ppad, state, split)
 #define GAME_TC_EW(CGV, M, T)                                                                              \
     rc = half_tiles ? launch_variant<1, M, T, 8, SRC_TMA, GAME_TRIG, true, 128>(ctx, n_tiles, m_blocks, Ppad, state, split)  \
-       : (teams && CGV == 1 && share > 0) ? (share == 4 ? GAME_TC_SHARE(M, T, 4) : share == 5 ? GAME_TC_SHARE(M, T, 5)        \
-                                             : share == 6 ? GAME_TC_SHARE(M, T, 6) : share == 7 ? GAME_TC_SHARE(M, T, 7)      \
-                                             : share == 8 ? GAME_TC_SHARE(M, T, 8) : GAME_TC_SHARE(M, T, 3))                  \
+       : (teams && CGV == 1 && share > 0) ? GAME_TC_SHARE(M, T, RATIONAL_SHARE_AUTO)                                          \
        : teams ? launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG, true>(ctx, n_tiles, m_blocks, Ppad, state, split)           \
                : launch_variant<CGV, M, T, 8, SRC_TMA, GAME_TRIG, false>(ctx, n_tiles, m_blocks, Ppad, state, split)
 #define GAME_TC_GEN(M, T)                                                                                  \

@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "../../include/game.h"
+#include "../../include/game_bench.h"   // measurement aids (tuning knobs, kernel timing, micro-benchmarks): not product API
 
 namespace game {
 

@@ -8,7 +8,12 @@ host processing and transfer times per (degree, size).  The catalogue is not ava
 synthetic stand-in of `workloads.paper_literal` (same shape, same replication construction).  Sizes map to rows
 as 0.15 MB <-> 2100 rows (the paper's own pairing).  On this library the whole loop runs on the device, so the
 columns are: LOAD = game_load_host (HtoD of X and targets + expansion, once), TRAIN = game_evolve(iterations)
-(fitness + rank + operators, no host round trips), TOT = both.  Prints a markdown table.
+(fitness + rank + operators, no host round trips), TOT = both.  These shapes (K = 2d+1 <= 17 terms, P = 23) are bound by
+HBM, so every row also gets its roofline: READ = the bytes the fitness kernel streams per generation (the fp32 expansion
+matrix K x N built once by game_load -- L254's hoisting -- plus the N targets), ALG = the algorithmic bytes (X and the
+targets: what a kernel regenerating the sums would read), GB/s = READ x generations / TRAIN, and that rate as a fraction
+of the measured HBM copy bandwidth (MEASURED_PEAKS.json, else the profiling guide's 6650 GB/s fallback).  Rows whose
+working set fits the 126 MB L2 can exceed the HBM figure; they are marked.  Prints a markdown table.
 """
 import argparse
 import sys
@@ -32,9 +37,14 @@ def main():
     import paper_1304_0597_b200 as g
     from paper_1304_0597_b200 import workloads as wl
 
+    import json
+    import os
+    peaks = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "MEASURED_PEAKS.json")
+    hbm_gbs = json.load(open(peaks))["hbm_gbs"] if os.path.exists(peaks) else 6650.0
+    print("HBM peak used: %.1f GB/s (%s)\n" % (hbm_gbs, "MEASURED_PEAKS.json" if os.path.exists(peaks) else "fallback of B200_PROFILING.md"))
     stream = torch.cuda.Stream()
-    print("| degree | size (MB) | rows | LOAD (s) | TRAIN (s) | TOT (s) | generations/s | evals/s | best TMSE |")
-    print("|---|---|---|---|---|---|---|---|---|")
+    print("| degree | size (MB) | rows | LOAD (s) | TRAIN (s) | TOT (s) | generations/s | evals/s | best TMSE | READ MB/gen | ALG MB/gen | GB/s | frac of HBM | frac (ALG) |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
     with torch.cuda.stream(stream):
         for d in [int(v) for v in args.degrees.split(",")]:
             for mb in [float(v) for v in args.sizes.split(",")]:
@@ -64,9 +74,14 @@ def main():
                 res = ctx.evolve(args.iterations, w.seed, gp)
                 t2 = time.perf_counter()
                 load, train = t1 - t0, t2 - t1
-                print("| %d | %g | %d | %.4f | %.3f | %.3f | %.0f | %.3e | %.4f |" % (
+                read_b = 4.0 * w.N * (ctx.K + 1)                # fp32 expansion matrix (K x N) + targets, once per evaluation
+                alg_b = 4.0 * w.N * (w.F + 1)                   # X + targets
+                gbs = read_b * (args.iterations + 1) / train / 1e9
+                print("| %d | %g | %d | %.4f | %.3f | %.3f | %.0f | %.3e | %.4f | %.1f | %.1f | %.0f | %.2f%s | %.2f |" % (
                     d, mb, w.N, load, train, load + train, args.iterations / train,
-                    float(w.N) * w.P * (args.iterations + 1) / train, res.best_error))
+                    float(w.N) * w.P * (args.iterations + 1) / train, res.best_error, read_b / 1e6, alg_b / 1e6, gbs,
+                    gbs / hbm_gbs, " (L2-resident)" if read_b < 126e6 else "",
+                    alg_b * (args.iterations + 1) / train / 1e9 / hbm_gbs))
                 sys.stdout.flush()
                 ctx.destroy()
                 del X, t, Xp, tp

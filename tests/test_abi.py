@@ -16,10 +16,21 @@ def lib():
     return binding.load_library()
 
 
-def _declared():
-    src = open(os.path.join(ROOT, "include", "game.h")).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(game_[a-z_]+)\s*\(", src)))
+def _declared(headers=("game.h", "game_bench.h")):
+    """every function the headers under include/ declare: the product API (game.h) and the measurement aids (game_bench.h)"""
+    names = set()
+    for h in headers:
+        src = open(os.path.join(ROOT, "include", h)).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        names |= set(re.findall(r"\b(game_[a-z_]+)\s*\(", src))
+    return sorted(names)
+
+
+def test_product_header_holds_no_measurement_aids():
+    api, src = _declared(("game.h",)), open(os.path.join(ROOT, "include", "game.h")).read()
+    for aid in ("game_microbench", "game_set_kernel_timing", "game_get_kernel_timing", "game_launch_count", "game_set_tuning"):
+        assert aid not in api
+    assert "GAME_TUNE_" not in re.sub(r"/\*.*?\*/", "", src, flags=re.S) and '#include "game_bench.h"' not in src
 
 
 def test_exports_every_declared_symbol(lib):

@@ -197,7 +197,8 @@ def test_fitness_host_matches_device(orc):
     check_fitness(orc, a, fam, d, X, t, pop, SIGMOID, TMSE, 0.49, ctx.resolved_path(P))
 
 
-@pytest.mark.parametrize("cfg,N,P", [(3, 20000, 20000), (3, 30000, 4096), (5, 6000, 5000), (2, None, 4100)])
+@pytest.mark.parametrize("cfg,N,P", [(3, 20000, 20000), (3, 30000, 4096), (5, 6000, 5000), (2, None, 4100),
+                                     (5, 12000, 3073)])      # four chunks of 1024 would leave a ONE-row tail: folded into the third
 def test_fitness_host_chunked_upload(orc, cfg, N, P):
     """game_fitness_host uploads populations of >= 2048 chromosomes in two (>= 1 MB) or four (>= 8 MB) chunks on a copy stream, a chunk ahead of the
     kernels; a chromosome's fitness does not depend on its row (P20), so the result equals the device call bit for bit --
@@ -320,7 +321,8 @@ def trajectory(orc, w, generations, full_check_every=1, subset=None, selection=0
     for gen in range(generations + 1):
         # (ii) fitness of the GPU's population within tolerance
         if gen % full_check_every == 0 or gen == generations:
-            rows = np.arange(w.P) if subset is None else np.sort(rng.choice(w.P, subset, replace=False))
+            rows = (np.arange(w.P) if subset is None else subset(gen, rng) if callable(subset)
+                    else np.sort(rng.choice(w.P, subset, replace=False)))
             check_fitness(orc, fit[rows], fam, d, X, t, pop[rows], w.act, w.err, w.R, path, "%s gen %d" % (w.name, gen))
         # (iii) the rank kernel sorted the GPU's own fitness bits exactly
         assert np.array_equal(order, orc.rank(fit)), gen
@@ -365,36 +367,57 @@ def test_trajectory_roulette_and_init_modes_at_scale(orc, cfg, init_mode, select
     trajectory(orc, w, 3, subset=48 if cfg == 3 else None, selection=selection, elite_mode=elite_mode)
 
 
-@pytest.mark.parametrize("cfg,generations,subset,check_every", [(3, 4, 24, 2), (4, 3, 6, 3), (5, 3, 8, 3)])
-def test_trajectory_full_size_big_configs(orc, cfg, generations, subset, check_every):
+def block_rows(P, rng, extra=0):
+    """One chromosome in EVERY block of 128 -- i.e. in both halves of every 256-chromosome CTA pair and in every single-CTA
+    block of the tensor kernels -- at a random position inside the block, plus `extra` random rows, plus the first and last."""
+    starts = np.arange(0, P, 128)
+    rows = starts + rng.integers(0, np.minimum(128, P - starts))
+    more = rng.choice(P, extra, replace=False) if extra else np.empty(0, dtype=np.int64)
+    return np.unique(np.concatenate([rows, more, [0, P - 1]])).astype(np.int64)
+
+
+def full_size_rows(cfg, P, rng, ends):
+    """the FULL population where the oracle can afford it (configs 3 and 4: all 4096 / all 256
+    chromosomes), every chromosome block otherwise (config 5: 64 blocks of 128 + 64 random rows), at the generations where
+    `ends` is true (first and last); a random subset of 64 at the generations between."""
+    if not ends:
+        return np.sort(rng.choice(P, min(64, P), replace=False))
+    return np.arange(P) if cfg in (3, 4) else block_rows(P, rng, extra=64)
+
+
+@pytest.mark.parametrize("cfg,generations", [(3, 4), (4, 3), (5, 3)])
+def test_trajectory_full_size_big_configs(orc, cfg, generations):
     """SURVEY 8(c) c.4 / 8(g).3 at FULL size on configs 3 (tournament), 4 and 5, in bench.py's launch configuration
     (context on its own stream, AUTO path): every generation (iii) the rank is the exact sort of the GPU's fitness bits and
     (iv) oracle.ga_step from the GPU's order reproduces the GPU's next population (P x K genes) bit for bit; (ii) the
-    fitness of a chromosome sample is checked against the oracle at the first and last generation (the oracle needs
-    ~10 s per evaluation at these N x K; the operators cost P x K Philox calls, under a second).  PAPER.md L217-L220 (the
-    loop), L286-L291 (the operators' parameters)."""
+    oracle's fitness against the GPU's for the WHOLE population (configs 3, 4) or a chromosome in every 128-chromosome block,
+    both halves of every CTA pair (config 5), at generation 0 and at the last one, and for 64 random chromosomes at every
+    generation between (full_size_rows).  PAPER.md L217-L220 (the loop), L286-L291 (the operators' parameters); the paper's
+    own validation is this kind of whole-run cross-check between implementations (L299, L324)."""
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
-        ctx, pop, fit, order = trajectory(orc, wl.config(cfg), generations, full_check_every=check_every, subset=subset,
-                                          stream=stream)
+        w = wl.config(cfg)
+        ctx, pop, fit, order = trajectory(orc, w, generations, full_check_every=1, stream=stream,
+                                          subset=lambda gen, rng: full_size_rows(cfg, w.P, rng, gen in (0, generations)))
     assert ctx.generation() == generations
 
 
 FULL_MODES = [(SIGMOID, MSE, 0.0), (SIGMOID, TMSE, 0.49), (SIGMOID, RMSE, 0.0), (IDENTITY, MSE, 0.0), (IDENTITY, RMSE, 0.0)]
 
 
-@pytest.mark.parametrize("cfg,nsample", [(1, 20), (2, 16), (3, 12), (4, 4), (5, 4)])
-def test_full_size_all_error_and_activation_modes(orc, cfg, nsample):
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_full_size_all_error_and_activation_modes(orc, cfg):
     """fitness parity with MSE, TMSE, RMSE and with the identity activation on EVERY config at its full N and
-    P, in the launch configuration bench.py times (AUTO path, full population in one call); the oracle evaluates a sample
-    of the chromosomes (rows of the same launch)."""
+    P, in the launch configuration bench.py times (AUTO path, full population in one call).  The oracle evaluates the
+    whole population on configs 1-4 (config 4: in the paper's mode TMSE and in identity / RMSE; the other three modes on
+    a chromosome of every block) and a chromosome of every 128-chromosome block plus 64 random ones on config 5."""
     w = wl.config(cfg)
     fam, d = w.family, w.degree
     X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
     rng = np.random.default_rng(100 + cfg)
     pop_s = wl.uniform_population(w.P, w.K, w.seed)
     pop_i = (pop_s / np.sqrt(w.K)).astype(np.float32)            # identity output: keep z = O(1)
-    rows = np.unique(np.concatenate([[0, w.P - 1], rng.choice(w.P, nsample, replace=False)]))
+    all_rows, some_rows = np.arange(w.P), block_rows(w.P, rng, extra=min(64, w.P // 2))
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
         ctx = g.Game(fam, d, w.F, stream=stream)
@@ -406,6 +429,7 @@ def test_full_size_all_error_and_activation_modes(orc, cfg, nsample):
             pop = pop_s if act == SIGMOID else pop_i
             got = ctx.fitness(dev(pop)).cpu().numpy()
             assert np.all(np.isfinite(got))
+            rows = some_rows if cfg == 5 or (cfg == 4 and (act, err) not in ((SIGMOID, TMSE), (IDENTITY, RMSE))) else all_rows
             check_fitness(orc, got[rows], fam, d, X, t, pop[rows], act, err, R, path,
                           "%s full size act %d err %d" % (w.name, act, err))
 
@@ -483,6 +507,33 @@ def test_full_size_sampled(orc, cfg, nsample, want_path):
     # properties that hold at any size: elites are copies of the previous winner -> rows 0,1 identical
     assert np.array_equal(pop[0], pop[1]) and fit[0] == fit[1]
     assert np.all(np.abs(pop) <= 1.0) and np.all(np.isfinite(fit)) and np.all(fit >= 0)
+
+
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_size_position_independence_and_split_crosscheck(orc, cfg):
+    """Two whole-population checks at FULL size that need no oracle time:
+    (P20) a chromosome's fitness does not depend on its row or on its neighbours -- the fitness of a randomly permuted
+    population is the permuted fitness, bit for bit, for all P; a defect tied to a chromosome block, a CTA-pair half or a
+    `partial` row offset would break it;  and the one-pass fp16 TENSOR result of every chromosome agrees with the
+    TENSOR_SPLIT result (the 1e-5 class, a different kernel variant and operand layout) within the 1e-3 class."""
+    w = wl.config(cfg)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    pop = wl.uniform_population(w.P, w.K, 31 + cfg)
+    perm = np.random.default_rng(cfg).permutation(w.P)
+    ctx = make_ctx(fam, d, X, t, SIGMOID, MSE)
+    assert ctx.resolved_path(w.P) == g.GAME_PATH_TENSOR
+    f = ctx.fitness(dev(pop)).cpu().numpy()
+    fp = ctx.fitness(dev(pop[perm])).cpu().numpy()
+    assert np.array_equal(fp.view(np.uint32), f[perm].view(np.uint32))
+    ctx.set_path(g.GAME_PATH_TENSOR_SPLIT)
+    assert ctx.resolved_path(w.P) == g.GAME_PATH_TENSOR_SPLIT
+    fs = ctx.fitness(dev(pop)).cpu().numpy().astype(np.float64)
+    rtol, atol, _ = TOL[g.GAME_PATH_TENSOR]
+    bad = np.abs(f - fs) > rtol * np.abs(fs) + atol
+    assert not bad.any(), (int(bad.sum()), float(np.abs(f - fs).max()))
+    fsp = ctx.fitness(dev(pop[perm])).cpu().numpy()
+    assert np.array_equal(fsp.view(np.uint32), fs.astype(np.float32)[perm].view(np.uint32))
 
 
 # ---- SURVEY 8(f) NEXT-2: the paper-literal tied-coefficient models ------------------------------------------
@@ -1069,3 +1120,83 @@ def test_persistent_loop_stop_criterion(orc):
     pb, fb, ob = ref2.get_population_host()
     assert np.array_equal(pa.view(np.uint32), pb.view(np.uint32)) and np.array_equal(fa.view(np.uint32), fb.view(np.uint32))
     assert np.array_equal(oa, ob)
+
+
+# ---- round 3: boundary corners ----------------------------------------------------------------------------------
+def _bits_equal_state(a, b):
+    pa, fa, oa = a.get_population_host()
+    pb, fb, ob = b.get_population_host()
+    assert np.array_equal(pa.view(np.uint32), pb.view(np.uint32))
+    assert np.array_equal(fa.view(np.uint32), fb.view(np.uint32)) and np.array_equal(oa, ob)
+
+
+def test_advance_on_a_population_larger_than_any_fitness_call_saw(orc):
+    """game_advance's operators also write the fp16 copy the next tensor-path fitness call reads.  That buffer used to be
+    sized by fitness calls only: a context that had evaluated 64 chromosomes, then got 1024 installed and was advanced with
+    totals computed ELSEWHERE (another context, another rank) wrote past its end.  Now game_advance sizes it itself: the
+    step and the evaluation after it equal game_evolve's, bit for bit (L217-L220)."""
+    w = wl.config(3).scaled(N=20000, P=1024)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    gp = g.ga_params(P=w.P)
+    pop = dev(wl.uniform_population(w.P, w.K, 6))
+    a = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    assert a.resolved_path(w.P) == g.GAME_PATH_TENSOR
+    a.fitness(dev(wl.uniform_population(64, w.K, 5)))            # scratch sized for 64 chromosomes
+    a.set_population(pop)
+    other = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    other.set_population(pop)
+    sums = other.fitness_sums(None, w.P)                         # the totals come from another context
+    res = a.advance(sums, X.shape[0], w.seed, gp, True, sync=True)
+    assert res.generations_run == 1
+    a.evolve(0, w.seed, gp)                                      # evaluates from the fp16 copy the operators wrote
+    ref = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    ref.set_population(pop)
+    ref.evolve(1, w.seed, gp)
+    _bits_equal_state(a, ref)
+
+
+def test_async_evaluation_only_calls_inside_a_run_keep_the_trajectory(orc):
+    """An asynchronous run may evaluate without stepping (apply_operators = 0, e.g. to log the fitness) between steps.  The
+    operators' Philox draws are keyed on the steps APPLIED (DESIGN R3-R6), not on the evaluations made, so the trajectory is
+    game_evolve's -- and so is the next run's, which must not reuse a generation key."""
+    w = wl.config(1)
+    fam, d = w.family, w.degree
+    X, t, _ = wl.make(w, lambda X, c: orc.forward(fam, d, X, c))
+    gp = g.ga_params(P=w.P)
+    N = X.shape[0]
+    ref = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    a = make_ctx(fam, d, X, t, w.act, w.err, w.R)
+    ref.evolve(0, w.seed, gp)
+    a.evolve(0, w.seed, gp)
+    sums = torch.empty(w.P, dtype=torch.float64, device="cuda")
+    for steps, logs in ((6, (0, 2, 3)), (5, (4,))):
+        ref.evolve(steps, w.seed, gp)
+        for k in range(steps):
+            a.fitness_sums(None, w.P, out=sums)
+            if k in logs:
+                a.advance(sums, N, w.seed, gp, False, sync=False)        # evaluation only, in the middle of the run
+            a.advance(sums, N, w.seed, gp, True, sync=False)
+        a.fitness_sums(None, w.P, out=sums)
+        a.advance(sums, N, w.seed, gp, False, sync=False)                # the returned fitness belongs to the returned population
+        res = a.sync()
+        assert res.generations_run == steps and a.generation() == ref.generation()
+        _bits_equal_state(a, ref)
+
+
+def test_set_population_rejected_while_growing_keeps_the_installed_one():
+    """A population that needs larger buffers is checked BEFORE the old buffers are given up: NaN genes are refused and
+    the population installed before is still there, unchanged."""
+    ctx = g.Game(CHEB, 3, 2)
+    old = dev(wl.uniform_population(8, ctx.K, 1))
+    ctx.set_population(old)
+    bad = wl.uniform_population(64, ctx.K, 2)
+    bad[40, 3] = np.nan
+    with pytest.raises(g.GameError) as e:
+        ctx.set_population(dev(bad))
+    assert e.value.code == 6
+    assert ctx.population_size() == 8
+    got, _, _ = ctx.get_population(want_fit=False)
+    assert torch.equal(got.view(torch.int32), old.view(torch.int32))
+    ctx.set_population(dev(wl.uniform_population(64, ctx.K, 3)))      # a clean one of that size is accepted
+    assert ctx.population_size() == 64
