@@ -199,10 +199,13 @@ evolve_persistent_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_c
             if (e == 0) mbar_wait(bfull_bar, 0);
             if (!a.local) mbar_wait(afull_bar, (uint32_t)(e & 1));      // (local mode: the tile was written before the CTA barrier)
             tc_fence_after();
+            int kr = 0;                                  // k-block inside the current K range (wrap counter: no division on the issue path)
             for (int kb = 0; kb < k_blocks; ++kb) {      // the launch path's k order, whatever block the data sits in
                 const int ja = kb < nres ? kb : kb - nres, jb = kb < kb1 ? kb : kb - kb1;
                 const uint64_t adesc = make_smem_desc(baseA + ja * PERS_KB_BYTES), bdesc = make_smem_desc(baseB + jb * PERS_KB_BYTES);
-                const int nk = (kb + 1) % kb1 == 0 ? a.k_last : BKB / UMMA_K;     // the last block of each K range ends in padding
+                const bool range_end = ++kr == kb1;
+                if (range_end) kr = 0;
+                const int nk = range_end ? a.k_last : BKB / UMMA_K;               // the last block of each K range ends in padding
                 if (elect_one()) {
 #pragma unroll
                     for (int k = 0; k < BKB / UMMA_K; ++k)

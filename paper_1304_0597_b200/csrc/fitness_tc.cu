@@ -335,6 +335,7 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                     mbar_wait<SUSP>(tempty_bar(acc), aph ^ 1);          // epilogue has drained this accumulator
                     tc_fence_after();
                     const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BNT);
+                    int kr = 0;                                         // k-block inside the current K range (wrap counter)
                     for (int kb = 0; kb < k_blocks; ++kb) {
                         mbar_wait<SUSP>(full_bar(s), ph);               // operands have landed (SRC_GEN: were generated)
                         tc_fence_after();
@@ -342,7 +343,12 @@ fitness_tc_kernel(const __grid_constant__ CUtensorMap tmC, const __grid_constant
                         const uint32_t sb = RESIDENT_A ? base + k_blocks * A_BYTES + s * GEN_B_BYTES : sa + A_BYTES;
                         const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sb);
                         const bool last = kb + 1 == k_blocks;
-                        const int nk = (kb + 1) % kb_range == 0 ? k_last : BKB / UMMA_K;      // padding steps would multiply zeros
+                        // the last k-block of a K range stops at its real k-steps: padding steps would multiply zeros.  A wrap
+                        // counter, NOT (kb + 1) % kb_range: the integer division by a run-time value sat on the issue path of
+                        // every k-block and cost config 5 7 % (2.17 vs 2.01 ms, same box: profiles/r03_ab_cfg5.md)
+                        const bool range_end = ++kr == kb_range;
+                        if (range_end) kr = 0;
+                        const int nk = range_end ? k_last : BKB / UMMA_K;
                         if (elect_one()) {
     #pragma unroll
                             for (int k = 0; k < BKB / UMMA_K; ++k) {
